@@ -1,0 +1,259 @@
+"""CPU fp64 oracle for the hierarchical reduced-basis matched filter (arXiv:2110.13115).
+
+THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only `tests/`,
+`__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` / `--impl reference`
+legs may import it.  It shares no code with the CUDA path (numpy only, no import
+of `paper_2110_13115_b200`), and takes the very arrays the library receives
+(complex64 strain / basis / coefficients, float32 sigma), promoted to fp64 and
+treated as exact.
+
+It follows the paper step by step, in the paper's order, with no blocking,
+fusion or reordering.  The method is not an exact-result accelerator (basis
+truncation and the binned first stage change which samples become triggers,
+PAPER.md:184-193), so "correct" = this algorithm, not the flat template search.
+
+Notation (the discrete normalisation is reading R2 in
+DESIGN.md because PAPER.md Eq. 4 is continuous):
+  N samples, bins j = 0..N/2, band B = [j_low, N/2)
+  d[j]   = unnormalised forward DFT of the whitened unit-variance series  (s~/sqrt(S_n))
+  b_k[j] = orthonormal reduced basis (p~_k), c_tk = decomposition coefficients
+  h'_t   = sum_k c_tk b_k
+  rho_t[n] = (s/sigma_t) sum_{j in B} d[j] conj(h'_t[j]) exp(+2 pi i j n/N),  s = sqrt(2/N)   (Eq. 4)
+  beta_k[n] = s sum_{j in B} d[j] conj(b_k[j]) exp(+2 pi i j n/N)
+  rho_t[n] = (1/sigma_t) sum_k conj(c_tk) beta_k[n]                                             (Eq. 7)
+  avg:  rho_bar_t[i] = (1/w) sum_{r<w} rho_t[i w + r]                                           (Eq. 9)
+  candidates C = {(t,i): |rho_bar_t[i]| >= thr1};  triggers = {(t,n): (t, n//w) in C, |rho_t[n]| >= thr2}
+
+Pins (tests/test_oracle_pins.py, all `-m "not gpu"`):
+  normalisation / FFT sign     brute-force time-domain circular correlation at small N; noise-free
+                               injection of optimal SNR A peaks at exactly A e^{i phi} at n0
+  direct-DFT vs FFT route      `snr_series_direct` (literal sum) vs `snr_series_fft` (numpy ifft)
+  reduced-basis identity       Eq. 7 == Eq. 4 with the full basis
+  truncation identity          Eq. 8
+  averaging                    Eq. 12 alias-fold route (`averaged_series_eq12`) == binned mean; w=1 => flat
+  thresholds / sets            independent pure-Python enumeration on tiny inputs
+  cost model                   Eq. 13-14 reproduce the paper's quoted ~6x / ~10x (tests/golden/paper_values.txt)
+Parity status: every function below is pinned by at least one of these; nothing is "parity unpinned".
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+
+
+# --------------------------------------------------------------------------- band
+def band(N: int, fs: float, f_low: float):
+    """Band B = [j_low, N/2): DC..j_low-1 and the Nyquist bin are ignored."""
+    j_low = int(math.ceil(f_low * N / fs - 1e-12))
+    return j_low, N // 2
+
+
+# ------------------------------------------------------------------ reconstruction
+def reconstructed_templates(coeffs, basis, idx=None):
+    """h'_t[j] = sum_k c_tk b_k[j].  Returns (len(idx), bins) complex128."""
+    C = np.asarray(coeffs, dtype=np.complex128)
+    if idx is not None:
+        C = C[np.atleast_1d(idx)]
+    return C @ np.asarray(basis, dtype=np.complex128)
+
+
+# ------------------------------------------------------------- SNR series, Eq. 4
+def snr_series_direct(d, h, sigma, N, j_low, n_chunk=256):
+    """rho[n] = (s/sigma) sum_{j in B} d[j] conj(h[j]) e^{+2 pi i j n / N}, evaluated literally
+    (direct O(N |B|) DFT; Eq. 4, discretised).  One template.  For small N."""
+    d = np.asarray(d, dtype=np.complex128)
+    h = np.asarray(h, dtype=np.complex128)
+    j = np.arange(j_low, N // 2, dtype=np.int64)
+    g = d[j] * np.conj(h[j])
+    s = math.sqrt(2.0 / N)
+    out = np.empty(N, dtype=np.complex128)
+    for a in range(0, N, n_chunk):
+        n = np.arange(a, min(N, a + n_chunk), dtype=np.int64)
+        ph = ((j[None, :] * n[:, None]) % N).astype(np.float64) * (2.0 * math.pi / N)  # exact index reduction
+        out[a:a + len(n)] = (np.exp(1j * ph) * g[None, :]).sum(axis=1)
+    return out * (s / float(sigma))
+
+
+def snr_point(d, h, sigma, N, j_low, n):
+    """rho[n] at one sample n by the literal O(|B|) sum of Eq. 4."""
+    d = np.asarray(d, dtype=np.complex128)
+    h = np.asarray(h, dtype=np.complex128)
+    j = np.arange(j_low, N // 2, dtype=np.int64)
+    ph = ((j * int(n)) % N).astype(np.float64) * (2.0 * math.pi / N)
+    return complex((d[j] * np.conj(h[j]) * np.exp(1j * ph)).sum() * (math.sqrt(2.0 / N) / float(sigma)))
+
+
+def snr_series_fft(d, h, sigma, N, j_low):
+    """Same series as `snr_series_direct`, the inverse DFT taken by numpy's FFT
+    ("The SNR as a function of time can be obtained efficiently by performing an inverse FFT").
+    `h` may be (bins,) or (M, bins); `sigma` scalar or (M,).  Returns (N,) or (M, N) complex128."""
+    d = np.asarray(d, dtype=np.complex128)
+    h = np.asarray(h, dtype=np.complex128)
+    one = h.ndim == 1
+    h2 = np.atleast_2d(h)
+    g = np.zeros((h2.shape[0], N), dtype=np.complex128)
+    g[:, j_low:N // 2] = d[None, j_low:N // 2] * np.conj(h2[:, j_low:N // 2])
+    rho = np.fft.ifft(g, axis=1) * N                      # unnormalised inverse DFT, e^{+2 pi i j n/N}
+    rho *= (math.sqrt(2.0 / N) / np.atleast_1d(np.asarray(sigma, dtype=np.float64)))[:, None]
+    return rho[0] if one else rho
+
+
+# ------------------------------------------------- reduced-basis route, Eq. 6 and 7
+def basis_series(d, basis, N, j_low):
+    """beta_k[n] = s sum_{j in B} d[j] conj(b_k[j]) e^{+2 pi i j n/N}.  (k, N) complex128."""
+    k = np.asarray(basis).shape[0]
+    return snr_series_fft(d, basis, np.ones(k), N, j_low)
+
+
+def snr_series_rb(beta, coeffs_t, sigma_t):
+    """rho_r[n] = (1/sigma_t) sum_k conj(c_tk) beta_k[n]  (Eq. 7)."""
+    c = np.asarray(coeffs_t, dtype=np.complex128)
+    return (np.conj(c)[None, :] @ np.asarray(beta, dtype=np.complex128))[0] / float(sigma_t)
+
+
+def truncation_loss(singular_values, p):
+    """<delta rho / rho> = 1 - sum_{k<p} sigma_k^2 / sum_k sigma_k^2  (Eq. 8)."""
+    s2 = np.asarray(singular_values, dtype=np.float64) ** 2
+    return 1.0 - s2[:p].sum() / s2.sum()
+
+
+# ------------------------------------------------------------------ averaging, Eq. 9
+def bin_average(series, w):
+    """x_avg[i] = (1/w) sum_{j<w} x[i w + j]  (Eq. 9): mean of the COMPLEX series over
+    non-overlapping bins aligned at sample 0.  Works on the last axis."""
+    x = np.asarray(series)
+    n = x.shape[-1]
+    if n % w:
+        raise ValueError("w must divide N")
+    return x.reshape(x.shape[:-1] + (n // w, w)).sum(axis=-1) / w
+
+
+def averaged_series_eq12(d, h, sigma, N, j_low, w):
+    """Averaged SNR series by the paper's fast first stage (Eq. 10-12):
+    Omega(f') = sum_{l<w} G[l N/w + f'] S(l N/w + f'),  S(f) = (1/w) sum_{r<w} e^{2 pi i f r/N},
+    rho_bar[b] = sum_{f'<N/w} e^{2 pi i f' b/(N/w)} Omega(f')  -- an inverse DFT of length N/w.
+    (Eq. 12 as printed is garbled; this is Eq. 10 with Eq. 11 substituted, reading R14 in DESIGN.md.)"""
+    d = np.asarray(d, dtype=np.complex128)
+    h = np.asarray(h, dtype=np.complex128)
+    G = np.zeros(N, dtype=np.complex128)
+    G[j_low:N // 2] = d[j_low:N // 2] * np.conj(h[j_low:N // 2])
+    G *= math.sqrt(2.0 / N) / float(sigma)
+    f = np.arange(N, dtype=np.int64)
+    S = np.zeros(N, dtype=np.complex128)
+    for r in range(w):
+        S += np.exp(2j * math.pi * ((f * r) % N) / N)
+    S /= w
+    M = N // w
+    Omega = (G * S).reshape(w, M).sum(axis=0)             # f = l*M + f'
+    return np.fft.ifft(Omega) * M
+
+
+# --------------------------------------------------------------- thresholds and sets
+def candidates_from_avg(rho_bar, thr1):
+    """First-stage triggers: bins whose averaged SNR modulus is >= thr1."""
+    return np.nonzero(np.abs(rho_bar) >= thr1)[0]
+
+
+def hierarchical_triggers_one(rho, w, thr1, thr2):
+    """Both stages for one template's full series `rho` (N,): returns (cand_bins, trig_n, flat_n, rho_bar).
+    Stage 2 = every sample inside the triggering bins, thresholded at thr2."""
+    rho_bar = bin_average(rho, w)
+    cand = candidates_from_avg(rho_bar, thr1)
+    mod = np.abs(rho)
+    flat = np.nonzero(mod >= thr2)[0]
+    in_cand = np.zeros(len(rho_bar), dtype=bool)
+    in_cand[cand] = True
+    trig = flat[in_cand[flat // w]]
+    return cand, trig, flat, rho_bar
+
+
+def oracle_filter(strain, basis, coeffs, sigma, N, fs, f_low, w, thr1, thr2, templates=None, chunk=64,
+                  keep_margins=True):
+    """The whole hot path for the listed templates (default all), template route:
+    h'_t -> rho_t (Eq. 4 by FFT) -> rho_bar_t (Eq. 9) -> thr1 -> thr2.
+
+    Returns dict with
+      triggers   structured array (template, time, re, im, avg_abs) sorted by (template, time)
+                 avg_abs = |rho_bar| of the bin the trigger lies in (for the tie-band rule)
+      candidates structured array (template, bin, re, im) sorted
+      n_flat     number of flat triggers |rho| >= thr2 over the same templates
+      near       structured array of every (template, time, re, im, avg_abs) with
+                 |rho| >= thr2 (1 - 2e-3) and |rho_bar| >= thr1 (1 - 2e-3): superset used for the allowed set
+    """
+    j_low, _ = band(N, fs, f_low)
+    T = np.asarray(coeffs).shape[0]
+    tids = np.arange(T) if templates is None else np.atleast_1d(np.asarray(templates))
+    trig_dt = np.dtype([("template", np.int64), ("time", np.int64), ("re", np.float64), ("im", np.float64),
+                        ("avg_abs", np.float64)])
+    cand_dt = np.dtype([("template", np.int64), ("bin", np.int64), ("re", np.float64), ("im", np.float64)])
+    trig_parts, cand_parts, near_parts = [], [], []
+    n_flat = 0
+    slack = 1.0 - 2e-3
+    for a in range(0, len(tids), chunk):
+        ids = tids[a:a + chunk]
+        h = reconstructed_templates(coeffs, basis, ids)
+        rho = snr_series_fft(strain, h, np.asarray(sigma, dtype=np.float64)[ids], N, j_low)
+        for m, t in enumerate(ids):
+            cand, trig, flat, rho_bar = hierarchical_triggers_one(rho[m], w, thr1, thr2)
+            n_flat += len(flat)
+            if len(cand):
+                c = np.empty(len(cand), dtype=cand_dt)
+                c["template"], c["bin"] = t, cand
+                c["re"], c["im"] = rho_bar[cand].real, rho_bar[cand].imag
+                cand_parts.append(c)
+            if len(trig):
+                r = np.empty(len(trig), dtype=trig_dt)
+                r["template"], r["time"] = t, trig
+                r["re"], r["im"] = rho[m][trig].real, rho[m][trig].imag
+                r["avg_abs"] = np.abs(rho_bar[trig // w])
+                trig_parts.append(r)
+            if keep_margins:
+                mod = np.abs(rho[m])
+                nn = np.nonzero(mod >= thr2 * slack)[0]
+                nn = nn[np.abs(rho_bar[nn // w]) >= thr1 * slack]
+                if len(nn):
+                    r = np.empty(len(nn), dtype=trig_dt)
+                    r["template"], r["time"] = t, nn
+                    r["re"], r["im"] = rho[m][nn].real, rho[m][nn].imag
+                    r["avg_abs"] = np.abs(rho_bar[nn // w])
+                    near_parts.append(r)
+    cat = lambda parts, dt: np.concatenate(parts) if parts else np.empty(0, dtype=dt)
+    return {"triggers": cat(trig_parts, trig_dt), "candidates": cat(cand_parts, cand_dt),
+            "near": cat(near_parts, trig_dt), "n_flat": n_flat}
+
+
+def evaluate_points(strain, basis, coeffs, sigma, N, fs, f_low, w, template, times):
+    """Pointwise re-evaluation for one template: returns (rho[n] for n in times, rho_bar of each n's bin),
+    every value by the literal O(|B|) sum of Eq. 4 (no FFT)."""
+    j_low, _ = band(N, fs, f_low)
+    h = reconstructed_templates(coeffs, basis, [template])[0]
+    sg = float(np.asarray(sigma, dtype=np.float64)[template])
+    rho, rbar = [], []
+    for n in np.atleast_1d(times):
+        n = int(n)
+        rho.append(snr_point(strain, h, sg, N, j_low, n))
+        b = n // w
+        rbar.append(sum(snr_point(strain, h, sg, N, j_low, b * w + r) for r in range(w)) / w)
+    return np.array(rho), np.array(rbar)
+
+
+# ------------------------------------------------------- cost model, Eq. 13-15
+def z_basic(N, T):
+    """Template-method flops, Eq. 13; log base 2 (reading R19)."""
+    return N * T * (5.0 * math.log2(N) + 6.0)
+
+
+def z_first(N, T, w):
+    """First-stage flops by the template route, Eq. 14."""
+    return N * T * (5.0 / w * math.log2(N / w) + 6.0 + 2.0 / w)
+
+
+def z_total(N, T, w, p, f_triggers):
+    """Eq. 15: z_first + 4 p w f T + N p (5 log N + 6)."""
+    return z_first(N, T, w) + 4.0 * p * w * f_triggers * T + N * p * (5.0 * math.log2(N) + 6.0)
+
+
+def throughput(N_seconds, T, t_seconds):
+    """Templates processed in real time = N T / t."""
+    return N_seconds * T / t_seconds
