@@ -1,0 +1,154 @@
+/* rbmf.h -- C ABI of the B200-native reduced-basis hierarchical matched filter.
+ *
+ * The library implements the hot path of Dhurkunde, Fehrmann & Nitz, "A hierarchical approach to
+ * matched filtering using a reduced basis" (arXiv:2110.13115; citations below are PAPER.md lines):
+ *
+ *   a1  g_k[j]      = s d[j] conj(b_k[j]),  j in band [j_low, N/2)
+ *   a2  beta_k[n]   = sum_j g_k[j] exp(+2 pi i j n / N)                        (Eq. 6)
+ *   a3  beta^avg_k[i] = (1/w) sum_{r<w} beta_k[i w + r]                        (Eq. 9)
+ *   a4  R_t[i]      = (1/sigma_t) sum_k conj(c_tk) beta^avg_k[i]               (Eq. 7)
+ *   a5  candidate (t,i)  iff |R_t[i]| >= thr_stage1
+ *   a6  rho_t[i w + r] = (1/sigma_t) sum_k conj(c_tk) beta_k[i w + r], r < w, for every candidate;
+ *       trigger iff |rho| >= thr_stage2
+ *
+ * with s = sqrt(2/N), d = unnormalised forward DFT of the whitened unit-variance strain, b_k orthonormal
+ * over the band, c_tk the decomposition coefficients.  Every step runs in hand-written CUDA
+ * kernels for sm_100a (batched Stockham FFT; tcgen05/TMEM split-bf16 GEMM with a fused threshold/compaction
+ * epilogue; a warp-per-candidate re-scoring kernel).  There is no CPU fallback.
+ *
+ * Conventions
+ *  - "dev" pointers are CUDA device memory owned by the caller; "host" pointers are ordinary host memory.
+ *  - The library never allocates or frees device memory: the caller provides one workspace
+ *    (rbmf_workspace_bytes / rbmf_plan_set_workspace) that must outlive the plan's use.
+ *  - rbmf_set_basis / rbmf_set_coeffs copy and re-lay-out their inputs into the workspace; the caller's
+ *    arrays may be freed after the stream has completed those calls.
+ *  - All work is enqueued on the plan's stream (rbmf_set_stream; default: the legacy default stream) and
+ *    is asynchronous unless stated.  No function throws or aborts; every one returns an rbmf_status.
+ *  - complex64 = interleaved (re, im) float32, little endian.
+ */
+#ifndef RBMF_H
+#define RBMF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rbmf_plan rbmf_plan; /* opaque */
+
+/* One final trigger: a sample whose SNR modulus is above thr_stage2 inside a first-stage bin. */
+typedef struct {
+    int32_t template_id; /* row of the coefficient matrix                       */
+    int32_t time_index;  /* sample n in [0, N)                                  */
+    float snr_re;        /* complex SNR rho_t[n] (already divided by sigma_t)   */
+    float snr_im;
+} rbmf_trigger;
+
+/* One first-stage candidate: a (template, bin) whose averaged SNR modulus is above thr_stage1. */
+typedef struct {
+    int32_t template_id;
+    int32_t bin_index; /* i in [0, N/w): samples i w .. i w + w - 1            */
+    float avg_re;      /* averaged complex SNR R_t[i]                         */
+    float avg_im;
+} rbmf_candidate;
+
+typedef enum {
+    RBMF_OK = 0,
+    RBMF_ERR_ARG = -1,         /* bad argument (NULL, size, alignment, range)                          */
+    RBMF_ERR_STATE = -2,       /* call order: workspace / basis / coefficients not set yet             */
+    RBMF_ERR_CUDA = -3,        /* a CUDA runtime/driver call failed (rbmf_last_cuda_error has the code) */
+    RBMF_ERR_OVERFLOW = -4,    /* more candidates or triggers than capacity; lists are truncated       */
+    RBMF_ERR_UNSUPPORTED = -5  /* valid but not implemented for this size / device                     */
+} rbmf_status;
+
+/* Stage-1 reconstruction kernels (rbmf_plan_set_gemm_impl). */
+typedef enum {
+    RBMF_GEMM_TCGEN05 = 0, /* default: TMA + tcgen05.mma (bf16x3 split precision) + TMEM epilogue     */
+    RBMF_GEMM_SIMT = 1     /* plain fp32 CUDA-core kernel on the same operands; verification only      */
+} rbmf_gemm_impl;
+
+/* Create a plan for segments of N samples (power of two, 2^10 <= N <= 2^20) at sampling rate fs [Hz],
+ * lower cutoff f_low [Hz] (0 < f_low < fs/2), k basis vectors (multiple of 16, 16 <= k <= 1024) and T >= 1
+ * templates.  Band = bins [ceil(f_low N / fs), N/2).  Host-only; no device work.  Defaults: w = 8,
+ * max_candidates = max_triggers = 2^22.  *out is set to NULL on failure. */
+rbmf_status rbmf_plan_create(rbmf_plan** out, int64_t N, double fs, double f_low, int32_t k, int32_t T);
+
+/* Stage-1 averaging window w of Eq. 9 (power of two, 1 <= w <= 64, N/w >= 128).  w = 1 is the flat search.
+ * Must be called before rbmf_workspace_bytes / rbmf_plan_set_workspace. */
+rbmf_status rbmf_plan_set_window(rbmf_plan* plan, int32_t w);
+
+/* Capacity (entries) of the internal candidate list and of the caller's trigger array.  Must be called
+ * before rbmf_workspace_bytes / rbmf_plan_set_workspace. */
+rbmf_status rbmf_plan_set_capacity(rbmf_plan* plan, int64_t max_candidates, int64_t max_triggers);
+
+/* Select the stage-1 kernel (default RBMF_GEMM_TCGEN05).  May be called at any time. */
+rbmf_status rbmf_plan_set_gemm_impl(rbmf_plan* plan, int32_t impl);
+
+/* Bytes of device workspace the plan needs (depends on N, k, T, w, capacities). */
+rbmf_status rbmf_workspace_bytes(const rbmf_plan* plan, size_t* bytes);
+
+/* Hand the plan its workspace: dev_ptr must be 1024-byte aligned device memory of >= rbmf_workspace_bytes.
+ * Enqueues the initialisation of the plan's constant tables (twiddles) on the plan's stream.  Invalidates
+ * any basis / coefficients set before. */
+rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes);
+
+/* cudaStream_t to enqueue on (NULL = legacy default stream). */
+rbmf_status rbmf_set_stream(rbmf_plan* plan, void* cuda_stream);
+
+/* basis_dev: k x (N/2+1) complex64, row-major: b_k[j] (p~_k of PAPER.md:82), orthonormal over the band.
+ * Values outside the band are ignored.  Copied (transposed to bins x k) into the workspace. */
+rbmf_status rbmf_set_basis(rbmf_plan* plan, const void* basis_dev);
+
+/* coeffs_dev: T x k complex64, row-major: c_tk, unconjugated.  sigma_dev: T float32 template
+ * norms sigma_t > 0, or NULL => sigma_t = ||c_t||_2.  Copied (conjugated, scaled by 1/sigma_t, split into bf16
+ * hi/lo planes) into the workspace. */
+rbmf_status rbmf_set_coeffs(rbmf_plan* plan, const void* coeffs_dev, const float* sigma_dev);
+
+/* Filter one segment.  strain_dev: (N/2+1) complex64, the unnormalised forward DFT of the whitened strain.
+ * thr_stage1 > 0 applies to the modulus of the w-averaged SNR, thr_stage2 > 0 to the modulus of the SNR.
+ * out_dev: array of max_triggers rbmf_trigger (unordered set on return).  n_out_dev: device int64 that
+ * receives the TOTAL number of triggers found (may exceed max_triggers; then only max_triggers were written).
+ * Enqueues only; results are valid once the stream has completed. */
+rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage1, float thr_stage2,
+                        rbmf_trigger* out_dev, int64_t* n_out_dev);
+
+/* End-to-end convenience with HOST buffers: copies the strain to the device, filters, waits, and copies
+ * the triggers back.  strain_host: (N/2+1) complex64.  out_host: capacity_out entries (<= max_triggers).
+ * *n_out_host = total found.  Synchronous.  Returns RBMF_ERR_OVERFLOW if either list overflowed. */
+rbmf_status rbmf_filter_host(rbmf_plan* plan, const void* strain_host, float thr_stage1, float thr_stage2,
+                             rbmf_trigger* out_host, int64_t capacity_out, int64_t* n_out_host);
+
+/* Counts of the last rbmf_filter (synchronises the stream).  RBMF_ERR_OVERFLOW if a capacity was exceeded. */
+rbmf_status rbmf_get_counts(rbmf_plan* plan, int64_t* n_candidates, int64_t* n_triggers);
+
+/* Copy up to `capacity` first-stage candidates of the last rbmf_filter to out_host (synchronises).
+ * *n_out = total candidates found. */
+rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64_t capacity, int64_t* n_out);
+
+/* Read-only device views of internal arrays for diagnostics and parity tests (valid after rbmf_filter on the
+ * plan's stream, until the next call).  which: 0 = beta (N x k complex64, time-major),
+ * 1 = beta^avg hi plane, 2 = beta^avg lo plane ((N/w) x 2k bfloat16 each; value = hi + lo).
+ * *dev_ptr receives the address, *bytes the size. */
+rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_ptr, size_t* bytes);
+
+/* Per-stage GPU time of the last rbmf_filter, in milliseconds (synchronises): ms[0] = a1-a3 (FFT stage),
+ * ms[1] = a4-a5 (GEMM + threshold), ms[2] = a6 (stage 2), ms[3] = whole call.  Timing events are recorded
+ * only after rbmf_plan_set_timing(plan, 1). */
+rbmf_status rbmf_plan_set_timing(rbmf_plan* plan, int32_t enabled);
+rbmf_status rbmf_get_stage_ms(rbmf_plan* plan, float ms[4]);
+
+/* Number of kernels rbmf_filter launches for this plan's configuration. */
+rbmf_status rbmf_launches_per_filter(const rbmf_plan* plan, int32_t* n);
+
+rbmf_status rbmf_plan_destroy(rbmf_plan* plan);
+
+const char* rbmf_status_string(rbmf_status status);
+/* Last cudaError_t / CUresult seen by this plan (0 if none). */
+int32_t rbmf_last_cuda_error(const rbmf_plan* plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RBMF_H */

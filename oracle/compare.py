@@ -1,0 +1,78 @@
+"""Comparison rule between a trigger list under test and the fp64 oracle's result (test infrastructure).
+
+"Identical trigger sets" across an fp32 GPU path and an fp64 oracle is decidable only away from the thresholds, so
+("comparison rule") with tau = 1e-3, the metric's own SNR tolerance:
+
+  mandatory set M = oracle triggers with |rho_bar|/thr1 - 1 >  tau  and  |rho|/thr2 - 1 >  tau
+  allowed   set A = oracle samples  with |rho_bar|/thr1 - 1 > -tau  and  |rho|/thr2 - 1 > -tau
+  pass  iff  M  subset-of  GOT  subset-of  A,  and for every trigger in GOT
+             | |rho_got| - |rho_or| | <= 1e-3 |rho_or|   and   |arg(rho_got conj(rho_or))| <= 1e-3 rad.
+
+This module imports nothing from the CUDA path.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+TAU = 1e-3
+
+
+def _keys(templates, times, N):
+    return np.asarray(templates, dtype=np.int64) * int(N) + np.asarray(times, dtype=np.int64)
+
+
+def compare_triggers(got, oracle_result, N, thr1, thr2, tau=TAU, snr_rtol=1e-3, phase_atol=1e-3):
+    """got: structured array with fields template, time, re, im.  oracle_result: dict from oracle_filter
+    (keep_margins=True).  Returns a report dict; report['ok'] is the verdict."""
+    near = oracle_result["near"]
+    trig = oracle_result["triggers"]
+    mod_near = np.hypot(near["re"], near["im"])
+    allowed = near[(near["avg_abs"] / thr1 - 1.0 > -tau) & (mod_near / thr2 - 1.0 > -tau)]
+    mod_trig = np.hypot(trig["re"], trig["im"])
+    mandatory = trig[(trig["avg_abs"] / thr1 - 1.0 > tau) & (mod_trig / thr2 - 1.0 > tau)]
+
+    k_got = _keys(got["template"], got["time"], N)
+    k_all = _keys(allowed["template"], allowed["time"], N)
+    k_man = _keys(mandatory["template"], mandatory["time"], N)
+    dup = len(k_got) - len(np.unique(k_got))
+    missing = np.setdiff1d(k_man, k_got)
+    extra = np.setdiff1d(k_got, k_all)
+
+    # per-trigger values against the oracle's value at the same (template, time)
+    order = np.argsort(k_all)
+    pos = np.searchsorted(k_all[order], k_got)
+    pos = np.clip(pos, 0, max(len(k_all) - 1, 0))
+    matched = len(k_all) > 0
+    max_rel, max_phase, bad_val = 0.0, 0.0, 0
+    if matched and len(k_got):
+        idx = order[pos]
+        hit = k_all[idx] == k_got
+        ref = allowed["re"][idx[hit]] + 1j * allowed["im"][idx[hit]]
+        val = got["re"][hit].astype(np.float64) + 1j * got["im"][hit].astype(np.float64)
+        rel = np.abs(np.abs(val) - np.abs(ref)) / np.abs(ref)
+        ph = np.abs(np.angle(val * np.conj(ref)))
+        if len(rel):
+            max_rel, max_phase = float(rel.max()), float(ph.max())
+            bad_val = int(((rel > snr_rtol) | (ph > phase_atol)).sum())
+    ok = dup == 0 and len(missing) == 0 and len(extra) == 0 and bad_val == 0
+    return {
+        "ok": bool(ok), "n_got": int(len(k_got)), "n_oracle": int(len(trig)), "n_mandatory": int(len(k_man)),
+        "n_allowed": int(len(k_all)), "n_missing": int(len(missing)), "n_extra": int(len(extra)),
+        "n_duplicates": int(dup), "n_bad_values": bad_val, "max_rel_snr_err": max_rel, "max_phase_err": max_phase,
+        "tie_band": int(len(k_all) - len(k_man)),
+    }
+
+
+def compare_candidates(got, oracle_result, n_bins, thr1, tau=TAU):
+    """First-stage candidate sets: oracle candidates with margin > tau must be present; every reported candidate must
+    have an oracle averaged SNR within tau of the threshold or above.  `got` has fields template, bin, re, im.
+    The allowed side needs |rho_bar| of bins just below thr1, which `oracle_filter` does not keep, so the caller
+    passes `oracle_result['cand_near']` when available; otherwise only the mandatory side is checked."""
+    cand = oracle_result["candidates"]
+    mod = np.hypot(cand["re"], cand["im"])
+    man = cand[mod / thr1 - 1.0 > tau]
+    k_got = _keys(got["template"], got["bin"], n_bins)
+    k_man = _keys(man["template"], man["bin"], n_bins)
+    missing = np.setdiff1d(k_man, k_got)
+    return {"n_got": int(len(k_got)), "n_oracle": int(len(cand)), "n_missing": int(len(missing)),
+            "ok": len(missing) == 0}

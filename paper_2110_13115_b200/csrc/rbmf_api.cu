@@ -1,0 +1,446 @@
+// The C ABI of librbmf.so (include/rbmf.h): plan management, workspace layout, TMA descriptors, launch sequence.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "rbmf_internal.h"
+
+using namespace rbmf;
+
+namespace {
+
+constexpr size_t kAlign = 1024;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+inline int ilog2(int64_t x) { int l = 0; while ((int64_t(1) << l) < x) ++l; return l; }
+
+struct Layout {
+    size_t basisT, Y, Yavg, beta, bavg_hi, bavg_lo, c_hi, c_lo, cs, tw_L, tw_lo_main, tw_hi_main, tw_lo_avg,
+        tw_hi_avg, S_table, ds, dS, cand, counters, strain_stage, trig_stage, total;
+};
+
+}  // namespace
+
+struct rbmf_plan {
+    int64_t N;
+    double fs, f_low;
+    int k, T, w;
+    int64_t M;          // N / w
+    int j_low, n_half;
+    int Tpad;
+    int logN1, logN2;   // main FFT: N = 2^logN1 * 2^logN2 (pass 1 length, pass 2 length)
+    int logM1, logM2;   // averaged FFT
+    int64_t max_cand, max_trig;
+    int gemm_impl;
+    int timing;
+    cudaStream_t stream;
+    uint8_t* ws;
+    size_t ws_bytes;
+    Layout lay;
+    bool have_ws, have_basis, have_coeffs, filtered;
+    int num_sms;
+    int last_cuda;
+    CUtensorMap tmA_hi, tmA_lo, tmB_hi, tmB_lo;
+    bool have_maps;
+    cudaEvent_t ev[5];
+    bool have_events;
+};
+
+namespace {
+
+Layout make_layout(const rbmf_plan* p) {
+    Layout L;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    const size_t k = (size_t)p->k, N = (size_t)p->N, M = (size_t)p->M;
+    L.basisT = take((size_t)p->n_half * k * 8);
+    L.Y = take(N * k * 8);
+    L.Yavg = take(p->w > 1 ? M * k * 8 : 0);
+    L.beta = take(N * k * 8);
+    L.bavg_hi = take(M * 2 * k * 2);
+    L.bavg_lo = take(M * 2 * k * 2);
+    L.c_hi = take((size_t)p->Tpad * 2 * 2 * k * 2);
+    L.c_lo = take((size_t)p->Tpad * 2 * 2 * k * 2);
+    L.cs = take((size_t)p->T * k * 8);
+    L.tw_L = take((size_t)kTwAllEntries * 8);
+    L.tw_lo_main = take(1024 * 8);
+    L.tw_hi_main = take((N / 1024 ? N / 1024 : 1) * 8);
+    L.tw_lo_avg = take(1024 * 8);
+    L.tw_hi_avg = take((M / 1024 ? M / 1024 : 1) * 8);
+    L.S_table = take((size_t)p->n_half * 8);
+    L.ds = take((size_t)p->n_half * 8);
+    L.dS = take((size_t)p->n_half * 8);
+    L.cand = take((size_t)p->max_cand * sizeof(rbmf_candidate));
+    L.counters = take(64);
+    L.strain_stage = take((size_t)(p->n_half + 1) * 8);
+    L.trig_stage = take((size_t)p->max_trig * sizeof(rbmf_trigger));
+    L.total = off;
+    return L;
+}
+
+void refresh(rbmf_plan* p) {
+    p->M = p->N / p->w;
+    const int n = ilog2(p->N), m = ilog2(p->M);
+    p->logN1 = (n + 1) / 2; p->logN2 = n / 2;
+    p->logM1 = (m + 1) / 2; p->logM2 = m / 2;
+    p->Tpad = (p->T + kGemmTT - 1) / kGemmTT * kGemmTT;
+    p->lay = make_layout(p);
+}
+
+rbmf_status cuda_fail(rbmf_plan* p, cudaError_t e) {
+    if (p) p->last_cuda = (int)e;
+    return RBMF_ERR_CUDA;
+}
+
+#define CK(call)                                              \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(plan, e__);  \
+    } while (0)
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+rbmf_status make_map(rbmf_plan* plan, CUtensorMap* map, void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres);
+        if (e != cudaSuccess) return cuda_fail(plan, e);
+        if (qres != cudaDriverEntryPointSuccess || !sym) { plan->last_cuda = -1; return RBMF_ERR_CUDA; }
+        fn = (EncodeTiledFn)sym;
+    }
+    const cuuint64_t dims[2] = {cols, rows};               // innermost first
+    const cuuint64_t strides[1] = {cols * 2};              // bytes, dims 1..rank-1
+    const cuuint32_t box[2] = {(cuuint32_t)kGemmBK, box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { plan->last_cuda = (int)r; return RBMF_ERR_CUDA; }
+    return RBMF_OK;
+}
+
+template <typename T> T* at(rbmf_plan* p, size_t off) { return reinterpret_cast<T*>(p->ws + off); }
+
+}  // namespace
+
+extern "C" {
+
+rbmf_status rbmf_plan_create(rbmf_plan** out, int64_t N, double fs, double f_low, int32_t k, int32_t T) {
+    if (!out) return RBMF_ERR_ARG;
+    *out = nullptr;
+    if (N < 1024 || N > (int64_t(1) << 20) || (N & (N - 1)) != 0) return RBMF_ERR_ARG;
+    if (!(fs > 0.0) || !(f_low > 0.0) || !(f_low < fs / 2)) return RBMF_ERR_ARG;
+    if (k < 16 || k > 1024 || (k % 16) != 0) return RBMF_ERR_ARG;
+    if (T < 1 || T > (1 << 24)) return RBMF_ERR_ARG;
+    rbmf_plan* p = new (std::nothrow) rbmf_plan;
+    if (!p) return RBMF_ERR_ARG;
+    memset(p, 0, sizeof(*p));
+    p->N = N; p->fs = fs; p->f_low = f_low; p->k = k; p->T = T;
+    p->w = 8;
+    p->n_half = (int)(N / 2);
+    p->j_low = (int)ceil(f_low * (double)N / fs - 1e-12);
+    if (p->j_low >= p->n_half) { delete p; return RBMF_ERR_ARG; }
+    p->max_cand = int64_t(1) << 22;
+    p->max_trig = int64_t(1) << 22;
+    p->gemm_impl = RBMF_GEMM_TCGEN05;
+    refresh(p);
+    *out = p;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_plan_set_window(rbmf_plan* plan, int32_t w) {
+    if (!plan) return RBMF_ERR_ARG;
+    if (plan->have_ws) return RBMF_ERR_STATE;
+    if (w < 1 || w > 32 || (w & (w - 1)) != 0) return RBMF_ERR_ARG;
+    if (plan->N / w < 1024) return RBMF_ERR_ARG;
+    plan->w = w;
+    refresh(plan);
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_plan_set_capacity(rbmf_plan* plan, int64_t max_candidates, int64_t max_triggers) {
+    if (!plan) return RBMF_ERR_ARG;
+    if (plan->have_ws) return RBMF_ERR_STATE;
+    if (max_candidates < 1 || max_triggers < 1 || max_candidates > (int64_t(1) << 31) ||
+        max_triggers > (int64_t(1) << 31))
+        return RBMF_ERR_ARG;
+    plan->max_cand = max_candidates;
+    plan->max_trig = max_triggers;
+    refresh(plan);
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_plan_set_gemm_impl(rbmf_plan* plan, int32_t impl) {
+    if (!plan) return RBMF_ERR_ARG;
+    if (impl != RBMF_GEMM_TCGEN05 && impl != RBMF_GEMM_SIMT) return RBMF_ERR_ARG;
+    plan->gemm_impl = impl;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_workspace_bytes(const rbmf_plan* plan, size_t* bytes) {
+    if (!plan || !bytes) return RBMF_ERR_ARG;
+    *bytes = plan->lay.total;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_set_stream(rbmf_plan* plan, void* cuda_stream) {
+    if (!plan) return RBMF_ERR_ARG;
+    plan->stream = (cudaStream_t)cuda_stream;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes) {
+    if (!plan || !dev_ptr) return RBMF_ERR_ARG;
+    if (((uintptr_t)dev_ptr % kAlign) != 0 || bytes < plan->lay.total) return RBMF_ERR_ARG;
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    int major = 0, minor = 0;
+    CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    CK(cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev));
+    if (major != 10) return RBMF_ERR_UNSUPPORTED;   // sm_100a only: tcgen05 / TMEM
+    CK(cudaDeviceGetAttribute(&plan->num_sms, cudaDevAttrMultiProcessorCount, dev));
+    plan->ws = (uint8_t*)dev_ptr;
+    plan->ws_bytes = bytes;
+    plan->have_ws = true;
+    plan->have_basis = plan->have_coeffs = plan->filtered = false;
+    const Layout& L = plan->lay;
+    CK(launch_init_tables(at<float2>(plan, L.tw_L), at<float2>(plan, L.tw_lo_main), at<float2>(plan, L.tw_hi_main),
+                          at<float2>(plan, L.tw_lo_avg), at<float2>(plan, L.tw_hi_avg), at<float2>(plan, L.S_table),
+                          plan->N, plan->M, plan->w, plan->stream));
+    CK(cudaMemsetAsync(plan->ws + L.counters, 0, 64, plan->stream));
+    CK(gemm_tcgen05_configure());
+    // TMA descriptors: A = beta^avg planes (M rows x 2k), B = coefficient planes (2*Tpad rows x 2k)
+    rbmf_status s;
+    const uint64_t k2 = 2 * (uint64_t)plan->k;
+    if ((s = make_map(plan, &plan->tmA_hi, plan->ws + L.bavg_hi, (uint64_t)plan->M, k2, kGemmBM)) != RBMF_OK) return s;
+    if ((s = make_map(plan, &plan->tmA_lo, plan->ws + L.bavg_lo, (uint64_t)plan->M, k2, kGemmBM)) != RBMF_OK) return s;
+    if ((s = make_map(plan, &plan->tmB_hi, plan->ws + L.c_hi, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
+    if ((s = make_map(plan, &plan->tmB_lo, plan->ws + L.c_lo, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
+    plan->have_maps = true;
+    if (!plan->have_events) {
+        for (int i = 0; i < 5; ++i) CK(cudaEventCreate(&plan->ev[i]));
+        plan->have_events = true;
+    }
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_set_basis(rbmf_plan* plan, const void* basis_dev) {
+    if (!plan || !basis_dev) return RBMF_ERR_ARG;
+    if (!plan->have_ws) return RBMF_ERR_STATE;
+    CK(launch_transpose_basis((const float2*)basis_dev, at<float2>(plan, plan->lay.basisT), plan->k, plan->N / 2 + 1,
+                              plan->j_low, plan->n_half, plan->stream));
+    plan->have_basis = true;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_set_coeffs(rbmf_plan* plan, const void* coeffs_dev, const float* sigma_dev) {
+    if (!plan || !coeffs_dev) return RBMF_ERR_ARG;
+    if (!plan->have_ws) return RBMF_ERR_STATE;
+    const Layout& L = plan->lay;
+    CK(launch_prep_coeffs((const float2*)coeffs_dev, sigma_dev, at<float2>(plan, L.cs), at<uint16_t>(plan, L.c_hi),
+                          at<uint16_t>(plan, L.c_lo), plan->T, plan->Tpad, plan->k, plan->stream));
+    plan->have_coeffs = true;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage1, float thr_stage2,
+                        rbmf_trigger* out_dev, int64_t* n_out_dev) {
+    if (!plan || !strain_dev || !out_dev || !n_out_dev) return RBMF_ERR_ARG;
+    if (!(thr_stage1 > 0.f) || !(thr_stage2 > 0.f)) return RBMF_ERR_ARG;
+    if (!plan->have_ws || !plan->have_basis || !plan->have_coeffs) return RBMF_ERR_STATE;
+    const Layout& L = plan->lay;
+    cudaStream_t st = plan->stream;
+    const bool tm = plan->timing != 0;
+    unsigned long long* counters = at<unsigned long long>(plan, L.counters);
+
+    if (tm) CK(cudaEventRecord(plan->ev[0], st));
+    CK(cudaMemsetAsync(counters, 0, 16, st));
+    CK(launch_prep_strain((const float2*)strain_dev, at<float2>(plan, L.S_table), at<float2>(plan, L.ds),
+                          at<float2>(plan, L.dS), plan->n_half, (float)sqrt(2.0 / (double)plan->N), st));
+
+    // ---- kernel 1: a1-a3 -----------------------------------------------------------------------
+    FftArgs a;
+    memset(&a, 0, sizeof(a));
+    a.k = plan->k; a.j_low = plan->j_low; a.n_half = plan->n_half;
+    a.fold = 1; a.fold_stride = 0;
+    a.plane_hi = at<uint16_t>(plan, L.bavg_hi);
+    a.plane_lo = at<uint16_t>(plan, L.bavg_lo);
+    // main transform, pass 1: basis x strain -> Y
+    a.in = at<float2>(plan, L.basisT); a.strain = at<float2>(plan, L.ds); a.out = at<float2>(plan, L.Y);
+    a.tw_L = at<float2>(plan, L.tw_L) + tw_table_offset(plan->logN1);
+    a.tw_lo = at<float2>(plan, L.tw_lo_main); a.tw_hi = at<float2>(plan, L.tw_hi_main);
+    a.lines = 1 << plan->logN2;
+    CK(launch_fft_pass1(a, plan->logN1, false, st));
+    // main transform, pass 2: Y -> beta (and the operand planes when w = 1)
+    a.in = at<float2>(plan, L.Y); a.out = at<float2>(plan, L.beta);
+    a.tw_L = at<float2>(plan, L.tw_L) + tw_table_offset(plan->logN2);
+    a.lines = 1 << plan->logN1;
+    CK(launch_fft_pass2(a, plan->logN2, plan->w == 1 ? 2 : 0, st));
+    if (plan->w > 1) {
+        // averaged transform (Eq. 12): fold w/2 aliases -> Yavg -> beta^avg planes
+        a.in = at<float2>(plan, L.basisT); a.strain = at<float2>(plan, L.dS); a.out = at<float2>(plan, L.Yavg);
+        a.tw_L = at<float2>(plan, L.tw_L) + tw_table_offset(plan->logM1);
+        a.tw_lo = at<float2>(plan, L.tw_lo_avg); a.tw_hi = at<float2>(plan, L.tw_hi_avg);
+        a.lines = 1 << plan->logM2;
+        a.fold = plan->w / 2 > 1 ? plan->w / 2 : 1;
+        a.fold_stride = (int)plan->M;
+        CK(launch_fft_pass1(a, plan->logM1, true, st));
+        a.in = at<float2>(plan, L.Yavg); a.out = nullptr;
+        a.tw_L = at<float2>(plan, L.tw_L) + tw_table_offset(plan->logM2);
+        a.lines = 1 << plan->logM1;
+        CK(launch_fft_pass2(a, plan->logM2, 1, st));
+    }
+    if (tm) CK(cudaEventRecord(plan->ev[1], st));
+
+    // ---- kernel 2: a4-a5 -----------------------------------------------------------------------
+    GemmArgs g;
+    memset(&g, 0, sizeof(g));
+    g.cand = at<rbmf_candidate>(plan, L.cand);
+    g.counters = counters;
+    g.cand_cap = (unsigned long long)plan->max_cand;
+    g.thr1_sq = thr_stage1 * thr_stage1;
+    g.T = plan->T; g.M = (int)plan->M; g.k2 = 2 * plan->k;
+    g.num_tb = plan->Tpad / kGemmTT;
+    g.num_ib = (int)(plan->M / kGemmBM);
+    g.group = 16;
+    if (plan->gemm_impl == RBMF_GEMM_TCGEN05) {
+        CK(launch_gemm_tcgen05(plan->tmA_hi, plan->tmA_lo, plan->tmB_hi, plan->tmB_lo, g, plan->num_sms, st));
+    } else {
+        CK(launch_gemm_simt(at<uint16_t>(plan, L.bavg_hi), at<uint16_t>(plan, L.bavg_lo), at<uint16_t>(plan, L.c_hi),
+                            at<uint16_t>(plan, L.c_lo), g, st));
+    }
+    if (tm) CK(cudaEventRecord(plan->ev[2], st));
+
+    // ---- kernel 3: a6 --------------------------------------------------------------------------
+    Stage2Args s2;
+    memset(&s2, 0, sizeof(s2));
+    s2.cand = g.cand; s2.cs = at<float2>(plan, L.cs); s2.beta = at<float2>(plan, L.beta);
+    s2.out = out_dev; s2.counters = counters;
+    s2.cand_cap = (unsigned long long)plan->max_cand; s2.trig_cap = (unsigned long long)plan->max_trig;
+    s2.thr2_sq = thr_stage2 * thr_stage2; s2.k = plan->k; s2.w = plan->w;
+    CK(launch_stage2(s2, plan->num_sms, st));
+    CK(cudaMemcpyAsync(n_out_dev, counters + 1, 8, cudaMemcpyDeviceToDevice, st));
+    if (tm) CK(cudaEventRecord(plan->ev[3], st));
+    plan->filtered = true;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_get_counts(rbmf_plan* plan, int64_t* n_candidates, int64_t* n_triggers) {
+    if (!plan) return RBMF_ERR_ARG;
+    if (!plan->filtered) return RBMF_ERR_STATE;
+    unsigned long long h[2] = {0, 0};
+    CK(cudaMemcpyAsync(h, plan->ws + plan->lay.counters, 16, cudaMemcpyDeviceToHost, plan->stream));
+    CK(cudaStreamSynchronize(plan->stream));
+    if (n_candidates) *n_candidates = (int64_t)h[0];
+    if (n_triggers) *n_triggers = (int64_t)h[1];
+    if ((int64_t)h[0] > plan->max_cand || (int64_t)h[1] > plan->max_trig) return RBMF_ERR_OVERFLOW;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64_t capacity, int64_t* n_out) {
+    if (!plan || !out_host || !n_out || capacity < 0) return RBMF_ERR_ARG;
+    int64_t nc = 0, nt = 0;
+    rbmf_status s = rbmf_get_counts(plan, &nc, &nt);
+    if (s != RBMF_OK && s != RBMF_ERR_OVERFLOW) return s;
+    *n_out = nc;
+    int64_t n = nc < plan->max_cand ? nc : plan->max_cand;
+    if (n > capacity) n = capacity;
+    if (n > 0) {
+        CK(cudaMemcpyAsync(out_host, plan->ws + plan->lay.cand, (size_t)n * sizeof(rbmf_candidate),
+                           cudaMemcpyDeviceToHost, plan->stream));
+        CK(cudaStreamSynchronize(plan->stream));
+    }
+    return s;
+}
+
+rbmf_status rbmf_filter_host(rbmf_plan* plan, const void* strain_host, float thr_stage1, float thr_stage2,
+                             rbmf_trigger* out_host, int64_t capacity_out, int64_t* n_out_host) {
+    if (!plan || !strain_host || !out_host || !n_out_host || capacity_out < 1) return RBMF_ERR_ARG;
+    if (!plan->have_ws || !plan->have_basis || !plan->have_coeffs) return RBMF_ERR_STATE;
+    if (capacity_out > plan->max_trig) capacity_out = plan->max_trig;
+    const Layout& L = plan->lay;
+    const size_t strain_bytes = (size_t)(plan->N / 2 + 1) * 8;
+    uint8_t* strain_dev = plan->ws + L.strain_stage;
+    rbmf_trigger* trig_dev = (rbmf_trigger*)(plan->ws + L.trig_stage);
+    int64_t* n_dev = (int64_t*)(plan->ws + L.counters + 32);
+    CK(cudaMemcpyAsync(strain_dev, strain_host, strain_bytes, cudaMemcpyHostToDevice, plan->stream));
+    rbmf_status s = rbmf_filter(plan, strain_dev, thr_stage1, thr_stage2, trig_dev, n_dev);
+    if (s != RBMF_OK) return s;
+    int64_t nc = 0, nt = 0;
+    s = rbmf_get_counts(plan, &nc, &nt);
+    if (s != RBMF_OK && s != RBMF_ERR_OVERFLOW) return s;
+    *n_out_host = nt;
+    int64_t n = nt < capacity_out ? nt : capacity_out;
+    if (n > 0) {
+        CK(cudaMemcpyAsync(out_host, trig_dev, (size_t)n * sizeof(rbmf_trigger), cudaMemcpyDeviceToHost,
+                           plan->stream));
+        CK(cudaStreamSynchronize(plan->stream));
+    }
+    return s;
+}
+
+rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_ptr, size_t* bytes) {
+    if (!plan || !dev_ptr || !bytes) return RBMF_ERR_ARG;
+    if (!plan->have_ws) return RBMF_ERR_STATE;
+    const Layout& L = plan->lay;
+    switch (which) {
+        case 0: *dev_ptr = plan->ws + L.beta; *bytes = (size_t)plan->N * plan->k * 8; break;
+        case 1: *dev_ptr = plan->ws + L.bavg_hi; *bytes = (size_t)plan->M * 2 * plan->k * 2; break;
+        case 2: *dev_ptr = plan->ws + L.bavg_lo; *bytes = (size_t)plan->M * 2 * plan->k * 2; break;
+        default: return RBMF_ERR_ARG;
+    }
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_plan_set_timing(rbmf_plan* plan, int32_t enabled) {
+    if (!plan) return RBMF_ERR_ARG;
+    plan->timing = enabled ? 1 : 0;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_get_stage_ms(rbmf_plan* plan, float ms[4]) {
+    if (!plan || !ms) return RBMF_ERR_ARG;
+    if (!plan->filtered || !plan->timing || !plan->have_events) return RBMF_ERR_STATE;
+    CK(cudaEventSynchronize(plan->ev[3]));
+    CK(cudaEventElapsedTime(&ms[0], plan->ev[0], plan->ev[1]));
+    CK(cudaEventElapsedTime(&ms[1], plan->ev[1], plan->ev[2]));
+    CK(cudaEventElapsedTime(&ms[2], plan->ev[2], plan->ev[3]));
+    CK(cudaEventElapsedTime(&ms[3], plan->ev[0], plan->ev[3]));
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_launches_per_filter(const rbmf_plan* plan, int32_t* n) {
+    if (!plan || !n) return RBMF_ERR_ARG;
+    // prep_strain + FFT pass 1 + pass 2 (+ fold pass 1 + planes pass 2 when w > 1) + GEMM + stage 2
+    *n = 1 + 2 + (plan->w > 1 ? 2 : 0) + 1 + 1;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_plan_destroy(rbmf_plan* plan) {
+    if (!plan) return RBMF_ERR_ARG;
+    if (plan->have_events)
+        for (int i = 0; i < 5; ++i) cudaEventDestroy(plan->ev[i]);
+    delete plan;
+    return RBMF_OK;
+}
+
+const char* rbmf_status_string(rbmf_status status) {
+    switch (status) {
+        case RBMF_OK: return "ok";
+        case RBMF_ERR_ARG: return "invalid argument";
+        case RBMF_ERR_STATE: return "call order: workspace, basis or coefficients not set";
+        case RBMF_ERR_CUDA: return "CUDA error (see rbmf_last_cuda_error)";
+        case RBMF_ERR_OVERFLOW: return "candidate or trigger capacity exceeded; lists truncated";
+        case RBMF_ERR_UNSUPPORTED: return "unsupported size or device";
+        default: return "unknown status";
+    }
+}
+
+int32_t rbmf_last_cuda_error(const rbmf_plan* plan) { return plan ? plan->last_cuda : 0; }
+
+}  // extern "C"

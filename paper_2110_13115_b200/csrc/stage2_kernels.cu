@@ -1,0 +1,128 @@
+// Kernel 3 (step a6): re-score every first-stage candidate at full time resolution and fp32 accuracy
+// (PAPER.md:180, :191, :230, :246), plus the plain fp32 verification version of kernel 2 (RBMF_GEMM_SIMT).
+#include <cuda_bf16.h>
+
+#include "rbmf_internal.h"
+
+namespace rbmf {
+
+// One warp per candidate (t, i): rho_t[i w + r] = sum_c cs[t][c] * beta[i w + r][c], r < w  (cs = conj(c)/sigma).
+// Reads one contiguous block of w*k complex64 of beta and the k coefficients of template t.
+__global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
+    const int lane = threadIdx.x & 31;
+    const unsigned long long warp0 = (unsigned long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const unsigned long long nwarps = (unsigned long long)gridDim.x * (blockDim.x >> 5);
+    unsigned long long n_cand = a.counters[0];
+    if (n_cand > a.cand_cap) n_cand = a.cand_cap;
+    const int k = a.k, w = a.w;
+    for (unsigned long long ci = warp0; ci < n_cand; ci += nwarps) {
+        const rbmf_candidate cd = a.cand[ci];
+        const float2* __restrict__ crow = a.cs + (size_t)cd.template_id * k;
+        const float2* __restrict__ brow = a.beta + (size_t)cd.bin_index * w * k;
+        float my_re = 0.f, my_im = 0.f;   // lane r keeps rho of sample r (w <= 32)
+        for (int r = 0; r < w; ++r) {
+            float re = 0.f, im = 0.f;
+            for (int c = lane; c < k; c += 32) {
+                const float2 p = __ldg(crow + c);
+                const float2 x = __ldg(brow + (size_t)r * k + c);
+                re = fmaf(p.x, x.x, re); re = fmaf(-p.y, x.y, re);
+                im = fmaf(p.x, x.y, im); im = fmaf(p.y, x.x, im);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                re += __shfl_xor_sync(0xffffffffu, re, o);
+                im += __shfl_xor_sync(0xffffffffu, im, o);
+            }
+            if (lane == r) { my_re = re; my_im = im; }
+        }
+        const bool hit = lane < w && (my_re * my_re + my_im * my_im >= a.thr2_sq);
+        const unsigned ballot = __ballot_sync(0xffffffffu, hit);
+        if (ballot) {
+            unsigned long long base = 0;
+            if (lane == 0) base = atomicAdd(a.counters + 1, (unsigned long long)__popc(ballot));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (hit) {
+                const unsigned long long idx = base + __popc(ballot & ((1u << lane) - 1u));
+                if (idx < a.trig_cap) {
+                    rbmf_trigger t;
+                    t.template_id = cd.template_id;
+                    t.time_index = cd.bin_index * w + lane;
+                    t.snr_re = my_re;
+                    t.snr_im = my_im;
+                    a.out[idx] = t;
+                }
+            }
+        }
+    }
+}
+
+cudaError_t launch_stage2(const Stage2Args& a, int num_sms, cudaStream_t st) {
+    stage2_kernel<<<num_sms * 8, 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Verification version of steps a4-a5 on CUDA cores: the same bf16 hi/lo operand planes as the tensor-core
+// kernel, recombined to fp32 (hi + lo) and multiplied in fp32.  64 time bins x 64 templates per CTA.
+__device__ __forceinline__ float plane_val(const uint16_t* hi, const uint16_t* lo, size_t e) {
+    return __bfloat162float(__ushort_as_bfloat16(hi[e])) + __bfloat162float(__ushort_as_bfloat16(lo[e]));
+}
+
+__global__ void __launch_bounds__(256) gemm_simt_kernel(const uint16_t* __restrict__ a_hi,
+                                                        const uint16_t* __restrict__ a_lo,
+                                                        const uint16_t* __restrict__ c_hi,
+                                                        const uint16_t* __restrict__ c_lo, const GemmArgs g) {
+    constexpr int TI = 64, TT = 64, KB = 32;
+    __shared__ float sA[TI][KB + 1];       // beta^avg rows (time bins) x K
+    __shared__ float sRe[TT][KB + 1];      // template "re" rows
+    __shared__ float sIm[TT][KB + 1];      // template "im" rows
+    const int i0 = blockIdx.x * TI, t0 = blockIdx.y * TT;
+    const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;   // 16 x 16 threads, 4 x 4 outputs each
+    float re[4][4] = {}, im[4][4] = {};
+    for (int k0 = 0; k0 < g.k2; k0 += KB) {
+        for (int e = threadIdx.x; e < TI * KB; e += 256) {
+            const int r = e / KB, kk = e % KB;
+            const int i = i0 + r;
+            sA[r][kk] = i < g.M ? plane_val(a_hi, a_lo, (size_t)i * g.k2 + k0 + kk) : 0.f;
+            const int t = t0 + r;   // t < Tpad always (grid covers padded templates)
+            const size_t row_re = (size_t)(t / kGemmTT) * 2 * kGemmTT + (t % kGemmTT);
+            sRe[r][kk] = plane_val(c_hi, c_lo, row_re * g.k2 + k0 + kk);
+            sIm[r][kk] = plane_val(c_hi, c_lo, (row_re + kGemmTT) * g.k2 + k0 + kk);
+        }
+        __syncthreads();
+#pragma unroll 4
+        for (int kk = 0; kk < KB; ++kk) {
+            float av[4], rv[4], iv[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { av[u] = sA[ty * 4 + u][kk]; rv[u] = sRe[tx * 4 + u][kk]; iv[u] = sIm[tx * 4 + u][kk]; }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int v = 0; v < 4; ++v) { re[u][v] = fmaf(av[u], rv[v], re[u][v]); im[u][v] = fmaf(av[u], iv[v], im[u][v]); }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            const int i = i0 + ty * 4 + u, t = t0 + tx * 4 + v;
+            if (i < g.M && t < g.T && re[u][v] * re[u][v] + im[u][v] * im[u][v] >= g.thr1_sq) {
+                const unsigned long long idx = atomicAdd(g.counters, 1ULL);
+                if (idx < g.cand_cap) {
+                    rbmf_candidate cd;
+                    cd.template_id = t; cd.bin_index = i; cd.avg_re = re[u][v]; cd.avg_im = im[u][v];
+                    g.cand[idx] = cd;
+                }
+            }
+        }
+}
+
+cudaError_t launch_gemm_simt(const uint16_t* a_hi, const uint16_t* a_lo, const uint16_t* c_hi, const uint16_t* c_lo,
+                             const GemmArgs& g, cudaStream_t st) {
+    dim3 grid((unsigned)((g.M + 63) / 64), (unsigned)(g.num_tb * kGemmTT / 64));
+    gemm_simt_kernel<<<grid, 256, 0, st>>>(a_hi, a_lo, c_hi, c_lo, g);
+    return cudaGetLastError();
+}
+
+}  // namespace rbmf

@@ -1,0 +1,248 @@
+"""Thin ctypes binding of librbmf.so (include/rbmf.h): argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels.  torch is used for device memory and streams.
+Importing this module raises ImportError when the library has not been built -- there is no fallback of any kind.
+The module-level functions carry the C names (rbmf_plan_create, rbmf_set_basis, rbmf_set_coeffs, rbmf_filter, ...);
+`Plan` is a small convenience wrapper that owns the workspace tensor.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_PKG_DIR = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG_DIR, "librbmf.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        "librbmf.so is not built (%s missing). Build it with `python -m paper_2110_13115_b200.build` "
+        "or `python -c 'import __graft_entry__ as g; g.build()'`. There is no CPU fallback." % LIB_PATH)
+
+_lib = ctypes.CDLL(LIB_PATH)
+
+RBMF_OK, RBMF_ERR_ARG, RBMF_ERR_STATE, RBMF_ERR_CUDA, RBMF_ERR_OVERFLOW, RBMF_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
+RBMF_GEMM_TCGEN05, RBMF_GEMM_SIMT = 0, 1
+
+TRIGGER_DTYPE = np.dtype([("template", np.int32), ("time", np.int32), ("re", np.float32), ("im", np.float32)])
+CANDIDATE_DTYPE = np.dtype([("template", np.int32), ("bin", np.int32), ("re", np.float32), ("im", np.float32)])
+
+# name -> (restype, argtypes); this table is also what tests/test_abi.py checks against include/rbmf.h
+_vp, _i32, _i64, _f32, _f64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c_double
+_pi32, _pi64, _psz = ctypes.POINTER(_i32), ctypes.POINTER(_i64), ctypes.POINTER(ctypes.c_size_t)
+SIGNATURES = {
+    "rbmf_plan_create": (_i32, [ctypes.POINTER(_vp), _i64, _f64, _f64, _i32, _i32]),
+    "rbmf_plan_set_window": (_i32, [_vp, _i32]),
+    "rbmf_plan_set_capacity": (_i32, [_vp, _i64, _i64]),
+    "rbmf_plan_set_gemm_impl": (_i32, [_vp, _i32]),
+    "rbmf_workspace_bytes": (_i32, [_vp, _psz]),
+    "rbmf_plan_set_workspace": (_i32, [_vp, _vp, ctypes.c_size_t]),
+    "rbmf_set_stream": (_i32, [_vp, _vp]),
+    "rbmf_set_basis": (_i32, [_vp, _vp]),
+    "rbmf_set_coeffs": (_i32, [_vp, _vp, _vp]),
+    "rbmf_filter": (_i32, [_vp, _vp, _f32, _f32, _vp, _vp]),
+    "rbmf_filter_host": (_i32, [_vp, _vp, _f32, _f32, _vp, _i64, _pi64]),
+    "rbmf_get_counts": (_i32, [_vp, _pi64, _pi64]),
+    "rbmf_get_candidates": (_i32, [_vp, _vp, _i64, _pi64]),
+    "rbmf_get_internal": (_i32, [_vp, _i32, ctypes.POINTER(_vp), _psz]),
+    "rbmf_plan_set_timing": (_i32, [_vp, _i32]),
+    "rbmf_get_stage_ms": (_i32, [_vp, ctypes.POINTER(_f32)]),
+    "rbmf_launches_per_filter": (_i32, [_vp, _pi32]),
+    "rbmf_plan_destroy": (_i32, [_vp]),
+    "rbmf_status_string": (ctypes.c_char_p, [_i32]),
+    "rbmf_last_cuda_error": (_i32, [_vp]),
+}
+for _name, (_res, _args) in SIGNATURES.items():
+    _fn = getattr(_lib, _name)          # AttributeError here = library does not export what rbmf.h declares
+    _fn.restype, _fn.argtypes = _res, _args
+    globals()[_name] = _fn
+
+
+class RbmfError(RuntimeError):
+    def __init__(self, status, where, cuda=0):
+        self.status = status
+        msg = _lib.rbmf_status_string(status).decode()
+        super().__init__("%s: %s (status %d, cuda error %d)" % (where, msg, status, cuda))
+
+
+def _ptr(t):
+    """Device (or host) address of a torch tensor / numpy array; None -> NULL."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+class Plan:
+    """Owns an rbmf_plan and its workspace tensor.  All tensors handed in must live on the plan's CUDA device."""
+
+    def __init__(self, N, fs, f_low, k, T, w=8, max_candidates=1 << 22, max_triggers=1 << 22, device="cuda:0",
+                 stream=None):
+        import torch
+        self._torch = torch
+        self.N, self.fs, self.f_low, self.k, self.T, self.w = int(N), float(fs), float(f_low), int(k), int(T), int(w)
+        self.max_candidates, self.max_triggers = int(max_candidates), int(max_triggers)
+        self.device = torch.device(device)
+        self._h = _vp()
+        self._check(_lib.rbmf_plan_create(ctypes.byref(self._h), self.N, self.fs, self.f_low, self.k, self.T),
+                    "rbmf_plan_create")
+        self._check(_lib.rbmf_plan_set_window(self._h, self.w), "rbmf_plan_set_window")
+        self._check(_lib.rbmf_plan_set_capacity(self._h, self.max_candidates, self.max_triggers),
+                    "rbmf_plan_set_capacity")
+        nbytes = ctypes.c_size_t()
+        self._check(_lib.rbmf_workspace_bytes(self._h, ctypes.byref(nbytes)), "rbmf_workspace_bytes")
+        self.workspace_bytes = nbytes.value
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(self.workspace_bytes + 1024, dtype=torch.uint8, device=self.device)
+            base = (self._ws.data_ptr() + 1023) // 1024 * 1024
+            self.set_stream(stream)
+            self._check(_lib.rbmf_plan_set_workspace(self._h, base, self.workspace_bytes), "rbmf_plan_set_workspace")
+            self._out = torch.empty(self.max_triggers * 4, dtype=torch.int32, device=self.device)
+            self._n_out = torch.zeros(1, dtype=torch.int64, device=self.device)
+        self._keep = []
+
+    # -- helpers -----------------------------------------------------------------------------
+    def _check(self, status, where, allow=()):
+        if status != RBMF_OK and status not in allow:
+            cuda = _lib.rbmf_last_cuda_error(self._h) if self._h else 0
+            raise RbmfError(status, where, cuda)
+        return status
+
+    def set_stream(self, stream=None):
+        torch = self._torch
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        self._check(_lib.rbmf_set_stream(self._h, _vp(stream.cuda_stream)), "rbmf_set_stream")
+
+    def _dev(self, x, dtype):
+        torch = self._torch
+        t = torch.as_tensor(x)
+        if t.dtype != dtype:
+            raise TypeError("expected %s, got %s" % (dtype, t.dtype))
+        return t.to(self.device).contiguous()
+
+    # -- ABI calls ---------------------------------------------------------------------------
+    def set_gemm_impl(self, impl):
+        self._check(_lib.rbmf_plan_set_gemm_impl(self._h, int(impl)), "rbmf_plan_set_gemm_impl")
+
+    def set_timing(self, enabled=True):
+        self._check(_lib.rbmf_plan_set_timing(self._h, 1 if enabled else 0), "rbmf_plan_set_timing")
+
+    def set_basis(self, basis):
+        torch = self._torch
+        b = self._dev(basis, torch.complex64)
+        if tuple(b.shape) != (self.k, self.N // 2 + 1):
+            raise ValueError("basis must be k x (N/2+1)")
+        with torch.cuda.device(self.device):
+            self._check(_lib.rbmf_set_basis(self._h, _ptr(b)), "rbmf_set_basis")
+        self.stream.synchronize()      # the library has copied; `b` may go away
+
+    def set_coeffs(self, coeffs, sigma=None):
+        torch = self._torch
+        c = self._dev(coeffs, torch.complex64)
+        if tuple(c.shape) != (self.T, self.k):
+            raise ValueError("coeffs must be T x k")
+        s = None if sigma is None else self._dev(sigma, torch.float32)
+        if s is not None and tuple(s.shape) != (self.T,):
+            raise ValueError("sigma must have T entries")
+        with torch.cuda.device(self.device):
+            self._check(_lib.rbmf_set_coeffs(self._h, _ptr(c), _ptr(s)), "rbmf_set_coeffs")
+        self.stream.synchronize()
+
+    def filter_async(self, strain_dev, thr1, thr2):
+        """Enqueue rbmf_filter on the plan's stream; strain_dev is a complex64 CUDA tensor of N/2+1 bins."""
+        torch = self._torch
+        if strain_dev.dtype != torch.complex64 or strain_dev.numel() != self.N // 2 + 1 or not strain_dev.is_cuda:
+            raise ValueError("strain must be a complex64 CUDA tensor with N/2+1 entries")
+        with torch.cuda.device(self.device):
+            self._check(_lib.rbmf_filter(self._h, _ptr(strain_dev), float(thr1), float(thr2), _ptr(self._out),
+                                         _ptr(self._n_out)), "rbmf_filter")
+
+    def counts(self, allow_overflow=False):
+        nc, nt = _i64(), _i64()
+        st = self._check(_lib.rbmf_get_counts(self._h, ctypes.byref(nc), ctypes.byref(nt)), "rbmf_get_counts",
+                         allow=(RBMF_ERR_OVERFLOW,) if allow_overflow else ())
+        return nc.value, nt.value, st
+
+    def triggers(self, allow_overflow=False):
+        """Synchronise and return the trigger list of the last filter call, sorted by (template, time)."""
+        nc, nt, _ = self.counts(allow_overflow)
+        n = min(nt, self.max_triggers)
+        raw = self._out[: 4 * n].cpu().numpy()
+        trig = raw.view(TRIGGER_DTYPE).copy() if n else np.empty(0, dtype=TRIGGER_DTYPE)
+        return np.sort(trig, order=("template", "time"))
+
+    def filter(self, strain, thr1, thr2, allow_overflow=False):
+        torch = self._torch
+        s = self._dev(strain, torch.complex64)
+        self.filter_async(s, thr1, thr2)
+        return self.triggers(allow_overflow)
+
+    def filter_host(self, strain_host, thr1, thr2, out_host=None):
+        """rbmf_filter_host: host strain in, host triggers out (unsorted); returns (array view, total found)."""
+        torch = self._torch
+        if out_host is None:
+            out_host = np.empty(self.max_triggers, dtype=TRIGGER_DTYPE)
+        n = _i64()
+        with torch.cuda.device(self.device):
+            st = _lib.rbmf_filter_host(self._h, _ptr(strain_host), float(thr1), float(thr2), _ptr(out_host),
+                                       len(out_host), ctypes.byref(n))
+        self._check(st, "rbmf_filter_host", allow=(RBMF_ERR_OVERFLOW,))
+        return out_host[: min(n.value, len(out_host))], n.value
+
+    def candidates(self):
+        nc, _, _ = self.counts(allow_overflow=True)
+        n = min(nc, self.max_candidates)
+        out = np.empty(max(n, 1), dtype=CANDIDATE_DTYPE)
+        tot = _i64()
+        self._check(_lib.rbmf_get_candidates(self._h, _ptr(out), n, ctypes.byref(tot)), "rbmf_get_candidates",
+                    allow=(RBMF_ERR_OVERFLOW,))
+        return np.sort(out[:n], order=("template", "bin"))
+
+    def internal(self, which):
+        """Copy of an internal array: 'beta' -> (N, k) complex64; 'beta_avg' -> (N/w, k) complex64 (hi + lo)."""
+        torch = self._torch
+        self.stream.synchronize()
+
+        def view(idx):
+            p, nb = _vp(), ctypes.c_size_t()
+            self._check(_lib.rbmf_get_internal(self._h, idx, ctypes.byref(p), ctypes.byref(nb)), "rbmf_get_internal")
+            off = p.value - self._ws.data_ptr()
+            return self._ws[off: off + nb.value]
+
+        if which == "beta":
+            return torch.view_as_complex(view(0).view(torch.float32).view(self.N, self.k, 2)).cpu().numpy()
+        if which == "beta_avg":
+            hi = view(1).view(torch.bfloat16).to(torch.float32)
+            lo = view(2).view(torch.bfloat16).to(torch.float32)
+            v = (hi + lo).view(self.N // self.w, self.k, 2)
+            return torch.view_as_complex(v.contiguous()).cpu().numpy()
+        raise KeyError(which)
+
+    def stage_ms(self):
+        ms = (_f32 * 4)()
+        self._check(_lib.rbmf_get_stage_ms(self._h, ms), "rbmf_get_stage_ms")
+        return {"fft": ms[0], "gemm": ms[1], "stage2": ms[2], "total": ms[3]}
+
+    def launches_per_filter(self):
+        n = _i32()
+        self._check(_lib.rbmf_launches_per_filter(self._h, ctypes.byref(n)), "rbmf_launches_per_filter")
+        return n.value
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            try:
+                self._torch.cuda.synchronize(self.device)
+            except Exception:
+                pass
+            _lib.rbmf_plan_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -221,6 +221,29 @@ def _spa_templates_cols(mc_msun: np.ndarray, cfg: WorkloadConfig, device, a: int
     return torch.polar(amp[None, :].expand(len(mc_msun), -1).contiguous(), phase)
 
 
+def make_strain(wl: dict, segment: int) -> tuple:
+    """Another strain segment for the same bank: segment 0 is `wl['strain']` itself; segment s > 0 draws fresh
+    noise and fresh injections (same count and SNR range) from default_rng(seed * 1000 + s).
+    Returns (strain complex64 (bins,), injections)."""
+    cfg = wl["config"]
+    if segment == 0:
+        return wl["strain"], wl["injections"]
+    rng = np.random.default_rng(cfg.seed * 1000 + int(segment))
+    N, bins = cfg.N, cfg.bins
+    d = np.fft.rfft(rng.standard_normal(N))
+    injections = []
+    jj = np.arange(bins, dtype=np.float64)
+    for _ in range(cfg.n_inj):
+        A = float(rng.uniform(cfg.snr_lo, cfg.snr_hi)) if cfg.snr_hi > cfg.snr_lo else float(cfg.snr_lo)
+        t = int(rng.integers(0, cfg.T))
+        n0 = int(rng.integers(0, N))
+        phi = float(rng.uniform(0.0, 2.0 * math.pi))
+        injections.append({"snr": A, "template": t, "n0": n0, "phase": phi})
+        u = _spa_templates(wl["mc"][t:t + 1], cfg, "cpu")[0].numpy()
+        d = d + A * math.sqrt(N / 2.0) * u * np.exp(-2j * np.pi * ((jj * n0) % N) / N) * np.exp(1j * phi)
+    return d.astype(np.complex64), injections
+
+
 def bank_templates(wl: dict, idx, device: Optional[str] = None) -> np.ndarray:
     """Unit-norm bank templates u_t for the listed template indices, (len, bins) complex128."""
     cfg = wl["config"]

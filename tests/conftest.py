@@ -24,3 +24,10 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(scope="session")
+def built_library():
+    """librbmf.so, (re)built in-tree from csrc/ if the sources changed (nvcc cross-compiles without a GPU)."""
+    from paper_2110_13115_b200 import build
+    return build.build()

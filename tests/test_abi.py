@@ -1,0 +1,124 @@
+"""Host-side checks of the C-ABI library: it loads, exports every symbol include/rbmf.h declares, validates its
+arguments and reports call-order errors.  No compute calls: none of this needs a GPU."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "rbmf.h")
+
+
+def _declared_symbols():
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(rbmf_[a-z0-9_]+)\s*\(", text)))
+
+
+@pytest.fixture(scope="module")
+def lib(built_library):
+    return ctypes.CDLL(built_library)
+
+
+@pytest.fixture(scope="module")
+def binding(built_library):
+    from paper_2110_13115_b200 import rbmf
+    return rbmf
+
+
+def test_header_symbols_are_exported(lib):
+    names = _declared_symbols()
+    assert len(names) >= 18 and "rbmf_filter" in names and "rbmf_plan_create" in names
+    for name in names:
+        assert hasattr(lib, name), "librbmf.so does not export %s" % name
+
+
+def test_binding_covers_the_header(binding):
+    assert sorted(binding.SIGNATURES) == _declared_symbols()
+
+
+def test_struct_sizes_match_header(binding):
+    assert binding.TRIGGER_DTYPE.itemsize == 16 and binding.CANDIDATE_DTYPE.itemsize == 16
+
+
+def _create(b, N=4096, fs=1024.0, f_low=30.0, k=16, T=64):
+    h = ctypes.c_void_p()
+    st = b.rbmf_plan_create(ctypes.byref(h), N, fs, f_low, k, T)
+    return st, h
+
+
+def test_plan_create_validates_arguments(binding):
+    b = binding
+    st, h = _create(b)
+    assert st == b.RBMF_OK and h.value
+    assert b.rbmf_plan_destroy(h) == b.RBMF_OK
+    for kw in (dict(N=4095), dict(N=512), dict(N=1 << 21), dict(k=20), dict(k=8), dict(k=2048), dict(T=0),
+               dict(f_low=0.0), dict(f_low=600.0), dict(fs=-1.0)):
+        st, h = _create(b, **kw)
+        assert st == b.RBMF_ERR_ARG and not h.value, kw
+    assert b.rbmf_plan_create(None, 4096, 1024.0, 30.0, 16, 64) == b.RBMF_ERR_ARG
+
+
+def test_window_capacity_and_workspace_size(binding):
+    b = binding
+    st, h = _create(b)
+    nbytes = ctypes.c_size_t()
+    assert b.rbmf_workspace_bytes(h, ctypes.byref(nbytes)) == b.RBMF_OK
+    default_bytes = nbytes.value
+    # beta (N k 8) + Y + basis^T alone are 2.5 N k 8 bytes
+    assert default_bytes > 2.5 * 4096 * 16 * 8
+    for w in (0, 3, 64, 8):          # 8: N/w = 512 < 1024
+        assert b.rbmf_plan_set_window(h, w) == b.RBMF_ERR_ARG
+    assert b.rbmf_plan_set_window(h, 4) == b.RBMF_OK
+    assert b.rbmf_plan_set_capacity(h, 0, 10) == b.RBMF_ERR_ARG
+    assert b.rbmf_plan_set_capacity(h, 1000, 1000) == b.RBMF_OK
+    assert b.rbmf_workspace_bytes(h, ctypes.byref(nbytes)) == b.RBMF_OK
+    assert nbytes.value < default_bytes          # smaller lists
+    n = ctypes.c_int32()
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 7
+    assert b.rbmf_plan_set_window(h, 1) == b.RBMF_OK
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 5
+    assert b.rbmf_plan_set_gemm_impl(h, 7) == b.RBMF_ERR_ARG
+    assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_SIMT) == b.RBMF_OK
+    b.rbmf_plan_destroy(h)
+
+
+def test_call_order_errors_without_workspace(binding):
+    b = binding
+    st, h = _create(b)
+    dummy = ctypes.c_void_p(1024)
+    assert b.rbmf_set_basis(h, dummy) == b.RBMF_ERR_STATE
+    assert b.rbmf_set_coeffs(h, dummy, None) == b.RBMF_ERR_STATE
+    assert b.rbmf_filter(h, dummy, 5.0, 6.0, dummy, dummy) == b.RBMF_ERR_STATE
+    assert b.rbmf_filter(h, dummy, -1.0, 6.0, dummy, dummy) == b.RBMF_ERR_ARG
+    assert b.rbmf_filter(h, None, 5.0, 6.0, dummy, dummy) == b.RBMF_ERR_ARG
+    assert b.rbmf_get_counts(h, None, None) == b.RBMF_ERR_STATE
+    # misaligned / too small workspace is rejected before any CUDA call
+    assert b.rbmf_plan_set_workspace(h, ctypes.c_void_p(1000), 1 << 40) == b.RBMF_ERR_ARG
+    assert b.rbmf_plan_set_workspace(h, ctypes.c_void_p(1024), 16) == b.RBMF_ERR_ARG
+    b.rbmf_plan_destroy(h)
+
+
+def test_status_strings(binding):
+    b = binding
+    seen = set()
+    for code in (0, -1, -2, -3, -4, -5):
+        s = b.rbmf_status_string(code)
+        assert s and s not in seen
+        seen.add(s)
+    assert b.rbmf_status_string(-99) == b"unknown status"
+
+
+def test_product_path_does_not_import_the_oracle():
+    """The oracle is test infrastructure: nothing under the package may import it (and vice versa)."""
+    pkg = os.path.join(ROOT, "paper_2110_13115_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in text and "from oracle" not in text, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith(".py"):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2110_13115_b200" not in text and "from paper_2110_13115_b200" not in text, f

@@ -1,0 +1,317 @@
+"""Parity of the CUDA path (through the C ABI) with the fp64 oracle, element by element on the same seeded inputs.
+
+Bars (BASELINE.json north_star): trigger sets identical under the tau = 1e-3 tie band,
+per-trigger |SNR| within 1e-3 relative and phase within 1e-3 rad; beta within 1e-5 absolute of the oracle's fp64
+series (output rms 1.41); beta^avg within 3e-5 (bf16 hi+lo storage, 2^-17 relative per value, plus the FFT error).
+"""
+import numpy as np
+import pytest
+
+from oracle import compare
+from oracle import rbmf_oracle as orc
+from paper_2110_13115_b200 import workloads as wlm
+
+pytestmark = pytest.mark.gpu
+
+BETA_ATOL = 1e-5
+BETA_AVG_ATOL = 3e-5
+
+
+@pytest.fixture(scope="module")
+def rbmf(built_library):
+    from paper_2110_13115_b200 import rbmf as mod
+    return mod
+
+
+_WL = {}
+
+
+def workload(name, **kw):
+    key = (name, tuple(sorted(kw.items())))
+    if key not in _WL:
+        cfg = wlm.CONFIGS[name]
+        if kw:
+            cfg = cfg.replace(**kw)
+        _WL[key] = wlm.make_workload(cfg, device="cuda")
+    return _WL[key]
+
+
+def make_plan(rbmf, wl, w=None, **kw):
+    import torch
+    cfg = wl["config"]
+    plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w if w is None else w,
+                     max_candidates=kw.pop("max_candidates", 1 << 20), max_triggers=kw.pop("max_triggers", 1 << 20))
+    plan.set_basis(torch.from_numpy(wl["basis"]))
+    plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+    return plan
+
+
+def oracle(wl, w, thr1, thr2, templates=None):
+    cfg = wl["config"]
+    return orc.oracle_filter(wl["strain"], wl["basis"], wl["coeffs"], wl["sigma"], cfg.N, cfg.fs, cfg.f_low, w,
+                             thr1, thr2, templates=templates)
+
+
+def check(rbmf, wl, w, thr1, thr2, impl=0, expect_triggers=True):
+    import torch
+    cfg = wl["config"]
+    plan = make_plan(rbmf, wl, w=w)
+    plan.set_gemm_impl(impl)
+    got = plan.filter(torch.from_numpy(wl["strain"]), thr1, thr2)
+    ref = oracle(wl, w, thr1, thr2)
+    rep = compare.compare_triggers(got, ref, cfg.N, thr1, thr2)
+    cand = plan.candidates()
+    crep = compare.compare_candidates(cand, ref, cfg.N // w, thr1)
+    plan.close()
+    assert rep["ok"], rep
+    assert crep["ok"], crep
+    if expect_triggers:
+        assert rep["n_got"] > 0 and rep["n_mandatory"] > 0
+    return rep, crep
+
+
+# ------------------------------------------------------------------------------------------ kernel 1
+@pytest.mark.parametrize("name", ["tiny", "mini"])
+def test_beta_matches_oracle_series(rbmf, name):
+    import torch
+    wl = workload(name)
+    cfg = wl["config"]
+    plan = make_plan(rbmf, wl)
+    plan.filter(torch.from_numpy(wl["strain"]), 50.0, 50.0)
+    beta = plan.internal("beta")                       # (N, k)
+    bavg = plan.internal("beta_avg")                   # (N/w, k)
+    plan.close()
+    ref = orc.basis_series(wl["strain"], wl["basis"], cfg.N, cfg.j_low)   # (k, N) fp64
+    assert abs(np.sqrt((np.abs(ref) ** 2).mean()) - np.sqrt(2.0)) < 0.2   # unit-variance quadratures
+    err = np.abs(beta.T.astype(np.complex128) - ref).max()
+    assert err < BETA_ATOL, err
+    ref_avg = orc.bin_average(ref, cfg.w)
+    err_avg = np.abs(bavg.T.astype(np.complex128) - ref_avg).max()
+    assert err_avg < BETA_AVG_ATOL, err_avg
+
+
+@pytest.mark.parametrize("N,w", [(1024, 1), (2048, 2), (8192, 4), (32768, 16), (65536, 32)])
+def test_beta_all_fft_lengths(rbmf, N, w):
+    """Every pass length the dispatcher can pick (L = 32 .. 1024 appear over these sizes, incl. the folded transform)."""
+    import torch
+    wl = workload("tiny", N=N, T=16, n_inj=0, index=50 + w)
+    cfg = wl["config"]
+    plan = make_plan(rbmf, wl, w=w)
+    plan.filter(torch.from_numpy(wl["strain"]), 50.0, 50.0)
+    beta, bavg = plan.internal("beta"), plan.internal("beta_avg")
+    plan.close()
+    ref = orc.basis_series(wl["strain"], wl["basis"], cfg.N, cfg.j_low)
+    assert np.abs(beta.T.astype(np.complex128) - ref).max() < BETA_ATOL
+    assert np.abs(bavg.T.astype(np.complex128) - orc.bin_average(ref, w)).max() < BETA_AVG_ATOL
+
+
+def test_beta_largest_length_sampled(rbmf):
+    """N = 2^20 (1024 x 1024 passes): sampled columns against the oracle's fp64 series."""
+    import torch
+    wl = workload("tiny", N=1 << 20, fs=4096.0, f_low=20.0, T=16, n_inj=0, index=60)
+    cfg = wl["config"]
+    plan = make_plan(rbmf, wl, w=8)
+    plan.filter(torch.from_numpy(wl["strain"]), 50.0, 50.0)
+    beta, bavg = plan.internal("beta"), plan.internal("beta_avg")
+    plan.close()
+    cols = [0, 7, 15]
+    ref = orc.basis_series(wl["strain"], wl["basis"][cols], cfg.N, cfg.j_low)
+    assert np.abs(beta[:, cols].T.astype(np.complex128) - ref).max() < BETA_ATOL
+    assert np.abs(bavg[:, cols].T.astype(np.complex128) - orc.bin_average(ref, 8)).max() < BETA_AVG_ATOL
+
+
+# ------------------------------------------------------------------------------- whole path, exhaustive
+@pytest.mark.parametrize("impl", [0, 1])
+@pytest.mark.parametrize("thr", [(3.0, 4.0), (5.0, 6.0)])
+def test_tiny_exhaustive(rbmf, impl, thr):
+    check(rbmf, workload("tiny"), 4, thr[0], thr[1], impl=impl)
+
+
+def test_tiny_narrow_exhaustive(rbmf):
+    rep, _ = check(rbmf, workload("tiny_narrow"), 4, 5.0, 6.0)
+    assert rep["n_got"] > 0
+
+
+@pytest.mark.parametrize("w", [1, 2, 4, 8, 16])
+def test_mini_all_windows(rbmf, w):
+    """N = 16384, k = 32, T = 300 (ragged against the 128-template tile), 3 injections."""
+    check(rbmf, workload("mini"), w, 4.0, 5.0)
+
+
+def test_mini_simt_and_tensor_core_candidates_agree(rbmf):
+    import torch
+    wl = workload("mini")
+    cfg = wl["config"]
+    sets = []
+    for impl in (0, 1):
+        plan = make_plan(rbmf, wl)
+        plan.set_gemm_impl(impl)
+        plan.filter(torch.from_numpy(wl["strain"]), 3.5, 4.5)
+        sets.append(plan.candidates())
+        plan.close()
+    a, b = sets
+    ka = a["template"].astype(np.int64) * cfg.N + a["bin"]
+    kb = b["template"].astype(np.int64) * cfg.N + b["bin"]
+    sym = np.setxor1d(ka, kb)
+    assert len(ka) > 1000
+    assert len(sym) <= max(2, len(ka) // 2000)          # only threshold ties may differ
+    common, ia, ib = np.intersect1d(ka, kb, return_indices=True)
+    assert np.abs(a["re"][ia] - b["re"][ib]).max() < 2e-4 and np.abs(a["im"][ia] - b["im"][ib]).max() < 2e-4
+
+
+def test_small_config_exhaustive(rbmf):
+    """BASELINE.json configs[1]: N = 131072, k = 128, T = 2000, w = 8, thresholds 5.0 / 6.0, 10 injections."""
+    rep, crep = check(rbmf, workload("small"), 8, 5.0, 6.0)
+    assert rep["n_got"] > 100
+
+
+def test_small_narrow_recovers_injections(rbmf):
+    """Narrow-Mc bank (truncation tolerance holds): every injection is recovered near its injected SNR."""
+    import torch
+    wl = workload("small_narrow")
+    cfg = wl["config"]
+    assert 1.0 - wl["captured"] < 1e-4
+    plan = make_plan(rbmf, wl)
+    got = plan.filter(torch.from_numpy(wl["strain"]), 5.0, 6.0)
+    plan.close()
+    ref = oracle(wl, 8, 5.0, 6.0, templates=sorted({i["template"] for i in wl["injections"]}))
+    sub = got[np.isin(got["template"], ref["triggers"]["template"])]
+    rep = compare.compare_triggers(sub, ref, cfg.N, 5.0, 6.0)
+    assert rep["ok"], rep
+    for inj in wl["injections"]:
+        if inj["snr"] < 8.0:
+            continue
+        m = (got["template"] == inj["template"]) & (np.abs(got["time"] - inj["n0"]) <= 1)
+        assert m.any(), inj
+        peak = np.hypot(got["re"][m], got["im"][m]).max()
+        assert abs(peak - inj["snr"]) < 3.5, (peak, inj)          # injected SNR +- noise
+
+
+# ----------------------------------------------------------------------------------------- edge cases
+def test_no_triggers_and_repeatability(rbmf):
+    import torch
+    wl = workload("tiny")
+    plan = make_plan(rbmf, wl)
+    s = torch.from_numpy(wl["strain"])
+    assert len(plan.filter(s, 40.0, 40.0)) == 0
+    assert plan.counts()[:2] == (0, 0)
+    a = plan.filter(s, 3.0, 4.0)
+    b = plan.filter(s, 3.0, 4.0)
+    assert len(a) > 0 and np.array_equal(a, b)           # set content is deterministic
+    plan.close()
+
+
+def test_zero_strain_gives_nothing(rbmf):
+    import torch
+    wl = workload("tiny")
+    plan = make_plan(rbmf, wl)
+    assert len(plan.filter(torch.zeros(wl["config"].bins, dtype=torch.complex64), 1.0, 1.0)) == 0
+    plan.close()
+
+
+def test_overflow_is_reported_and_bounded(rbmf):
+    import torch
+    wl = workload("tiny")
+    plan = make_plan(rbmf, wl, max_candidates=64, max_triggers=16)
+    plan.filter_async(torch.from_numpy(wl["strain"]).cuda(), 2.0, 2.0)
+    nc, nt, st = plan.counts(allow_overflow=True)
+    assert st == rbmf.RBMF_ERR_OVERFLOW and nc > 64
+    trig = plan.triggers(allow_overflow=True)
+    assert len(trig) <= 16
+    with pytest.raises(rbmf.RbmfError):
+        plan.counts()
+    plan.close()
+    # triggers-only overflow: candidate list large enough, trigger list too small
+    plan = make_plan(rbmf, wl, max_candidates=1 << 18, max_triggers=16)
+    plan.filter_async(torch.from_numpy(wl["strain"]).cuda(), 2.0, 2.0)
+    nc, nt, st = plan.counts(allow_overflow=True)
+    ref = oracle(wl, 4, 2.0, 2.0)
+    assert st == rbmf.RBMF_ERR_OVERFLOW and abs(nt - len(ref["triggers"])) <= max(5, len(ref["near"]) - len(ref["triggers"]))
+    plan.close()
+
+
+def test_sigma_null_uses_coefficient_norm(rbmf):
+    import torch
+    wl = workload("tiny")
+    cfg = wl["config"]
+    plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, max_candidates=1 << 18, max_triggers=1 << 18)
+    plan.set_basis(torch.from_numpy(wl["basis"]))
+    plan.set_coeffs(torch.from_numpy(wl["coeffs"]), None)
+    got = plan.filter(torch.from_numpy(wl["strain"]), 3.0, 4.0)
+    plan.close()
+    sig = np.linalg.norm(wl["coeffs"].astype(np.complex128), axis=1).astype(np.float32)
+    ref = orc.oracle_filter(wl["strain"], wl["basis"], wl["coeffs"], sig, cfg.N, cfg.fs, cfg.f_low, cfg.w, 3.0, 4.0)
+    assert compare.compare_triggers(got, ref, cfg.N, 3.0, 4.0)["ok"]
+
+
+def test_unit_sigma_is_the_papers_convention(rbmf):
+    """sigma_t = 1 (templates 'normalized to unity'): SNRs scale by ||c_t||."""
+    import torch
+    wl = workload("tiny")
+    cfg = wl["config"]
+    ones = np.ones(cfg.T, dtype=np.float32)
+    plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, max_candidates=1 << 18, max_triggers=1 << 18)
+    plan.set_basis(torch.from_numpy(wl["basis"]))
+    plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(ones))
+    got = plan.filter(torch.from_numpy(wl["strain"]), 2.0, 2.5)
+    plan.close()
+    ref = orc.oracle_filter(wl["strain"], wl["basis"], wl["coeffs"], ones, cfg.N, cfg.fs, cfg.f_low, cfg.w, 2.0, 2.5)
+    rep = compare.compare_triggers(got, ref, cfg.N, 2.0, 2.5)
+    assert rep["ok"] and rep["n_got"] > 0, rep
+
+
+def test_filter_host_matches_device_call(rbmf):
+    import torch
+    wl = workload("tiny")
+    plan = make_plan(rbmf, wl, max_candidates=1 << 16, max_triggers=1 << 16)
+    a = plan.filter(torch.from_numpy(wl["strain"]), 3.0, 4.0)
+    pinned = torch.from_numpy(wl["strain"]).pin_memory()
+    out, n = plan.filter_host(pinned.numpy(), 3.0, 4.0)
+    plan.close()
+    assert n == len(a)
+    assert np.array_equal(np.sort(out, order=("template", "time")), a)
+
+
+def test_non_default_stream(rbmf):
+    import torch
+    wl = workload("tiny")
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        plan = make_plan(rbmf, wl)
+        a = plan.filter(torch.from_numpy(wl["strain"]), 3.0, 4.0)
+        plan.close()
+    ref = oracle(wl, 4, 3.0, 4.0)
+    assert compare.compare_triggers(a, ref, wl["config"].N, 3.0, 4.0)["ok"]
+
+
+# ------------------------------------------------------------- full size, bench launch configuration
+def test_paper_scale_sampled(rbmf):
+    """BASELINE.json configs[2] (N = 524288, k = 256, T = 20000, w = 8; what bench.py times): soundness of sampled
+    reported triggers by pointwise O(|B|) re-evaluation (no FFT), completeness on a template subset (all injected
+    templates + seeded random ones) by the exhaustive oracle."""
+    import torch
+    wl = workload("paper")
+    cfg = wl["config"]
+    plan = make_plan(rbmf, wl, max_candidates=1 << 22, max_triggers=1 << 22)
+    got = plan.filter(torch.from_numpy(wl["strain"]), cfg.thr1, cfg.thr2)
+    nc, nt, _ = plan.counts()
+    plan.close()
+    assert nt == len(got) > 0 and nc > 0
+    rng = np.random.default_rng(5)
+    # soundness: sampled triggers re-evaluated one by one
+    pick = rng.choice(len(got), size=min(24, len(got)), replace=False)
+    for i in pick:
+        t, n = int(got["template"][i]), int(got["time"][i])
+        rho, rbar = orc.evaluate_points(wl["strain"], wl["basis"], wl["coeffs"], wl["sigma"], cfg.N, cfg.fs,
+                                        cfg.f_low, cfg.w, t, [n])
+        val = complex(got["re"][i], got["im"][i])
+        assert abs(abs(val) - abs(rho[0])) <= 1e-3 * abs(rho[0])
+        assert abs(np.angle(val * np.conj(rho[0]))) <= 1e-3
+        assert abs(rho[0]) >= cfg.thr2 * (1 - 1e-3) and abs(rbar[0]) >= cfg.thr1 * (1 - 1e-3)
+    # completeness on a subset of templates
+    subset = sorted({i["template"] for i in wl["injections"]} | set(rng.choice(cfg.T, 14, replace=False).tolist()))
+    ref = oracle(wl, cfg.w, cfg.thr1, cfg.thr2, templates=subset)
+    sub = got[np.isin(got["template"], subset)]
+    rep = compare.compare_triggers(sub, ref, cfg.N, cfg.thr1, cfg.thr2)
+    assert rep["ok"], rep
+    assert rep["n_mandatory"] > 0

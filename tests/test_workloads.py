@@ -1,0 +1,39 @@
+"""The seeded input generator: determinism, shapes, and that extra strain segments keep the bank."""
+import numpy as np
+
+from paper_2110_13115_b200 import workloads as wlm
+
+
+def test_tiny_workload_is_deterministic_and_shaped():
+    a = wlm.make_workload(wlm.CONFIGS["tiny"])
+    b = wlm.make_workload(wlm.CONFIGS["tiny"])
+    cfg = a["config"]
+    assert a["strain"].shape == (cfg.bins,) and a["strain"].dtype == np.complex64
+    assert a["basis"].shape == (cfg.k, cfg.bins) and a["basis"].dtype == np.complex64
+    assert a["coeffs"].shape == (cfg.T, cfg.k) and a["sigma"].shape == (cfg.T,) and a["sigma"].dtype == np.float32
+    for key in ("strain", "basis", "coeffs", "sigma"):
+        assert np.array_equal(a[key], b[key])
+    assert cfg.j_low == 120 and cfg.bins == 2049
+    assert len(a["injections"]) == 1 and a["injections"][0]["snr"] == 12.0
+
+
+def test_config_table_matches_baseline_json():
+    c = wlm.CONFIGS
+    assert (c["small"].N, c["small"].k, c["small"].T, c["small"].f_low) == (131072, 128, 2000, 25.0)
+    assert (c["paper"].N, c["paper"].k, c["paper"].T, c["paper"].n_inj) == (524288, 256, 20000, 50)
+    assert (c["large"].N, c["large"].k, c["large"].T, c["large"].fs) == (262144, 256, 100000, 4096.0)
+    assert c["paper"].j_low == 5120 and c["small"].j_low == 1600
+
+
+def test_extra_segments_share_the_bank():
+    wl = wlm.make_workload(wlm.CONFIGS["tiny"])
+    s0, inj0 = wlm.make_strain(wl, 0)
+    assert s0 is wl["strain"] and inj0 is wl["injections"]
+    s1, inj1 = wlm.make_strain(wl, 1)
+    s1b, _ = wlm.make_strain(wl, 1)
+    assert s1.shape == s0.shape and s1.dtype == np.complex64
+    assert np.array_equal(s1, s1b) and not np.array_equal(s1, s0)
+    assert len(inj1) == len(inj0)
+    # noise normalisation: |d[j]|^2 averages N for unit-variance white noise
+    cfg = wl["config"]
+    assert abs((np.abs(s1[10:-10]) ** 2).mean() / cfg.N - 1.0) < 0.15
