@@ -169,7 +169,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
     const uint32_t tmem_base = *tmem_slot_ptr;
 
     const int ntiles = num_tiles(g);
-    const int num_kb = g.k2 / BK;
+    const int num_kb = (g.k2 + BK - 1) / BK;   // a ragged last block is zero-filled by TMA (k2 = 32 when k = 16)
 
     if (warp == 0) {
         // ================================ TMA producer ================================
