@@ -170,8 +170,10 @@ fft_pass_kernel(const FftArgs a) {
     extern __shared__ float2 sm[];   // (L + L/16) rows x KC columns
 
     const int c = threadIdx.x % KC, wk = threadIdx.x / KC;
-    const int o = blockIdx.x;
-    const int col = blockIdx.y * KC + c;
+    // Column chunks are the fastest-varying block index: the CTAs that touch the two 64-byte halves of one 128-byte
+    // line run at the same time, so the second half is an L2 hit instead of a second DRAM fetch.
+    const int o = blockIdx.y;
+    const int col = blockIdx.x * KC + c;
     const float2* __restrict__ tw = a.tw_L;
     float2 u[EPT];
 
@@ -239,7 +241,7 @@ cudaError_t launch_one(const FftArgs& a, cudaStream_t st) {
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    dim3 grid((unsigned)a.lines, (unsigned)(a.k / KC));
+    dim3 grid((unsigned)(a.k / KC), (unsigned)a.lines);
     fft_pass_kernel<LOGL, MODE><<<grid, NT, smem, st>>>(a);
     return cudaGetLastError();
 }
