@@ -75,7 +75,7 @@ typedef enum {
  * max_candidates = max_triggers = 2^22.  *out is set to NULL on failure. */
 rbmf_status rbmf_plan_create(rbmf_plan** out, int64_t N, double fs, double f_low, int32_t k, int32_t T);
 
-/* Stage-1 averaging window w of Eq. 9 (power of two, 1 <= w <= 64, N/w >= 128).  w = 1 is the flat search.
+/* Stage-1 averaging window w of Eq. 9 (power of two, 1 <= w <= 32, N/w >= 128).  w = 1 is the flat search.
  * Must be called before rbmf_workspace_bytes / rbmf_plan_set_workspace. */
 rbmf_status rbmf_plan_set_window(rbmf_plan* plan, int32_t w);
 
@@ -98,7 +98,7 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
 rbmf_status rbmf_set_stream(rbmf_plan* plan, void* cuda_stream);
 
 /* basis_dev: k x (N/2+1) complex64, row-major: b_k[j] (p~_k of PAPER.md:82), orthonormal over the band.
- * Values outside the band are ignored.  Copied (transposed to bins x k) into the workspace. */
+ * Values outside the band are ignored.  Copied (re-laid-out in the order the FFT reads it) into the workspace. */
 rbmf_status rbmf_set_basis(rbmf_plan* plan, const void* basis_dev);
 
 /* coeffs_dev: T x k complex64, row-major: c_tk, unconjugated.  sigma_dev: T float32 template
@@ -128,8 +128,10 @@ rbmf_status rbmf_get_counts(rbmf_plan* plan, int64_t* n_candidates, int64_t* n_t
 rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64_t capacity, int64_t* n_out);
 
 /* Read-only device views of internal arrays for diagnostics and parity tests (valid after rbmf_filter on the
- * plan's stream, until the next call).  which: 0 = beta (N x k complex64, time-major),
- * 1 = beta^avg hi plane, 2 = beta^avg lo plane ((N/w) x 2k bfloat16 each; value = hi + lo).
+ * plan's stream, until the next call), in the library's blocked layouts:
+ *   which = 0: beta, complex64, [k/4 chunks][N samples][4 columns]: beta_c[n] at ((c/4) N + n) 4 + c%4;
+ *   which = 1 / 2: beta^avg hi / lo plane, bfloat16, [ceil(k/32) K blocks][N/w bins][32 columns][re, im]
+ *                  (value = hi + lo; columns >= k of the last block are zero).
  * *dev_ptr receives the address, *bytes the size. */
 rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_ptr, size_t* bytes);
 

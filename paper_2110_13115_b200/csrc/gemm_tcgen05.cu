@@ -71,6 +71,13 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         : "memory");
 }
 
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y, int z) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(dst),
+        "l"(map), "r"(bar), "r"(x), "r"(y), "r"(z)
+        : "memory");
+}
+
 // K-major operand tile in shared memory, 128-byte rows, SWIZZLE_128B: 8-row groups are 1024 B apart (SBO);
 // descriptor version 1 (sm_100), layout type 2 (SWIZZLE_128B).  Advancing along K by 16 bf16 = +32 B on the start
 // address (the hardware applies the XOR swizzle on the absolute shared-memory address bits).
@@ -183,8 +190,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
                     mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sbase = smem_base + stage * STAGE_BYTES;
                     mbar_expect_tx(full_bar(stage), STAGE_BYTES);
-                    tma_load_2d(sbase, &tmA_hi, full_bar(stage), kb * BK, ib * BM);
-                    tma_load_2d(sbase + A_BYTES, &tmA_lo, full_bar(stage), kb * BK, ib * BM);
+                    // beta^avg planes are K-block major, [kb][bin][64]: one box = 16 KB contiguous
+                    tma_load_3d(sbase, &tmA_hi, full_bar(stage), 0, ib * BM, kb);
+                    tma_load_3d(sbase + A_BYTES, &tmA_lo, full_bar(stage), 0, ib * BM, kb);
                     tma_load_2d(sbase + 2 * A_BYTES, &tmB_hi, full_bar(stage), kb * BK, tb * BN);
                     tma_load_2d(sbase + 2 * A_BYTES + B_BYTES, &tmB_lo, full_bar(stage), kb * BK, tb * BN);
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }

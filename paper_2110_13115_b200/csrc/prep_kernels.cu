@@ -1,4 +1,4 @@
-// Set-up kernels: constant tables, basis transpose, coefficient planes, per-call strain scaling.
+// Set-up kernels: constant tables, basis re-layout, coefficient planes, per-call strain scaling.
 // None of them is on the per-segment critical path except prep_strain (N/2 elements).
 #include <cuda_bf16.h>
 
@@ -16,75 +16,61 @@ __device__ __forceinline__ float2 unit_root(long long num, long long den) {
     return make_float2((float)c, (float)s);
 }
 
-__global__ void init_tables_kernel(float2* tw_L_all, float2* tw_lo_main, float2* tw_hi_main, float2* tw_lo_avg,
-                                   float2* tw_hi_avg, float2* S_table, long long N, long long M, int w) {
+// tw1[q * R0 + b] = e^{2 pi i q b / L} (stage-1 twiddles of a length-L = R0 * R1 line, q < R1, b < R0);
+// twN[j2 * L1 + n1] = e^{2 pi i j2 n1 / N} (inter-pass twiddles of the four-step FFT).
+__global__ void init_tables_kernel(float2* tw1_a, float2* tw1_b, float2* twN, int logL1, int logL2) {
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    // per-length tables, L = 32 .. 1024
-    if (i < kTwAllEntries) {
-        for (int logL = 5; logL <= 10; ++logL) {
-            const int L = 1 << logL;
-            const int off = tw_table_offset(logL);
-            if (i >= off && i < off + L) tw_L_all[i] = unit_root(i - off, L);
-        }
-    }
-    if (i < 1024) {
-        tw_lo_main[i] = unit_root(i, N);
-        tw_lo_avg[i] = unit_root(i, M);
-    }
-    const long long nh_main = N / 1024 > 0 ? N / 1024 : 1;
-    const long long nh_avg = M / 1024 > 0 ? M / 1024 : 1;
-    if (i < nh_main) tw_hi_main[i] = unit_root(i * 1024, N);
-    if (i < nh_avg) tw_hi_avg[i] = unit_root(i * 1024, M);
-    // S(j) = (1/w) sum_{r<w} e^{2 pi i j r / N}: the frequency response of the w-sample bin average
-    // (Eq. 10-11, :199-208); used to obtain beta^avg as a length-N/w inverse FFT (Eq. 12).
-    if (i < N / 2) {
-        double sr = 0.0, si = 0.0;
-        for (int r = 0; r < w; ++r) {
-            double s, c;
-            sincospi(2.0 * (double)((i * r) % N) / (double)N, &s, &c);
-            sr += c;
-            si += s;
-        }
-        S_table[i] = make_float2((float)(sr / w), (float)(si / w));
-    }
+    const int L1 = 1 << logL1, L2 = 1 << logL2;
+    const long long N = (long long)L1 * L2;
+    if (i < L1) { const int R0 = fft_r0(logL1); tw1_a[i] = unit_root((i / R0) * (i % R0), L1); }
+    if (i < L2) { const int R0 = fft_r0(logL2); tw1_b[i] = unit_root((i / R0) * (i % R0), L2); }
+    if (i < N) twN[i] = unit_root((i / L1) * (i % L1), N);
 }
 
-cudaError_t launch_init_tables(float2* tw_L_all, float2* tw_lo_main, float2* tw_hi_main, float2* tw_lo_avg,
-                               float2* tw_hi_avg, float2* S_table, int64_t N, int64_t M, int w, cudaStream_t st) {
-    long long n = N / 2 > 2048 ? N / 2 : 2048;
+cudaError_t launch_init_tables(float2* tw1_a, float2* tw1_b, float2* twN, int logL1, int logL2, cudaStream_t st) {
+    const long long n = 1LL << (logL1 + logL2);
     const int threads = 256;
-    init_tables_kernel<<<(unsigned)((n + threads - 1) / threads), threads, 0, st>>>(
-        tw_L_all, tw_lo_main, tw_hi_main, tw_lo_avg, tw_hi_avg, S_table, N, M, w);
+    init_tables_kernel<<<(unsigned)((n + threads - 1) / threads), threads, 0, st>>>(tw1_a, tw1_b, twN, logL1, logL2);
     return cudaGetLastError();
 }
 
-// ------------------------------------------------------------------------------ basis transpose
-// basis: k x bins (row-major, caller's layout)  ->  basisT: (N/2) x k, zero outside the band.
-__global__ void transpose_basis_kernel(const float2* __restrict__ basis, float2* __restrict__ basisT, int k,
-                                       long long bins, int j_low, int n_half) {
-    __shared__ float2 tile[32][33];
-    const long long j0 = (long long)blockIdx.x * 32;
-    const int c0 = blockIdx.y * 32;
-    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-        const int c = c0 + r;
-        const long long j = j0 + threadIdx.x;
-        float2 v = make_float2(0.f, 0.f);
-        if (c < k && j >= j_low && j < n_half) v = basis[(long long)c * bins + j];
-        tile[r][threadIdx.x] = v;
-    }
+// --------------------------------------------------------------------------------- basis re-layout
+// basis: k x bins (row-major, caller's layout)  ->  basisP[chunk][j2][j1 < L1/2][C] with j = j1 L2 + j2,
+// zero outside the band: the block a pass-1 tile reads is contiguous.
+__global__ void layout_basis_kernel(const float2* __restrict__ basis, float2* __restrict__ basisP, long long bins,
+                                    int j_low, int logL1, int logL2) {
+    __shared__ float2 tile[kFftC][32][33];
+    const int L2 = 1 << logL2, H = (1 << logL1) / 2;
+    const int chunk = blockIdx.z;
+    const int j2_0 = blockIdx.x * 32, j1_0 = blockIdx.y * 32;
+    const int tx = threadIdx.x % 32, ty = threadIdx.x / 32;   // 32 x 8
+    for (int c = 0; c < kFftC; ++c)
+        for (int r = ty; r < 32; r += 8) {
+            const int j1 = j1_0 + r, j2 = j2_0 + tx;
+            float2 v = make_float2(0.f, 0.f);
+            if (j1 < H && j2 < L2) {
+                const long long j = (long long)j1 * L2 + j2;
+                if (j >= j_low) v = basis[(long long)(chunk * kFftC + c) * bins + j];
+            }
+            tile[c][r][tx] = v;
+        }
     __syncthreads();
-    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-        const long long j = j0 + r;
-        const int c = c0 + threadIdx.x;
-        if (c < k && j < n_half) basisT[j * k + c] = tile[threadIdx.x][r];
+    // write: for each j2 of the tile, 32 j1 x C columns are contiguous
+    for (int r = ty; r < 32; r += 8) {
+        const int j2 = j2_0 + r;
+        if (j2 >= L2) continue;
+        for (int e = tx; e < 32 * kFftC; e += 32) {
+            const int j1 = j1_0 + e / kFftC, c = e % kFftC;
+            if (j1 < H) basisP[(((size_t)chunk * L2 + j2) * H + j1) * kFftC + c] = tile[c][e / kFftC][r];
+        }
     }
 }
 
-cudaError_t launch_transpose_basis(const float2* basis, float2* basisT, int k, int64_t bins, int j_low,
-                                   int n_half, cudaStream_t st) {
-    dim3 grid((unsigned)((n_half + 31) / 32), (unsigned)((k + 31) / 32));
-    dim3 block(32, 8);
-    transpose_basis_kernel<<<grid, block, 0, st>>>(basis, basisT, k, bins, j_low, n_half);
+cudaError_t launch_layout_basis(const float2* basis, float2* basisP, int k, int64_t bins, int j_low, int logL1,
+                                int logL2, cudaStream_t st) {
+    const int L2 = 1 << logL2, H = (1 << logL1) / 2;
+    dim3 grid((unsigned)((L2 + 31) / 32), (unsigned)((H + 31) / 32), (unsigned)(k / kFftC));
+    layout_basis_kernel<<<grid, 256, 0, st>>>(basis, basisP, bins, j_low, logL1, logL2);
     return cudaGetLastError();
 }
 
@@ -158,21 +144,21 @@ cudaError_t launch_prep_coeffs(const float2* coeffs, const float* sigma, float2*
 }
 
 // ------------------------------------------------------------------------------------ strain prep
-// ds[j] = s d[j] (s = sqrt(2/N));  dS[j] = ds[j] S(j)  (alias-fold weights, Eq. 12).
-__global__ void prep_strain_kernel(const float2* __restrict__ strain, const float2* __restrict__ S_table,
-                                   float2* __restrict__ ds, float2* __restrict__ dS, int n_half, float scale) {
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n_half) return;
+// dsT[j2][j1] = s d[j1 L2 + j2], j1 < L1/2 (s = sqrt(2/N)): the strain in the order pass 1
+// of the FFT reads it.
+__global__ void prep_strain_kernel(const float2* __restrict__ strain, float2* __restrict__ dsT, int logL1,
+                                   int logL2, float scale) {
+    const int L2 = 1 << logL2, H = (1 << logL1) / 2;
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;   // j = j1 L2 + j2 < N/2
+    if (j >= H * L2) return;
     const float2 d = strain[j];
-    const float2 v = make_float2(d.x * scale, d.y * scale);
-    ds[j] = v;
-    const float2 s = S_table[j];
-    dS[j] = make_float2(v.x * s.x - v.y * s.y, v.x * s.y + v.y * s.x);
+    dsT[(size_t)(j % L2) * H + j / L2] = make_float2(d.x * scale, d.y * scale);
 }
 
-cudaError_t launch_prep_strain(const float2* strain, const float2* S_table, float2* ds, float2* dS, int n_half,
-                               float scale, cudaStream_t st) {
-    prep_strain_kernel<<<(n_half + 255) / 256, 256, 0, st>>>(strain, S_table, ds, dS, n_half, scale);
+cudaError_t launch_prep_strain(const float2* strain, float2* dsT, int logL1, int logL2, float scale,
+                               cudaStream_t st) {
+    const int n_half = 1 << (logL1 + logL2 - 1);
+    prep_strain_kernel<<<(n_half + 255) / 256, 256, 0, st>>>(strain, dsT, logL1, logL2, scale);
     return cudaGetLastError();
 }
 

@@ -16,8 +16,9 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 inline int ilog2(int64_t x) { int l = 0; while ((int64_t(1) << l) < x) ++l; return l; }
 
 struct Layout {
-    size_t basisT, Y, Yavg, beta, bavg_hi, bavg_lo, c_hi, c_lo, cs, tw_L, tw_lo_main, tw_hi_main, tw_lo_avg,
-        tw_hi_avg, S_table, ds, dS, cand, counters, strain_stage, trig_stage, total;
+    size_t basisP, Y, beta, bavg_hi, bavg_lo, c_hi, c_lo, cs, tw1_a, tw1_b, twN, dsT, cand, counters, sched,
+        strain_stage, trig_stage, total;
+    size_t plane_bytes;
 };
 
 }  // namespace
@@ -29,8 +30,8 @@ struct rbmf_plan {
     int64_t M;          // N / w
     int j_low, n_half;
     int Tpad;
-    int logN1, logN2;   // main FFT: N = 2^logN1 * 2^logN2 (pass 1 length, pass 2 length)
-    int logM1, logM2;   // averaged FFT
+    int logN1, logN2;   // FFT: N = 2^logN1 * 2^logN2 (pass 1 length, pass 2 length)
+    int fft_grid;       // persistent CTAs of the fused FFT kernel
     int64_t max_cand, max_trig;
     int gemm_impl;
     int timing;
@@ -54,25 +55,23 @@ Layout make_layout(const rbmf_plan* p) {
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     const size_t k = (size_t)p->k, N = (size_t)p->N, M = (size_t)p->M;
-    L.basisT = take((size_t)p->n_half * k * 8);
-    L.Y = take(N * k * 8);
-    L.Yavg = take(p->w > 1 ? M * k * 8 : 0);
+    const size_t nkb = (k + 31) / 32;
+    L.plane_bytes = nkb * M * 64 * 2;
+    L.basisP = take((size_t)p->n_half * k * 8);
+    L.Y = take((size_t)kFftRing * N * kFftC * 8);
     L.beta = take(N * k * 8);
-    L.bavg_hi = take(M * 2 * k * 2);
-    L.bavg_lo = take(M * 2 * k * 2);
+    L.bavg_hi = take(L.plane_bytes);
+    L.bavg_lo = take(L.plane_bytes);
     L.c_hi = take((size_t)p->Tpad * 2 * 2 * k * 2);
     L.c_lo = take((size_t)p->Tpad * 2 * 2 * k * 2);
     L.cs = take((size_t)p->T * k * 8);
-    L.tw_L = take((size_t)kTwAllEntries * 8);
-    L.tw_lo_main = take(1024 * 8);
-    L.tw_hi_main = take((N / 1024 ? N / 1024 : 1) * 8);
-    L.tw_lo_avg = take(1024 * 8);
-    L.tw_hi_avg = take((M / 1024 ? M / 1024 : 1) * 8);
-    L.S_table = take((size_t)p->n_half * 8);
-    L.ds = take((size_t)p->n_half * 8);
-    L.dS = take((size_t)p->n_half * 8);
+    L.tw1_a = take(((size_t)1 << p->logN1) * 8);
+    L.tw1_b = take(((size_t)1 << p->logN2) * 8);
+    L.twN = take(N * 8);
+    L.dsT = take((size_t)p->n_half * 8);
     L.cand = take((size_t)p->max_cand * sizeof(rbmf_candidate));
-    L.counters = take(64);
+    L.counters = take(64 + (size_t)kSchedWords * 4);   // counters, then the FFT scheduler words: one memset
+    L.sched = L.counters + 64;
     L.strain_stage = take((size_t)(p->n_half + 1) * 8);
     L.trig_stage = take((size_t)p->max_trig * sizeof(rbmf_trigger));
     L.total = off;
@@ -81,9 +80,8 @@ Layout make_layout(const rbmf_plan* p) {
 
 void refresh(rbmf_plan* p) {
     p->M = p->N / p->w;
-    const int n = ilog2(p->N), m = ilog2(p->M);
+    const int n = ilog2(p->N);
     p->logN1 = (n + 1) / 2; p->logN2 = n / 2;
-    p->logM1 = (m + 1) / 2; p->logM2 = m / 2;
     p->Tpad = (p->T + kGemmTT - 1) / kGemmTT * kGemmTT;
     p->lay = make_layout(p);
 }
@@ -103,7 +101,8 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-rbmf_status make_map(rbmf_plan* plan, CUtensorMap* map, void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+rbmf_status encode_map(rbmf_plan* plan, CUtensorMap* map, void* base, int rank, const cuuint64_t* dims,
+                       const cuuint64_t* strides, const cuuint32_t* box) {
     static EncodeTiledFn fn = nullptr;
     if (!fn) {
         void* sym = nullptr;
@@ -113,15 +112,29 @@ rbmf_status make_map(rbmf_plan* plan, CUtensorMap* map, void* base, uint64_t row
         if (qres != cudaDriverEntryPointSuccess || !sym) { plan->last_cuda = -1; return RBMF_ERR_CUDA; }
         fn = (EncodeTiledFn)sym;
     }
-    const cuuint64_t dims[2] = {cols, rows};               // innermost first
-    const cuuint64_t strides[1] = {cols * 2};              // bytes, dims 1..rank-1
-    const cuuint32_t box[2] = {(cuuint32_t)kGemmBK, box_rows};
-    const cuuint32_t estr[2] = {1, 1};
-    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, dims, strides, box, estr,
+    const cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, base, dims, strides, box, estr,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { plan->last_cuda = (int)r; return RBMF_ERR_CUDA; }
     return RBMF_OK;
+}
+
+// Coefficient planes: rows x cols bf16, row-major; box = 64 columns x box_rows.
+rbmf_status make_map_rows(rbmf_plan* plan, CUtensorMap* map, void* base, uint64_t rows, uint64_t cols,
+                          uint32_t box_rows) {
+    const cuuint64_t dims[2] = {cols, rows};               // innermost first
+    const cuuint64_t strides[1] = {cols * 2};              // bytes, dims 1..rank-1
+    const cuuint32_t box[2] = {(cuuint32_t)kGemmBK, box_rows};
+    return encode_map(plan, map, base, 2, dims, strides, box);
+}
+
+// beta^avg planes: [kb][bin < M][64] bf16; box = one K block x 128 bins (16 KB contiguous).
+rbmf_status make_map_planes(rbmf_plan* plan, CUtensorMap* map, void* base, uint64_t M, uint64_t nkb) {
+    const cuuint64_t dims[3] = {(cuuint64_t)kGemmBK, M, nkb};
+    const cuuint64_t strides[2] = {(cuuint64_t)kGemmBK * 2, M * kGemmBK * 2};
+    const cuuint32_t box[3] = {(cuuint32_t)kGemmBK, (cuuint32_t)kGemmBM, 1};
+    return encode_map(plan, map, base, 3, dims, strides, box);
 }
 
 template <typename T> T* at(rbmf_plan* p, size_t off) { return reinterpret_cast<T*>(p->ws + off); }
@@ -157,7 +170,7 @@ rbmf_status rbmf_plan_set_window(rbmf_plan* plan, int32_t w) {
     if (!plan) return RBMF_ERR_ARG;
     if (plan->have_ws) return RBMF_ERR_STATE;
     if (w < 1 || w > 32 || (w & (w - 1)) != 0) return RBMF_ERR_ARG;
-    if (plan->N / w < 1024) return RBMF_ERR_ARG;
+    if (plan->N / w < kGemmBM) return RBMF_ERR_ARG;
     plan->w = w;
     refresh(plan);
     return RBMF_OK;
@@ -209,18 +222,28 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     plan->have_ws = true;
     plan->have_basis = plan->have_coeffs = plan->filtered = false;
     const Layout& L = plan->lay;
-    CK(launch_init_tables(at<float2>(plan, L.tw_L), at<float2>(plan, L.tw_lo_main), at<float2>(plan, L.tw_hi_main),
-                          at<float2>(plan, L.tw_lo_avg), at<float2>(plan, L.tw_hi_avg), at<float2>(plan, L.S_table),
-                          plan->N, plan->M, plan->w, plan->stream));
-    CK(cudaMemsetAsync(plan->ws + L.counters, 0, 64, plan->stream));
+    CK(launch_init_tables(at<float2>(plan, L.tw1_a), at<float2>(plan, L.tw1_b), at<float2>(plan, L.twN), plan->logN1,
+                          plan->logN2, plan->stream));
+    CK(cudaMemsetAsync(plan->ws + L.counters, 0, 64 + (size_t)kSchedWords * 4, plan->stream));
+    // columns of the last K block beyond k are never written by the FFT: they must be finite (they meet zeros)
+    CK(cudaMemsetAsync(plan->ws + L.bavg_hi, 0, L.plane_bytes, plan->stream));
+    CK(cudaMemsetAsync(plan->ws + L.bavg_lo, 0, L.plane_bytes, plan->stream));
     CK(gemm_tcgen05_configure());
-    // TMA descriptors: A = beta^avg planes (M rows x 2k), B = coefficient planes (2*Tpad rows x 2k)
+    {
+        int per_sm = 0;
+        size_t smem = 0;
+        CK(fft_fused_configure(plan->logN1, plan->logN2, &per_sm, &smem));
+        if (per_sm < 1) return RBMF_ERR_UNSUPPORTED;
+        plan->fft_grid = per_sm * plan->num_sms;
+    }
+    // TMA descriptors: A = beta^avg planes ([kb][M][64]), B = coefficient planes (2*Tpad rows x 2k)
     rbmf_status s;
     const uint64_t k2 = 2 * (uint64_t)plan->k;
-    if ((s = make_map(plan, &plan->tmA_hi, plan->ws + L.bavg_hi, (uint64_t)plan->M, k2, kGemmBM)) != RBMF_OK) return s;
-    if ((s = make_map(plan, &plan->tmA_lo, plan->ws + L.bavg_lo, (uint64_t)plan->M, k2, kGemmBM)) != RBMF_OK) return s;
-    if ((s = make_map(plan, &plan->tmB_hi, plan->ws + L.c_hi, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
-    if ((s = make_map(plan, &plan->tmB_lo, plan->ws + L.c_lo, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
+    const uint64_t nkb = (uint64_t)((plan->k + 31) / 32);
+    if ((s = make_map_planes(plan, &plan->tmA_hi, plan->ws + L.bavg_hi, (uint64_t)plan->M, nkb)) != RBMF_OK) return s;
+    if ((s = make_map_planes(plan, &plan->tmA_lo, plan->ws + L.bavg_lo, (uint64_t)plan->M, nkb)) != RBMF_OK) return s;
+    if ((s = make_map_rows(plan, &plan->tmB_hi, plan->ws + L.c_hi, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
+    if ((s = make_map_rows(plan, &plan->tmB_lo, plan->ws + L.c_lo, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
     plan->have_maps = true;
     if (!plan->have_events) {
         for (int i = 0; i < 5; ++i) CK(cudaEventCreate(&plan->ev[i]));
@@ -232,8 +255,8 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
 rbmf_status rbmf_set_basis(rbmf_plan* plan, const void* basis_dev) {
     if (!plan || !basis_dev) return RBMF_ERR_ARG;
     if (!plan->have_ws) return RBMF_ERR_STATE;
-    CK(launch_transpose_basis((const float2*)basis_dev, at<float2>(plan, plan->lay.basisT), plan->k, plan->N / 2 + 1,
-                              plan->j_low, plan->n_half, plan->stream));
+    CK(launch_layout_basis((const float2*)basis_dev, at<float2>(plan, plan->lay.basisP), plan->k, plan->N / 2 + 1,
+                           plan->j_low, plan->logN1, plan->logN2, plan->stream));
     plan->have_basis = true;
     return RBMF_OK;
 }
@@ -259,42 +282,20 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     unsigned long long* counters = at<unsigned long long>(plan, L.counters);
 
     if (tm) CK(cudaEventRecord(plan->ev[0], st));
-    CK(cudaMemsetAsync(counters, 0, 16, st));
-    CK(launch_prep_strain((const float2*)strain_dev, at<float2>(plan, L.S_table), at<float2>(plan, L.ds),
-                          at<float2>(plan, L.dS), plan->n_half, (float)sqrt(2.0 / (double)plan->N), st));
+    CK(cudaMemsetAsync(counters, 0, 64 + (size_t)kSchedWords * 4, st));   // counters + FFT scheduler words
+    CK(launch_prep_strain((const float2*)strain_dev, at<float2>(plan, L.dsT), plan->logN1, plan->logN2,
+                          (float)sqrt(2.0 / (double)plan->N), st));
 
-    // ---- kernel 1: a1-a3 -----------------------------------------------------------------------
+    // ---- kernel 1: a1-a3, one persistent launch ------------------------------------------------
     FftArgs a;
     memset(&a, 0, sizeof(a));
-    a.k = plan->k; a.j_low = plan->j_low; a.n_half = plan->n_half;
-    a.fold = 1; a.fold_stride = 0;
-    a.plane_hi = at<uint16_t>(plan, L.bavg_hi);
-    a.plane_lo = at<uint16_t>(plan, L.bavg_lo);
-    // main transform, pass 1: basis x strain -> Y
-    a.in = at<float2>(plan, L.basisT); a.strain = at<float2>(plan, L.ds); a.out = at<float2>(plan, L.Y);
-    a.tw_L = at<float2>(plan, L.tw_L) + tw_table_offset(plan->logN1);
-    a.tw_lo = at<float2>(plan, L.tw_lo_main); a.tw_hi = at<float2>(plan, L.tw_hi_main);
-    a.lines = 1 << plan->logN2;
-    CK(launch_fft_pass1(a, plan->logN1, false, st));
-    // main transform, pass 2: Y -> beta (and the operand planes when w = 1)
-    a.in = at<float2>(plan, L.Y); a.out = at<float2>(plan, L.beta);
-    a.tw_L = at<float2>(plan, L.tw_L) + tw_table_offset(plan->logN2);
-    a.lines = 1 << plan->logN1;
-    CK(launch_fft_pass2(a, plan->logN2, plan->w == 1 ? 2 : 0, st));
-    if (plan->w > 1) {
-        // averaged transform (Eq. 12): fold w/2 aliases -> Yavg -> beta^avg planes
-        a.in = at<float2>(plan, L.basisT); a.strain = at<float2>(plan, L.dS); a.out = at<float2>(plan, L.Yavg);
-        a.tw_L = at<float2>(plan, L.tw_L) + tw_table_offset(plan->logM1);
-        a.tw_lo = at<float2>(plan, L.tw_lo_avg); a.tw_hi = at<float2>(plan, L.tw_hi_avg);
-        a.lines = 1 << plan->logM2;
-        a.fold = plan->w / 2 > 1 ? plan->w / 2 : 1;
-        a.fold_stride = (int)plan->M;
-        CK(launch_fft_pass1(a, plan->logM1, true, st));
-        a.in = at<float2>(plan, L.Yavg); a.out = nullptr;
-        a.tw_L = at<float2>(plan, L.tw_L) + tw_table_offset(plan->logM2);
-        a.lines = 1 << plan->logM1;
-        CK(launch_fft_pass2(a, plan->logM2, 1, st));
-    }
+    a.basisP = at<float2>(plan, L.basisP); a.dsT = at<float2>(plan, L.dsT);
+    a.tw1_a = at<float2>(plan, L.tw1_a); a.tw1_b = at<float2>(plan, L.tw1_b); a.twN = at<float2>(plan, L.twN);
+    a.Y = at<float2>(plan, L.Y); a.beta = at<float2>(plan, L.beta);
+    a.plane_hi = at<uint16_t>(plan, L.bavg_hi); a.plane_lo = at<uint16_t>(plan, L.bavg_lo);
+    a.sched = at<unsigned>(plan, L.sched);
+    a.N = plan->N; a.M = (int)plan->M; a.nchunk = plan->k / kFftC; a.w = plan->w; a.inv_w = 1.0f / (float)plan->w;
+    CK(launch_fft_fused(a, plan->logN1, plan->logN2, plan->fft_grid, st));
     if (tm) CK(cudaEventRecord(plan->ev[1], st));
 
     // ---- kernel 2: a4-a5 -----------------------------------------------------------------------
@@ -322,7 +323,7 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     s2.cand = g.cand; s2.cs = at<float2>(plan, L.cs); s2.beta = at<float2>(plan, L.beta);
     s2.out = out_dev; s2.counters = counters;
     s2.cand_cap = (unsigned long long)plan->max_cand; s2.trig_cap = (unsigned long long)plan->max_trig;
-    s2.thr2_sq = thr_stage2 * thr_stage2; s2.k = plan->k; s2.w = plan->w;
+    s2.thr2_sq = thr_stage2 * thr_stage2; s2.k = plan->k; s2.w = plan->w; s2.N = plan->N;
     CK(launch_stage2(s2, plan->num_sms, st));
     CK(cudaMemcpyAsync(n_out_dev, counters + 1, 8, cudaMemcpyDeviceToDevice, st));
     if (tm) CK(cudaEventRecord(plan->ev[3], st));
@@ -390,8 +391,8 @@ rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_p
     const Layout& L = plan->lay;
     switch (which) {
         case 0: *dev_ptr = plan->ws + L.beta; *bytes = (size_t)plan->N * plan->k * 8; break;
-        case 1: *dev_ptr = plan->ws + L.bavg_hi; *bytes = (size_t)plan->M * 2 * plan->k * 2; break;
-        case 2: *dev_ptr = plan->ws + L.bavg_lo; *bytes = (size_t)plan->M * 2 * plan->k * 2; break;
+        case 1: *dev_ptr = plan->ws + L.bavg_hi; *bytes = L.plane_bytes; break;
+        case 2: *dev_ptr = plan->ws + L.bavg_lo; *bytes = L.plane_bytes; break;
         default: return RBMF_ERR_ARG;
     }
     return RBMF_OK;
@@ -416,8 +417,8 @@ rbmf_status rbmf_get_stage_ms(rbmf_plan* plan, float ms[4]) {
 
 rbmf_status rbmf_launches_per_filter(const rbmf_plan* plan, int32_t* n) {
     if (!plan || !n) return RBMF_ERR_ARG;
-    // prep_strain + FFT pass 1 + pass 2 (+ fold pass 1 + planes pass 2 when w > 1) + GEMM + stage 2
-    *n = 1 + 2 + (plan->w > 1 ? 2 : 0) + 1 + 1;
+    // prep_strain + fused FFT + GEMM + stage 2
+    *n = 4;
     return RBMF_OK;
 }
 

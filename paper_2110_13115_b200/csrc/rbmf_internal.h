@@ -9,27 +9,44 @@
 
 namespace rbmf {
 
-constexpr int kFftKC = 8;          // basis columns per FFT CTA (64-byte row segments)
+constexpr int kFftC = 4;           // basis columns per FFT chunk (32-byte row segments)
+constexpr int kFftThreads = 256;   // threads per FFT CTA
+constexpr int kFftRing = 3;        // chunk slots of the L2-resident intermediate Y
+constexpr int kMaxChunks = 256;    // k <= 1024
 constexpr int kGemmBM = 128;       // time bins per GEMM tile (UMMA M)
 constexpr int kGemmTT = 128;       // templates per GEMM tile (UMMA N = 2*kGemmTT: re | im rows)
-constexpr int kGemmBK = 64;        // bf16 elements per K block (= one 128-byte swizzle row)
+constexpr int kGemmBK = 64;        // bf16 elements per K block (= one 128-byte swizzle row = 32 basis columns)
 
-// Device views handed to the FFT kernels.
+// Per-length configuration of the in-CTA transform: L = R0 * R1, two Stockham stages.
+// A thread owns one column and R0 elements; W = L / R0 = R1 threads cooperate on one column of one line.
+__host__ __device__ constexpr int fft_r0(int logL) { return logL >= 9 ? 32 : (logL >= 7 ? 16 : 8); }
+__host__ __device__ constexpr int fft_r1(int logL) { return (1 << logL) / fft_r0(logL); }
+// lines (independent transforms) a 256-thread CTA works on in lockstep
+__host__ __device__ constexpr int fft_sub(int logL) { return kFftThreads / (fft_r1(logL) * kFftC); }
+// inner row group of the Y layout: Y[slot][n1 / g][j2][n1 % g][C]
+__host__ __device__ constexpr int fft_group(int logL2) { return fft_sub(logL2) < 8 ? fft_sub(logL2) : 8; }
+
+// Scheduler words (uint32) in the workspace: [0] ticket, [16 + c] pass-1 tiles done of chunk c,
+// [16 + kMaxChunks + c] pass-2 items done of chunk c.
+constexpr int kSchedWords = 16 + 2 * kMaxChunks;
+
+// Device views handed to the fused FFT kernel.
 struct FftArgs {
-    const float2* in;        // pass 1: basisT (rows j < N/2, k columns); pass 2: Y
-    const float2* strain;    // pass 1: scaled strain ds[j] (main) or dS[j] = ds[j] S(j) (fold)
-    float2* out;             // pass 1: Y; pass 2: beta (may be null)
-    uint16_t* plane_hi;      // pass 2 plane modes: (rows) x 2k bf16
+    const float2* basisP;    // [chunk][j2 < L2][j1 < L1/2][C]: conj NOT applied, zero outside the band
+    const float2* dsT;       // [j2 < L2][j1 < L1/2]: s * d[j1 L2 + j2]
+    const float2* tw1_a;     // pass 1 stage-1 twiddles  [q < R1][b < R0] = e^{2 pi i q b / L1}
+    const float2* tw1_b;     // pass 2 stage-1 twiddles, same for L2
+    const float2* twN;       // inter-pass twiddles [j2 < L2][n1 < L1] = e^{2 pi i j2 n1 / N}
+    float2* Y;               // ring of kFftRing chunk slots, N * C entries each
+    float2* beta;            // [chunk][n < N][C]
+    uint16_t* plane_hi;      // [kb = col / 32][bin < M][64]: bf16 (re, im) of column col % 32
     uint16_t* plane_lo;
-    const float2* tw_L;      // e^{2 pi i m / L}, m < L (table of this pass's length)
-    const float2* tw_lo;     // e^{2 pi i m / Ntot}, m < 1024
-    const float2* tw_hi;     // e^{2 pi i 1024 m / Ntot}, m < max(1, Ntot/1024)
-    int k;                   // columns
-    int lines;               // O = Ntot / L: number of independent lines (grid.x)
-    int j_low;               // first in-band bin
-    int n_half;              // N/2 (first out-of-band bin)
-    int fold;                // pass 1 fold mode: number of aliases to sum = max(1, w/2); else 1
-    int fold_stride;         // M = N/w (bins between aliases)
+    unsigned* sched;         // kSchedWords
+    long long N;
+    int M;                   // N / w
+    int nchunk;              // k / C
+    int w;
+    float inv_w;
 };
 
 struct GemmArgs {
@@ -48,37 +65,33 @@ struct GemmArgs {
 struct Stage2Args {
     const rbmf_candidate* cand;
     const float2* cs;         // T x k: conj(c_tk) / sigma_t
-    const float2* beta;       // N x k
+    const float2* beta;       // [chunk][n][C]
     rbmf_trigger* out;
     unsigned long long* counters;
     unsigned long long cand_cap;
     unsigned long long trig_cap;
+    long long N;
     float thr2_sq;
     int k;
     int w;
 };
 
 // ---- launchers (each returns the cudaError_t of the launch) -------------------------------------
-cudaError_t launch_init_tables(float2* tw_L_all, float2* tw_lo_main, float2* tw_hi_main, float2* tw_lo_avg,
-                               float2* tw_hi_avg, float2* S_table, int64_t N, int64_t M, int w, cudaStream_t st);
-cudaError_t launch_transpose_basis(const float2* basis, float2* basisT, int k, int64_t bins, int j_low,
-                                   int n_half, cudaStream_t st);
+cudaError_t launch_init_tables(float2* tw1_a, float2* tw1_b, float2* twN, int logL1, int logL2, cudaStream_t st);
+cudaError_t launch_layout_basis(const float2* basis, float2* basisP, int k, int64_t bins, int j_low, int logL1,
+                                int logL2, cudaStream_t st);
 cudaError_t launch_prep_coeffs(const float2* coeffs, const float* sigma, float2* cs, uint16_t* c_hi,
                                uint16_t* c_lo, int T, int Tpad, int k, cudaStream_t st);
-cudaError_t launch_prep_strain(const float2* strain, const float2* S_table, float2* ds, float2* dS,
-                               int n_half, float scale, cudaStream_t st);
-cudaError_t launch_fft_pass1(const FftArgs& a, int logL, bool fold, cudaStream_t st);
-// mode: 0 = write beta, 1 = write planes, 2 = both
-cudaError_t launch_fft_pass2(const FftArgs& a, int logL, int mode, cudaStream_t st);
+cudaError_t launch_prep_strain(const float2* strain, float2* dsT, int logL1, int logL2, float scale,
+                               cudaStream_t st);
+// Fused FFT (a1-a3): configure once per (logL1, logL2) -> CTAs per SM; then launch.
+cudaError_t fft_fused_configure(int logL1, int logL2, int* ctas_per_sm, size_t* smem_bytes);
+cudaError_t launch_fft_fused(const FftArgs& a, int logL1, int logL2, int grid, cudaStream_t st);
 cudaError_t launch_gemm_simt(const uint16_t* a_hi, const uint16_t* a_lo, const uint16_t* c_hi,
                              const uint16_t* c_lo, const GemmArgs& g, cudaStream_t st);
 cudaError_t launch_gemm_tcgen05(const CUtensorMap& tmA_hi, const CUtensorMap& tmA_lo, const CUtensorMap& tmB_hi,
                                 const CUtensorMap& tmB_lo, const GemmArgs& g, int num_sms, cudaStream_t st);
 cudaError_t gemm_tcgen05_configure();   // sets the dynamic shared memory attribute once
 cudaError_t launch_stage2(const Stage2Args& a, int num_sms, cudaStream_t st);
-
-// Offset (in float2 entries) of the length-2^logL twiddle table inside tw_L_all; tables for logL = 5..10.
-__host__ __device__ inline int tw_table_offset(int logL) { return (1 << logL) - 32; }
-constexpr int kTwAllEntries = 2048 - 32;
 
 }  // namespace rbmf

@@ -7,7 +7,9 @@
 namespace rbmf {
 
 // One warp per candidate (t, i): rho_t[i w + r] = sum_c cs[t][c] * beta[i w + r][c], r < w  (cs = conj(c)/sigma).
-// Reads one contiguous block of w*k complex64 of beta and the k coefficients of template t.
+// beta is chunk-blocked, [chunk][n][C = 4]: per chunk the candidate's w rows are one contiguous block of w * 32
+// bytes.  The warp walks float4 items e = (chunk, r, half) in this order, e = lane, lane + 32, ...: with 2w <= 32 a
+// lane always sees the same (r, half), so it accumulates one row's partial sum; w = 32 alternates between two rows.
 __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
     const int lane = threadIdx.x & 31;
     const unsigned long long warp0 = (unsigned long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -15,41 +17,54 @@ __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
     unsigned long long n_cand = a.counters[0];
     if (n_cand > a.cand_cap) n_cand = a.cand_cap;
     const int k = a.k, w = a.w;
+    const int per_chunk = 2 * w;                       // float4 items per chunk
+    const int total = (k / kFftC) * per_chunk;
+    const size_t chunk_stride = (size_t)a.N * kFftC;    // float2 entries
     for (unsigned long long ci = warp0; ci < n_cand; ci += nwarps) {
         const rbmf_candidate cd = a.cand[ci];
         const float2* __restrict__ crow = a.cs + (size_t)cd.template_id * k;
-        const float2* __restrict__ brow = a.beta + (size_t)cd.bin_index * w * k;
-        float my_re = 0.f, my_im = 0.f;   // lane r keeps rho of sample r (w <= 32)
-        for (int r = 0; r < w; ++r) {
-            float re = 0.f, im = 0.f;
-            for (int c = lane; c < k; c += 32) {
-                const float2 p = __ldg(crow + c);
-                const float2 x = __ldg(brow + (size_t)r * k + c);
-                re = fmaf(p.x, x.x, re); re = fmaf(-p.y, x.y, re);
-                im = fmaf(p.x, x.y, im); im = fmaf(p.y, x.x, im);
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                re += __shfl_xor_sync(0xffffffffu, re, o);
-                im += __shfl_xor_sync(0xffffffffu, im, o);
-            }
-            if (lane == r) { my_re = re; my_im = im; }
+        const float2* __restrict__ brow = a.beta + (size_t)cd.bin_index * w * kFftC;
+        float re0 = 0.f, im0 = 0.f, re1 = 0.f, im1 = 0.f;
+        int par = 0;
+        for (int e = lane; e < total; e += 32, par ^= 1) {
+            const int ch = e / per_chunk, rem = e % per_chunk;
+            const int r = rem >> 1, h = rem & 1;
+            const float4 p = __ldg(reinterpret_cast<const float4*>(crow + ch * kFftC + 2 * h));
+            const float4 x = __ldg(reinterpret_cast<const float4*>(brow + ch * chunk_stride + r * kFftC + 2 * h));
+            float vr = p.x * x.x, vi = p.x * x.y;
+            vr = fmaf(-p.y, x.y, vr); vr = fmaf(p.z, x.z, vr); vr = fmaf(-p.w, x.w, vr);
+            vi = fmaf(p.y, x.x, vi); vi = fmaf(p.z, x.w, vi); vi = fmaf(p.w, x.z, vi);
+            if (per_chunk > 32 && par) { re1 += vr; im1 += vi; } else { re0 += vr; im0 += vi; }
         }
-        const bool hit = lane < w && (my_re * my_re + my_im * my_im >= a.thr2_sq);
-        const unsigned ballot = __ballot_sync(0xffffffffu, hit);
-        if (ballot) {
-            unsigned long long base = 0;
-            if (lane == 0) base = atomicAdd(a.counters + 1, (unsigned long long)__popc(ballot));
-            base = __shfl_sync(0xffffffffu, base, 0);
-            if (hit) {
-                const unsigned long long idx = base + __popc(ballot & ((1u << lane) - 1u));
-                if (idx < a.trig_cap) {
-                    rbmf_trigger t;
-                    t.template_id = cd.template_id;
-                    t.time_index = cd.bin_index * w + lane;
-                    t.snr_re = my_re;
-                    t.snr_im = my_im;
-                    a.out[idx] = t;
+        // lanes that share a row differ in bit 0 (half) and in the bits >= log2(2w)
+        for (int o = 1; o < 32; o <<= 1) {
+            if (o == 1 || o >= per_chunk) {
+                re0 += __shfl_xor_sync(0xffffffffu, re0, o); im0 += __shfl_xor_sync(0xffffffffu, im0, o);
+                re1 += __shfl_xor_sync(0xffffffffu, re1, o); im1 += __shfl_xor_sync(0xffffffffu, im1, o);
+            }
+        }
+        // even lane 2r < 2w holds row r (and row 16 + r in slot 1 when w = 32)
+        const int nslot = per_chunk > 32 ? 2 : 1;
+        for (int s = 0; s < nslot; ++s) {
+            const int r = (lane >> 1) + 16 * s;
+            const float vr = s ? re1 : re0, vi = s ? im1 : im0;
+            const bool owner = (lane & 1) == 0 && lane < per_chunk;
+            const bool hit = owner && (vr * vr + vi * vi >= a.thr2_sq);
+            const unsigned ballot = __ballot_sync(0xffffffffu, hit);
+            if (ballot) {
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(a.counters + 1, (unsigned long long)__popc(ballot));
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (hit) {
+                    const unsigned long long idx = base + __popc(ballot & ((1u << lane) - 1u));
+                    if (idx < a.trig_cap) {
+                        rbmf_trigger t;
+                        t.template_id = cd.template_id;
+                        t.time_index = cd.bin_index * w + r;
+                        t.snr_re = vr;
+                        t.snr_im = vi;
+                        a.out[idx] = t;
+                    }
                 }
             }
         }
@@ -83,7 +98,7 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(const uint16_t* __restri
         for (int e = threadIdx.x; e < TI * KB; e += 256) {
             const int r = e / KB, kk = e % KB;
             const int i = i0 + r;
-            sA[r][kk] = i < g.M ? plane_val(a_hi, a_lo, (size_t)i * g.k2 + k0 + kk) : 0.f;
+            sA[r][kk] = i < g.M ? plane_val(a_hi, a_lo, ((size_t)((k0 + kk) / 64) * g.M + i) * 64 + (k0 + kk) % 64) : 0.f;
             const int t = t0 + r;   // t < Tpad always (grid covers padded templates)
             const size_t row_re = (size_t)(t / kGemmTT) * 2 * kGemmTT + (t % kGemmTT);
             sRe[r][kk] = plane_val(c_hi, c_lo, row_re * g.k2 + k0 + kk);

@@ -213,12 +213,15 @@ class Plan:
             off = p.value - self._ws.data_ptr()
             return self._ws[off: off + nb.value]
 
+        C = 4   # columns per chunk of the library's chunk-blocked layouts (include/rbmf.h, rbmf_get_internal)
         if which == "beta":
-            return torch.view_as_complex(view(0).view(torch.float32).view(self.N, self.k, 2)).cpu().numpy()
+            v = view(0).view(torch.float32).view(self.k // C, self.N, C, 2)          # [chunk][n][C]
+            return torch.view_as_complex(v.permute(1, 0, 2, 3).reshape(self.N, self.k, 2).contiguous()).cpu().numpy()
         if which == "beta_avg":
+            M, nkb = self.N // self.w, (self.k + 31) // 32
             hi = view(1).view(torch.bfloat16).to(torch.float32)
             lo = view(2).view(torch.bfloat16).to(torch.float32)
-            v = (hi + lo).view(self.N // self.w, self.k, 2)
+            v = (hi + lo).view(nkb, M, 32, 2).permute(1, 0, 2, 3).reshape(M, nkb * 32, 2)[:, : self.k]   # [kb][bin][32]
             return torch.view_as_complex(v.contiguous()).cpu().numpy()
         raise KeyError(which)
 

@@ -66,19 +66,23 @@ def test_window_capacity_and_workspace_size(binding):
     nbytes = ctypes.c_size_t()
     assert b.rbmf_workspace_bytes(h, ctypes.byref(nbytes)) == b.RBMF_OK
     default_bytes = nbytes.value
-    # beta (N k 8) + Y + basis^T alone are 2.5 N k 8 bytes
-    assert default_bytes > 2.5 * 4096 * 16 * 8
-    for w in (0, 3, 64, 8):          # 8: N/w = 512 < 1024
+    # beta (N k 8) + the re-laid-out basis (N/2 k 8) alone are 1.5 N k 8 bytes
+    assert default_bytes > 1.5 * 4096 * 16 * 8
+    for w in (0, 3, 64):             # not a power of two in [1, 32]
         assert b.rbmf_plan_set_window(h, w) == b.RBMF_ERR_ARG
+    st2, h2 = _create(b, N=1024)
+    assert b.rbmf_plan_set_window(h2, 16) == b.RBMF_ERR_ARG      # N/w = 64 < 128 bins (one GEMM tile)
+    assert b.rbmf_plan_set_window(h2, 8) == b.RBMF_OK
+    b.rbmf_plan_destroy(h2)
     assert b.rbmf_plan_set_window(h, 4) == b.RBMF_OK
     assert b.rbmf_plan_set_capacity(h, 0, 10) == b.RBMF_ERR_ARG
     assert b.rbmf_plan_set_capacity(h, 1000, 1000) == b.RBMF_OK
     assert b.rbmf_workspace_bytes(h, ctypes.byref(nbytes)) == b.RBMF_OK
     assert nbytes.value < default_bytes          # smaller lists
     n = ctypes.c_int32()
-    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 7
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 4
     assert b.rbmf_plan_set_window(h, 1) == b.RBMF_OK
-    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 5
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 4
     assert b.rbmf_plan_set_gemm_impl(h, 7) == b.RBMF_ERR_ARG
     assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_SIMT) == b.RBMF_OK
     b.rbmf_plan_destroy(h)
