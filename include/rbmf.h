@@ -65,8 +65,14 @@ typedef enum {
 
 /* Stage-1 reconstruction kernels (rbmf_plan_set_gemm_impl). */
 typedef enum {
-    RBMF_GEMM_TCGEN05 = 0, /* default: TMA + tcgen05.mma (bf16x3 split precision) + TMEM epilogue     */
-    RBMF_GEMM_SIMT = 1     /* plain fp32 CUDA-core kernel on the same operands; verification only      */
+    RBMF_GEMM_TCGEN05 = 0, /* TMA + tcgen05.mma, bf16x3 split precision (fp32-equivalent) + TMEM epilogue          */
+    RBMF_GEMM_SIMT = 1,    /* plain fp32 CUDA-core kernel on the same operands; verification only                  */
+    RBMF_GEMM_SCREEN = 2   /* default: the same tensor-core kernel with ONE fp16 product per term and thr_stage1
+                              lowered, per (bin, template block), by a rigorous bound of the fp16 error, so its
+                              output is a superset of the true candidates; kernel 3 then repeats the stage-1 test at
+                              fp32 accuracy (the mean of the w fp32 samples it computes anyway is the averaged SNR of
+                              Eq. 9) before scoring.  Same candidate and trigger sets as RBMF_GEMM_TCGEN05 up to
+                              fp32 rounding at the threshold, one third of the tensor-core work.               */
 } rbmf_gemm_impl;
 
 /* Create a plan for segments of N samples (power of two, 2^10 <= N <= 2^20) at sampling rate fs [Hz],
@@ -83,7 +89,7 @@ rbmf_status rbmf_plan_set_window(rbmf_plan* plan, int32_t w);
  * before rbmf_workspace_bytes / rbmf_plan_set_workspace. */
 rbmf_status rbmf_plan_set_capacity(rbmf_plan* plan, int64_t max_candidates, int64_t max_triggers);
 
-/* Select the stage-1 kernel (default RBMF_GEMM_TCGEN05).  May be called at any time. */
+/* Select the stage-1 kernel (default RBMF_GEMM_SCREEN).  May be called at any time. */
 rbmf_status rbmf_plan_set_gemm_impl(rbmf_plan* plan, int32_t impl);
 
 /* Bytes of device workspace the plan needs (depends on N, k, T, w, capacities). */
@@ -120,7 +126,9 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
 rbmf_status rbmf_filter_host(rbmf_plan* plan, const void* strain_host, float thr_stage1, float thr_stage2,
                              rbmf_trigger* out_host, int64_t capacity_out, int64_t* n_out_host);
 
-/* Counts of the last rbmf_filter (synchronises the stream).  RBMF_ERR_OVERFLOW if a capacity was exceeded. */
+/* Counts of the last rbmf_filter (synchronises the stream).  RBMF_ERR_OVERFLOW if a capacity was exceeded
+ * (in RBMF_GEMM_SCREEN mode the capacity max_candidates applies to the screened superset, while *n_candidates
+ * reports the candidates confirmed at fp32 accuracy). */
 rbmf_status rbmf_get_counts(rbmf_plan* plan, int64_t* n_candidates, int64_t* n_triggers);
 
 /* Copy up to `capacity` first-stage candidates of the last rbmf_filter to out_host (synchronises).
@@ -131,7 +139,8 @@ rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64
  * plan's stream, until the next call), in the library's blocked layouts:
  *   which = 0: beta, complex64, [k/4 chunks][N samples][4 columns]: beta_c[n] at ((c/4) N + n) 4 + c%4;
  *   which = 1 / 2: beta^avg hi / lo plane, bfloat16, [ceil(k/32) K blocks][N/w bins][32 columns][re, im]
- *                  (value = hi + lo; columns >= k of the last block are zero).
+ *                  (value = hi + lo; columns >= k of the last block are zero).  In RBMF_GEMM_SCREEN mode plane 1
+ *                  holds ONE float16 rounding of beta^avg in the same layout and plane 2 is stale.
  * *dev_ptr receives the address, *bytes the size. */
 rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_ptr, size_t* bytes);
 

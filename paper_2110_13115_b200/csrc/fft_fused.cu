@@ -22,6 +22,7 @@
 // butterflies of radix R1.  SUB = 256 / (R1 * C) lines are processed in lockstep.  All layouts (basis, Y, beta,
 // planes) are chosen so that the 32 lanes of a warp always touch 128..256 contiguous bytes.
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 
 #include "rbmf_internal.h"
 
@@ -202,6 +203,12 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int chunk, int tile, f
 
 // ------------------------------------------------------------------------------------------- pass 2
 __device__ __forceinline__ void store_planes(const FftArgs& a, int bin, int gcol, float2 v) {
+    if (a.plane_fp16) {
+        // screen mode: one fp16 plane (round to nearest; |v| > 65504 becomes inf, which the screen lets through)
+        const size_t e = ((size_t)(gcol / 32) * a.M + bin) * 64 + (gcol % 32) * 2;
+        *reinterpret_cast<__half2*>(a.plane_hi + e) = __floats2half2_rn(v.x, v.y);
+        return;
+    }
     const __nv_bfloat16 hx = __float2bfloat16_rn(v.x), hy = __float2bfloat16_rn(v.y);
     const __nv_bfloat16 lx = __float2bfloat16_rn(v.x - __bfloat162float(hx));
     const __nv_bfloat16 ly = __float2bfloat16_rn(v.y - __bfloat162float(hy));

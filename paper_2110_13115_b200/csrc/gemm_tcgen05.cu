@@ -32,11 +32,16 @@ constexpr int BM = kGemmBM;            // 128 time bins
 constexpr int BN = 2 * kGemmTT;        // 256 = 128 templates x {re, im}
 constexpr int BK = kGemmBK;            // 64 bf16 = 128 B
 constexpr int UMMA_K = 16;
-constexpr int STAGES = 2;
 constexpr uint32_t A_BYTES = BM * BK * 2;                     // 16 KB per plane
 constexpr uint32_t B_BYTES = BN * BK * 2;                     // 32 KB per plane
-constexpr uint32_t STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;   // A_hi, A_lo, B_hi, B_lo = 96 KB
-constexpr uint32_t SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+// MODE 0 (bf16x3): planes A_hi, A_lo, B_hi, B_lo = 96 KB per stage, 2 stages.
+// MODE 1 (fp16 screen): one A and one B plane = 48 KB per stage, 4 stages.
+template <int MODE> struct ModeCfg {
+    static constexpr int PLANES = MODE == 0 ? 2 : 1;
+    static constexpr int STAGES = MODE == 0 ? 2 : 4;
+    static constexpr uint32_t STAGE_BYTES = PLANES * (A_BYTES + B_BYTES);
+    static constexpr uint32_t SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+};
 constexpr uint32_t TMEM_COLS = 512;
 constexpr int NUM_THREADS = 192;
 
@@ -91,16 +96,18 @@ __device__ __forceinline__ uint64_t make_smem_desc(uint32_t addr) {
     return d;
 }
 
-// kind::f16 instruction descriptor: D = F32, A = B = BF16, both K-major, N = 256, M = 128.
-constexpr uint32_t kInstrDesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) |
-                                ((uint32_t)(BM >> 4) << 24);
+// kind::f16 instruction descriptors: D = F32, both operands K-major, N = 256, M = 128; A = B = BF16 (format 1) for
+// the bf16x3 products, A = B = F16 (format 0) for the screen.
+constexpr uint32_t kInstrDescF16 = (1u << 4) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+constexpr uint32_t kInstrDescBF16 = kInstrDescF16 | (1u << 7) | (1u << 10);
 
-__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+template <uint32_t IDESC>
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
-        "l"(adesc), "l"(bdesc), "r"(kInstrDesc), "r"(accumulate)
+        "l"(adesc), "l"(bdesc), "n"(IDESC), "r"(accumulate)
         : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
@@ -137,10 +144,13 @@ __device__ __forceinline__ int num_tiles(const GemmArgs& g) { return g.num_tb * 
 
 }  // namespace
 
+template <int MODE>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
                     const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
                     const GemmArgs g) {
+    constexpr int STAGES = ModeCfg<MODE>::STAGES;
+    constexpr uint32_t STAGE_BYTES = ModeCfg<MODE>::STAGE_BYTES;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
@@ -191,10 +201,15 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
                     const uint32_t sbase = smem_base + stage * STAGE_BYTES;
                     mbar_expect_tx(full_bar(stage), STAGE_BYTES);
                     // beta^avg planes are K-block major, [kb][bin][64]: one box = 16 KB contiguous
-                    tma_load_3d(sbase, &tmA_hi, full_bar(stage), 0, ib * BM, kb);
-                    tma_load_3d(sbase + A_BYTES, &tmA_lo, full_bar(stage), 0, ib * BM, kb);
-                    tma_load_2d(sbase + 2 * A_BYTES, &tmB_hi, full_bar(stage), kb * BK, tb * BN);
-                    tma_load_2d(sbase + 2 * A_BYTES + B_BYTES, &tmB_lo, full_bar(stage), kb * BK, tb * BN);
+                    if (MODE == 0) {
+                        tma_load_3d(sbase, &tmA_hi, full_bar(stage), 0, ib * BM, kb);
+                        tma_load_3d(sbase + A_BYTES, &tmA_lo, full_bar(stage), 0, ib * BM, kb);
+                        tma_load_2d(sbase + 2 * A_BYTES, &tmB_hi, full_bar(stage), kb * BK, tb * BN);
+                        tma_load_2d(sbase + 2 * A_BYTES + B_BYTES, &tmB_lo, full_bar(stage), kb * BK, tb * BN);
+                    } else {
+                        tma_load_3d(sbase, &tmA_hi, full_bar(stage), 0, ib * BM, kb);
+                        tma_load_2d(sbase + A_BYTES, &tmB_hi, full_bar(stage), kb * BK, tb * BN);
+                    }
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
             }
@@ -217,13 +232,19 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
 #pragma unroll
                     for (int k4 = 0; k4 < BK / UMMA_K; ++k4) {
                         const uint32_t koff = k4 * UMMA_K * 2;   // bytes
-                        const uint64_t a_hi = make_smem_desc(sbase + koff);
-                        const uint64_t a_lo = make_smem_desc(sbase + A_BYTES + koff);
-                        const uint64_t b_hi = make_smem_desc(sbase + 2 * A_BYTES + koff);
-                        const uint64_t b_lo = make_smem_desc(sbase + 2 * A_BYTES + B_BYTES + koff);
-                        umma_bf16(tmem_d, a_lo, b_hi, (kb | k4) != 0 ? 1u : 0u);   // small terms first
-                        umma_bf16(tmem_d, a_hi, b_lo, 1u);
-                        umma_bf16(tmem_d, a_hi, b_hi, 1u);
+                        if (MODE == 0) {
+                            const uint64_t a_hi = make_smem_desc(sbase + koff);
+                            const uint64_t a_lo = make_smem_desc(sbase + A_BYTES + koff);
+                            const uint64_t b_hi = make_smem_desc(sbase + 2 * A_BYTES + koff);
+                            const uint64_t b_lo = make_smem_desc(sbase + 2 * A_BYTES + B_BYTES + koff);
+                            umma_f16<kInstrDescBF16>(tmem_d, a_lo, b_hi, (kb | k4) != 0 ? 1u : 0u);   // small terms first
+                            umma_f16<kInstrDescBF16>(tmem_d, a_hi, b_lo, 1u);
+                            umma_f16<kInstrDescBF16>(tmem_d, a_hi, b_hi, 1u);
+                        } else {
+                            const uint64_t a_h = make_smem_desc(sbase + koff);
+                            const uint64_t b_h = make_smem_desc(sbase + A_BYTES + koff);
+                            umma_f16<kInstrDescF16>(tmem_d, a_h, b_h, (kb | k4) != 0 ? 1u : 0u);
+                        }
                     }
                     umma_commit(empty_bar(stage));                       // frees the smem slot when the MMAs retire
                     if (kb == num_kb - 1) umma_commit(tfull_bar(buf));   // accumulator complete
@@ -244,6 +265,15 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(buf * BN);
             const int bin = ib * BM + row;
+            // MODE 0: the stage-1 threshold itself.  MODE 1: thr1 lowered by a rigorous bound of the fp16 screen's
+            // error for this (bin, template block), so that no true candidate can be missed (see file header).
+            float thr_sq = g.thr1_sq;
+            if (MODE == 1) {
+                const float Bn = bin < g.M ? __ldg(g.bin_norm + bin) : 0.f;
+                const float nmax = __ldg(g.tnorm_blk + tb);
+                const float te = g.thr1 - (g.kappa1 * nmax * Bn + g.kappa2 * (Bn + nmax) + g.slack);
+                thr_sq = te > 0.f ? te * te : 0.f;
+            }
 #pragma unroll 1
             for (int ch = 0; ch < kGemmTT / 32; ++ch) {
                 uint32_t re[32], im[32];
@@ -254,7 +284,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
 #pragma unroll
                 for (int j = 0; j < 32; ++j) {
                     const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
-                    mask |= (fmaf(x, x, y * y) >= g.thr1_sq ? 1u : 0u) << j;
+                    mask |= (!(fmaf(x, x, y * y) < thr_sq) ? 1u : 0u) << j;   // NaN (fp16 overflow) passes
                 }
                 if (bin >= g.M) mask = 0;
                 if (__any_sync(0xffffffffu, mask != 0)) {
@@ -302,14 +332,26 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
 }
 
 cudaError_t gemm_tcgen05_configure() {
-    return cudaFuncSetAttribute(gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(gemm_tcgen05_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)ModeCfg<0>::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(gemm_tcgen05_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)ModeCfg<1>::SMEM_BYTES);
 }
 
 cudaError_t launch_gemm_tcgen05(const CUtensorMap& tmA_hi, const CUtensorMap& tmA_lo, const CUtensorMap& tmB_hi,
                                 const CUtensorMap& tmB_lo, const GemmArgs& g, int num_sms, cudaStream_t st) {
     const int ntiles = g.num_tb * g.num_ib;
     const int grid = ntiles < num_sms ? ntiles : num_sms;
-    gemm_tcgen05_kernel<<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmA_hi, tmA_lo, tmB_hi, tmB_lo, g);
+    gemm_tcgen05_kernel<0><<<grid, NUM_THREADS, ModeCfg<0>::SMEM_BYTES, st>>>(tmA_hi, tmA_lo, tmB_hi, tmB_lo, g);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gemm_screen(const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmArgs& g, int num_sms,
+                               cudaStream_t st) {
+    const int ntiles = g.num_tb * g.num_ib;
+    const int grid = ntiles < num_sms ? ntiles : num_sms;
+    gemm_tcgen05_kernel<1><<<grid, NUM_THREADS, ModeCfg<1>::SMEM_BYTES, st>>>(tmA, tmA, tmB, tmB, g);
     return cudaGetLastError();
 }
 

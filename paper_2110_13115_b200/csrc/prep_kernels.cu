@@ -1,6 +1,7 @@
 // Set-up kernels: constant tables, basis re-layout, coefficient planes, per-call strain scaling.
 // None of them is on the per-segment critical path except prep_strain (N/2 elements).
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 
 #include "rbmf_internal.h"
 
@@ -87,21 +88,26 @@ __device__ __forceinline__ void split_bf16(float v, uint16_t& hi, uint16_t& lo) 
     lo = __bfloat16_as_ushort(l);
 }
 
+// Screen mode (RBMF_GEMM_SCREEN) additionally needs the same two rows rounded ONCE to fp16 (c_h16) and, per block of
+// 128 templates, tnorm_blk[tb] = max_t ||c_t||_2 / sigma_t (fp32 values as stored in cs; zero-initialised by the
+// launcher, positive floats order like their bit patterns so atomicMax on the bits is exact).
 __global__ void prep_coeffs_kernel(const float2* __restrict__ coeffs, const float* __restrict__ sigma,
                                    float2* __restrict__ cs, uint16_t* __restrict__ c_hi,
-                                   uint16_t* __restrict__ c_lo, int T, int k) {
+                                   uint16_t* __restrict__ c_lo, uint16_t* __restrict__ c_h16,
+                                   float* __restrict__ tnorm_blk, int T, int k) {
     const int t = blockIdx.x;
     const int tb = t / kGemmTT, r = t % kGemmTT;
     const size_t row_re = ((size_t)tb * 2 * kGemmTT + r) * (size_t)(2 * k);
     const size_t row_im = ((size_t)tb * 2 * kGemmTT + kGemmTT + r) * (size_t)(2 * k);
     if (t >= T) {
         for (int c = threadIdx.x; c < 2 * k; c += blockDim.x) {
-            c_hi[row_re + c] = 0; c_lo[row_re + c] = 0;
-            c_hi[row_im + c] = 0; c_lo[row_im + c] = 0;
+            c_hi[row_re + c] = 0; c_lo[row_re + c] = 0; c_h16[row_re + c] = 0;
+            c_hi[row_im + c] = 0; c_lo[row_im + c] = 0; c_h16[row_im + c] = 0;
         }
         return;
     }
     __shared__ double red[32];
+    __shared__ double red2[32];
     __shared__ float inv_sigma;
     if (sigma == nullptr) {
         double acc = 0.0;
@@ -122,10 +128,17 @@ __global__ void prep_coeffs_kernel(const float2* __restrict__ coeffs, const floa
     }
     __syncthreads();
     const float is = inv_sigma;
+    double nsq = 0.0;
     for (int c = threadIdx.x; c < k; c += blockDim.x) {
         const float2 v = coeffs[(size_t)t * k + c];
         const float a = v.x * is, b = v.y * is;
+        nsq += (double)a * a + (double)b * b;
         cs[(size_t)t * k + c] = make_float2(a, -b);   // conj(c)/sigma for stage 2
+        {
+            const uint16_t ha = __half_as_ushort(__float2half_rn(a)), hb = __half_as_ushort(__float2half_rn(b));
+            c_h16[row_re + 2 * c] = ha;     c_h16[row_re + 2 * c + 1] = hb;
+            c_h16[row_im + 2 * c] = hb ^ 0x8000u; c_h16[row_im + 2 * c + 1] = ha;
+        }
         uint16_t h, l;
         split_bf16(a, h, l);
         c_hi[row_re + 2 * c] = h;     c_lo[row_re + 2 * c] = l;
@@ -135,11 +148,58 @@ __global__ void prep_coeffs_kernel(const float2* __restrict__ coeffs, const floa
         split_bf16(-b, h, l);
         c_hi[row_im + 2 * c] = h;     c_lo[row_im + 2 * c] = l;
     }
+    for (int o = 16; o > 0; o >>= 1) nsq += __shfl_xor_sync(0xffffffffu, nsq, o);
+    if ((threadIdx.x & 31) == 0) red2[threadIdx.x >> 5] = nsq;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s2 = 0.0;
+        for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s2 += red2[i];
+        const float nt = (float)(sqrt(s2) * (1.0 + 1e-6));
+        atomicMax(reinterpret_cast<unsigned*>(tnorm_blk + tb), __float_as_uint(nt));
+    }
 }
 
 cudaError_t launch_prep_coeffs(const float2* coeffs, const float* sigma, float2* cs, uint16_t* c_hi,
-                               uint16_t* c_lo, int T, int Tpad, int k, cudaStream_t st) {
-    prep_coeffs_kernel<<<Tpad, 128, 0, st>>>(coeffs, sigma, cs, c_hi, c_lo, T, k);
+                               uint16_t* c_lo, uint16_t* c_h16, float* tnorm_blk, int T, int Tpad, int k,
+                               cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(tnorm_blk, 0, (size_t)(Tpad / kGemmTT) * sizeof(float), st);
+    if (e != cudaSuccess) return e;
+    prep_coeffs_kernel<<<Tpad, 128, 0, st>>>(coeffs, sigma, cs, c_hi, c_lo, c_h16, tnorm_blk, T, k);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------ per-bin norms (screen mode)
+// bin_norm[i] >= ||beta^avg[i]||_2 over the k columns, from the fp16 plane [kb][bin][64]: the stored values are
+// within 2^-11 relative (+ 2^-25 absolute in the subnormal range) of the fp32 ones, hence the inflation.
+// Eight lanes share a bin (16 bytes each of its 128-byte K-block row); consecutive lanes read consecutive bytes.
+__global__ void __launch_bounds__(256) bin_norm_kernel(const uint16_t* __restrict__ plane, float* __restrict__ bin_norm,
+                                                       int M, int nkb) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long bin = gid >> 3;
+    const int piece = (int)(gid & 7);
+    float acc = 0.f;
+    if (bin < M) {
+        const uint4* p = reinterpret_cast<const uint4*>(plane) + bin * 8 + piece;
+        for (int kb = 0; kb < nkb; ++kb) {
+            const uint4 v = __ldg(p + (size_t)kb * M * 8);
+            const unsigned wds[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&wds[i]));
+                acc = fmaf(f.x, f.x, acc);
+                acc = fmaf(f.y, f.y, acc);
+            }
+        }
+    }
+    acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+    acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+    acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+    if (bin < M && piece == 0) bin_norm[bin] = sqrtf(acc) * (1.0f + 0x1p-9f) + 1e-5f;
+}
+
+cudaError_t launch_bin_norm(const uint16_t* plane_h16, float* bin_norm, int M, int nkb, cudaStream_t st) {
+    const long long threads = (long long)M * 8;
+    bin_norm_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(plane_h16, bin_norm, M, nkb);
     return cudaGetLastError();
 }
 

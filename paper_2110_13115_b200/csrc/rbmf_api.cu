@@ -16,8 +16,8 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 inline int ilog2(int64_t x) { int l = 0; while ((int64_t(1) << l) < x) ++l; return l; }
 
 struct Layout {
-    size_t basisP, Y, beta, bavg_hi, bavg_lo, c_hi, c_lo, cs, tw1_a, tw1_b, twN, dsT, cand, counters, sched,
-        strain_stage, trig_stage, total;
+    size_t basisP, Y, beta, bavg_hi, bavg_lo, c_hi, c_lo, c_h16, tnorm_blk, bin_norm, cs, tw1_a, tw1_b, twN, dsT,
+        cand, cand2, counters, sched, strain_stage, trig_stage, total;
     size_t plane_bytes;
 };
 
@@ -34,6 +34,7 @@ struct rbmf_plan {
     int fft_grid;       // persistent CTAs of the fused FFT kernel
     int64_t max_cand, max_trig;
     int gemm_impl;
+    int last_impl;      // gemm_impl of the last rbmf_filter (decides which candidate list / counter is final)
     int timing;
     cudaStream_t stream;
     uint8_t* ws;
@@ -42,7 +43,7 @@ struct rbmf_plan {
     bool have_ws, have_basis, have_coeffs, filtered;
     int num_sms;
     int last_cuda;
-    CUtensorMap tmA_hi, tmA_lo, tmB_hi, tmB_lo;
+    CUtensorMap tmA_hi, tmA_lo, tmB_hi, tmB_lo, tmB_h16;
     bool have_maps;
     cudaEvent_t ev[5];
     bool have_events;
@@ -64,12 +65,16 @@ Layout make_layout(const rbmf_plan* p) {
     L.bavg_lo = take(L.plane_bytes);
     L.c_hi = take((size_t)p->Tpad * 2 * 2 * k * 2);
     L.c_lo = take((size_t)p->Tpad * 2 * 2 * k * 2);
+    L.c_h16 = take((size_t)p->Tpad * 2 * 2 * k * 2);
+    L.tnorm_blk = take((size_t)(p->Tpad / kGemmTT) * 4);
+    L.bin_norm = take(M * 4);
     L.cs = take((size_t)p->T * k * 8);
     L.tw1_a = take(((size_t)1 << p->logN1) * 8);
     L.tw1_b = take(((size_t)1 << p->logN2) * 8);
     L.twN = take(N * 8);
     L.dsT = take((size_t)p->n_half * 8);
     L.cand = take((size_t)p->max_cand * sizeof(rbmf_candidate));
+    L.cand2 = take((size_t)p->max_cand * sizeof(rbmf_candidate));
     L.counters = take(64 + (size_t)kSchedWords * 4);   // counters, then the FFT scheduler words: one memset
     L.sched = L.counters + 64;
     L.strain_stage = take((size_t)(p->n_half + 1) * 8);
@@ -160,7 +165,7 @@ rbmf_status rbmf_plan_create(rbmf_plan** out, int64_t N, double fs, double f_low
     if (p->j_low >= p->n_half) { delete p; return RBMF_ERR_ARG; }
     p->max_cand = int64_t(1) << 22;
     p->max_trig = int64_t(1) << 22;
-    p->gemm_impl = RBMF_GEMM_TCGEN05;
+    p->gemm_impl = RBMF_GEMM_SCREEN;
     refresh(p);
     *out = p;
     return RBMF_OK;
@@ -190,7 +195,7 @@ rbmf_status rbmf_plan_set_capacity(rbmf_plan* plan, int64_t max_candidates, int6
 
 rbmf_status rbmf_plan_set_gemm_impl(rbmf_plan* plan, int32_t impl) {
     if (!plan) return RBMF_ERR_ARG;
-    if (impl != RBMF_GEMM_TCGEN05 && impl != RBMF_GEMM_SIMT) return RBMF_ERR_ARG;
+    if (impl != RBMF_GEMM_TCGEN05 && impl != RBMF_GEMM_SIMT && impl != RBMF_GEMM_SCREEN) return RBMF_ERR_ARG;
     plan->gemm_impl = impl;
     return RBMF_OK;
 }
@@ -244,6 +249,8 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     if ((s = make_map_planes(plan, &plan->tmA_lo, plan->ws + L.bavg_lo, (uint64_t)plan->M, nkb)) != RBMF_OK) return s;
     if ((s = make_map_rows(plan, &plan->tmB_hi, plan->ws + L.c_hi, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
     if ((s = make_map_rows(plan, &plan->tmB_lo, plan->ws + L.c_lo, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
+    // fp16 data through a 16-bit tensor map: TMA only moves bytes, the element type is irrelevant without OOB fill
+    if ((s = make_map_rows(plan, &plan->tmB_h16, plan->ws + L.c_h16, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
     plan->have_maps = true;
     if (!plan->have_events) {
         for (int i = 0; i < 5; ++i) CK(cudaEventCreate(&plan->ev[i]));
@@ -266,7 +273,8 @@ rbmf_status rbmf_set_coeffs(rbmf_plan* plan, const void* coeffs_dev, const float
     if (!plan->have_ws) return RBMF_ERR_STATE;
     const Layout& L = plan->lay;
     CK(launch_prep_coeffs((const float2*)coeffs_dev, sigma_dev, at<float2>(plan, L.cs), at<uint16_t>(plan, L.c_hi),
-                          at<uint16_t>(plan, L.c_lo), plan->T, plan->Tpad, plan->k, plan->stream));
+                          at<uint16_t>(plan, L.c_lo), at<uint16_t>(plan, L.c_h16), at<float>(plan, L.tnorm_blk),
+                          plan->T, plan->Tpad, plan->k, plan->stream));
     plan->have_coeffs = true;
     return RBMF_OK;
 }
@@ -295,7 +303,12 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     a.plane_hi = at<uint16_t>(plan, L.bavg_hi); a.plane_lo = at<uint16_t>(plan, L.bavg_lo);
     a.sched = at<unsigned>(plan, L.sched);
     a.N = plan->N; a.M = (int)plan->M; a.nchunk = plan->k / kFftC; a.w = plan->w; a.inv_w = 1.0f / (float)plan->w;
+    const bool screen = plan->gemm_impl == RBMF_GEMM_SCREEN;
+    a.plane_fp16 = screen ? 1 : 0;
     CK(launch_fft_fused(a, plan->logN1, plan->logN2, plan->fft_grid, st));
+    if (screen)
+        CK(launch_bin_norm(at<uint16_t>(plan, L.bavg_hi), at<float>(plan, L.bin_norm), (int)plan->M,
+                           (plan->k + 31) / 32, st));
     if (tm) CK(cudaEventRecord(plan->ev[1], st));
 
     // ---- kernel 2: a4-a5 -----------------------------------------------------------------------
@@ -309,7 +322,20 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     g.num_tb = plan->Tpad / kGemmTT;
     g.num_ib = (int)(plan->M / kGemmBM);
     g.group = 16;
-    if (plan->gemm_impl == RBMF_GEMM_TCGEN05) {
+    if (screen) {
+        // Rigorous bound of |R_fp16 - R| for the one-product fp16 screen (derivation: gemm_tcgen05.cu header):
+        // operand rounding u = 2^-11 relative (+ eta = 2^-25 sqrt(2) absolute per complex value in the subnormal
+        // range), fp32 accumulation of 2k exact products bounded by (2k + 64) 2^-22 sqrt(2) relative to ||a|| ||b||.
+        const double u = ldexp(1.0, -11), eta = ldexp(1.0, -25) * 1.4142135623730951;
+        const double k = (double)plan->k;
+        g.bin_norm = at<float>(plan, L.bin_norm);
+        g.tnorm_blk = at<float>(plan, L.tnorm_blk);
+        g.thr1 = thr_stage1;
+        g.kappa1 = (float)((2.0 * u + u * u + (2.0 * k + 64.0) * ldexp(1.0, -22) * 1.4142135623730951) * 1.001);
+        g.kappa2 = (float)(eta * sqrt(k) * 1.001);
+        g.slack = 1e-4f;   // fp32 rounding of the confirm step and of this threshold arithmetic
+        CK(launch_gemm_screen(plan->tmA_hi, plan->tmB_h16, g, plan->num_sms, st));
+    } else if (plan->gemm_impl == RBMF_GEMM_TCGEN05) {
         CK(launch_gemm_tcgen05(plan->tmA_hi, plan->tmA_lo, plan->tmB_hi, plan->tmB_lo, g, plan->num_sms, st));
     } else {
         CK(launch_gemm_simt(at<uint16_t>(plan, L.bavg_hi), at<uint16_t>(plan, L.bavg_lo), at<uint16_t>(plan, L.c_hi),
@@ -322,22 +348,26 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     memset(&s2, 0, sizeof(s2));
     s2.cand = g.cand; s2.cs = at<float2>(plan, L.cs); s2.beta = at<float2>(plan, L.beta);
     s2.out = out_dev; s2.counters = counters;
+    s2.confirmed = at<rbmf_candidate>(plan, L.cand2); s2.thr1_sq = g.thr1_sq; s2.screen = screen ? 1 : 0;
     s2.cand_cap = (unsigned long long)plan->max_cand; s2.trig_cap = (unsigned long long)plan->max_trig;
     s2.thr2_sq = thr_stage2 * thr_stage2; s2.k = plan->k; s2.w = plan->w; s2.N = plan->N;
     CK(launch_stage2(s2, plan->num_sms, st));
     CK(cudaMemcpyAsync(n_out_dev, counters + 1, 8, cudaMemcpyDeviceToDevice, st));
     if (tm) CK(cudaEventRecord(plan->ev[3], st));
     plan->filtered = true;
+    plan->last_impl = plan->gemm_impl;
     return RBMF_OK;
 }
 
 rbmf_status rbmf_get_counts(rbmf_plan* plan, int64_t* n_candidates, int64_t* n_triggers) {
     if (!plan) return RBMF_ERR_ARG;
     if (!plan->filtered) return RBMF_ERR_STATE;
-    unsigned long long h[2] = {0, 0};
-    CK(cudaMemcpyAsync(h, plan->ws + plan->lay.counters, 16, cudaMemcpyDeviceToHost, plan->stream));
+    unsigned long long h[3] = {0, 0, 0};
+    CK(cudaMemcpyAsync(h, plan->ws + plan->lay.counters, 24, cudaMemcpyDeviceToHost, plan->stream));
     CK(cudaStreamSynchronize(plan->stream));
-    if (n_candidates) *n_candidates = (int64_t)h[0];
+    // screen mode: h[0] counts the screened superset, h[2] the candidates confirmed at fp32 accuracy
+    const bool screen = plan->last_impl == RBMF_GEMM_SCREEN;
+    if (n_candidates) *n_candidates = (int64_t)(screen ? h[2] : h[0]);
     if (n_triggers) *n_triggers = (int64_t)h[1];
     if ((int64_t)h[0] > plan->max_cand || (int64_t)h[1] > plan->max_trig) return RBMF_ERR_OVERFLOW;
     return RBMF_OK;
@@ -352,7 +382,8 @@ rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64
     int64_t n = nc < plan->max_cand ? nc : plan->max_cand;
     if (n > capacity) n = capacity;
     if (n > 0) {
-        CK(cudaMemcpyAsync(out_host, plan->ws + plan->lay.cand, (size_t)n * sizeof(rbmf_candidate),
+        const size_t off = plan->last_impl == RBMF_GEMM_SCREEN ? plan->lay.cand2 : plan->lay.cand;
+        CK(cudaMemcpyAsync(out_host, plan->ws + off, (size_t)n * sizeof(rbmf_candidate),
                            cudaMemcpyDeviceToHost, plan->stream));
         CK(cudaStreamSynchronize(plan->stream));
     }
@@ -417,8 +448,8 @@ rbmf_status rbmf_get_stage_ms(rbmf_plan* plan, float ms[4]) {
 
 rbmf_status rbmf_launches_per_filter(const rbmf_plan* plan, int32_t* n) {
     if (!plan || !n) return RBMF_ERR_ARG;
-    // prep_strain + fused FFT + GEMM + stage 2
-    *n = 4;
+    // prep_strain + fused FFT + (screen: bin norms) + GEMM + stage 2
+    *n = plan->gemm_impl == RBMF_GEMM_SCREEN ? 5 : 4;
     return RBMF_OK;
 }
 

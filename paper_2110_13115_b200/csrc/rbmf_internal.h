@@ -47,9 +47,15 @@ struct FftArgs {
     int nchunk;              // k / C
     int w;
     float inv_w;
+    int plane_fp16;          // 1: write ONE fp16 plane (screen mode) into plane_hi; 0: bf16 hi + lo planes
 };
 
 struct GemmArgs {
+    // screen mode only (see gemm_tcgen05.cu): per-bin norms, per-template-block norm maxima, bound constants
+    const float* bin_norm;    // M floats: upper bound of ||beta^avg[i]||_2
+    const float* tnorm_blk;   // num_tb floats: max_t ||c_t||_2 / sigma_t over the block's templates
+    float thr1;
+    float kappa1, kappa2, slack;
     rbmf_candidate* cand;
     unsigned long long* counters;   // [0] = candidates, [1] = triggers
     unsigned long long cand_cap;
@@ -67,6 +73,9 @@ struct Stage2Args {
     const float2* cs;         // T x k: conj(c_tk) / sigma_t
     const float2* beta;       // [chunk][n][C]
     rbmf_trigger* out;
+    rbmf_candidate* confirmed;   // screen mode: candidates whose fp32 averaged SNR passes thr1 (counters[2])
+    float thr1_sq;
+    int screen;                  // 1: `cand` is the screened superset; confirm before scoring
     unsigned long long* counters;
     unsigned long long cand_cap;
     unsigned long long trig_cap;
@@ -81,7 +90,9 @@ cudaError_t launch_init_tables(float2* tw1_a, float2* tw1_b, float2* twN, int lo
 cudaError_t launch_layout_basis(const float2* basis, float2* basisP, int k, int64_t bins, int j_low, int logL1,
                                 int logL2, cudaStream_t st);
 cudaError_t launch_prep_coeffs(const float2* coeffs, const float* sigma, float2* cs, uint16_t* c_hi,
-                               uint16_t* c_lo, int T, int Tpad, int k, cudaStream_t st);
+                               uint16_t* c_lo, uint16_t* c_h16, float* tnorm_blk, int T, int Tpad, int k,
+                               cudaStream_t st);
+cudaError_t launch_bin_norm(const uint16_t* plane_h16, float* bin_norm, int M, int nkb, cudaStream_t st);
 cudaError_t launch_prep_strain(const float2* strain, float2* dsT, int logL1, int logL2, float scale,
                                cudaStream_t st);
 // Fused FFT (a1-a3): configure once per (logL1, logL2) -> CTAs per SM; then launch.
@@ -91,6 +102,9 @@ cudaError_t launch_gemm_simt(const uint16_t* a_hi, const uint16_t* a_lo, const u
                              const uint16_t* c_lo, const GemmArgs& g, cudaStream_t st);
 cudaError_t launch_gemm_tcgen05(const CUtensorMap& tmA_hi, const CUtensorMap& tmA_lo, const CUtensorMap& tmB_hi,
                                 const CUtensorMap& tmB_lo, const GemmArgs& g, int num_sms, cudaStream_t st);
+// screen mode: one fp16 product; tmA = beta^avg fp16 plane, tmB = coefficient fp16 plane
+cudaError_t launch_gemm_screen(const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmArgs& g, int num_sms,
+                               cudaStream_t st);
 cudaError_t gemm_tcgen05_configure();   // sets the dynamic shared memory attribute once
 cudaError_t launch_stage2(const Stage2Args& a, int num_sms, cudaStream_t st);
 

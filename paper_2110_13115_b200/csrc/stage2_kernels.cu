@@ -45,6 +45,28 @@ __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
         }
         // even lane 2r < 2w holds row r (and row 16 + r in slot 1 when w = 32)
         const int nslot = per_chunk > 32 ? 2 : 1;
+        if (a.screen) {
+            // `cand` is the fp16 screen's superset: the fp32 average of the w samples IS the averaged SNR of Eq. 9
+            // (linearity), so the stage-1 test is repeated here at fp32 accuracy.
+            const bool own = (lane & 1) == 0 && lane < per_chunk;
+            float sr = own ? re0 + (nslot == 2 ? re1 : 0.f) : 0.f;
+            float si = own ? im0 + (nslot == 2 ? im1 : 0.f) : 0.f;
+            for (int o = 16; o > 0; o >>= 1) {
+                sr += __shfl_xor_sync(0xffffffffu, sr, o);
+                si += __shfl_xor_sync(0xffffffffu, si, o);
+            }
+            const float inv_w = 1.0f / (float)w;
+            sr *= inv_w; si *= inv_w;
+            if (!(sr * sr + si * si >= a.thr1_sq)) continue;   // warp-uniform
+            if (lane == 0) {
+                const unsigned long long idx = atomicAdd(a.counters + 2, 1ULL);
+                if (idx < a.cand_cap) {
+                    rbmf_candidate c2;
+                    c2.template_id = cd.template_id; c2.bin_index = cd.bin_index; c2.avg_re = sr; c2.avg_im = si;
+                    a.confirmed[idx] = c2;
+                }
+            }
+        }
         for (int s = 0; s < nslot; ++s) {
             const int r = (lane >> 1) + 16 * s;
             const float vr = s ? re1 : re0, vi = s ? im1 : im0;

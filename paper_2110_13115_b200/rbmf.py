@@ -23,7 +23,7 @@ if not os.path.exists(LIB_PATH):
 _lib = ctypes.CDLL(LIB_PATH)
 
 RBMF_OK, RBMF_ERR_ARG, RBMF_ERR_STATE, RBMF_ERR_CUDA, RBMF_ERR_OVERFLOW, RBMF_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
-RBMF_GEMM_TCGEN05, RBMF_GEMM_SIMT = 0, 1
+RBMF_GEMM_TCGEN05, RBMF_GEMM_SIMT, RBMF_GEMM_SCREEN = 0, 1, 2
 
 TRIGGER_DTYPE = np.dtype([("template", np.int32), ("time", np.int32), ("re", np.float32), ("im", np.float32)])
 CANDIDATE_DTYPE = np.dtype([("template", np.int32), ("bin", np.int32), ("re", np.float32), ("im", np.float32)])
@@ -102,6 +102,7 @@ class Plan:
             self._out = torch.empty(self.max_triggers * 4, dtype=torch.int32, device=self.device)
             self._n_out = torch.zeros(1, dtype=torch.int64, device=self.device)
         self._keep = []
+        self.gemm_impl = RBMF_GEMM_SCREEN      # the library's default (include/rbmf.h)
 
     # -- helpers -----------------------------------------------------------------------------
     def _check(self, status, where, allow=()):
@@ -127,6 +128,7 @@ class Plan:
     # -- ABI calls ---------------------------------------------------------------------------
     def set_gemm_impl(self, impl):
         self._check(_lib.rbmf_plan_set_gemm_impl(self._h, int(impl)), "rbmf_plan_set_gemm_impl")
+        self.gemm_impl = int(impl)
 
     def set_timing(self, enabled=True):
         self._check(_lib.rbmf_plan_set_timing(self._h, 1 if enabled else 0), "rbmf_plan_set_timing")
@@ -203,7 +205,8 @@ class Plan:
         return np.sort(out[:n], order=("template", "bin"))
 
     def internal(self, which):
-        """Copy of an internal array: 'beta' -> (N, k) complex64; 'beta_avg' -> (N/w, k) complex64 (hi + lo)."""
+        """Copy of an internal array: 'beta' -> (N, k) complex64; 'beta_avg' -> (N/w, k) complex64 (bf16 hi + lo, or
+        the single fp16 plane in RBMF_GEMM_SCREEN mode)."""
         torch = self._torch
         self.stream.synchronize()
 
@@ -219,8 +222,12 @@ class Plan:
             return torch.view_as_complex(v.permute(1, 0, 2, 3).reshape(self.N, self.k, 2).contiguous()).cpu().numpy()
         if which == "beta_avg":
             M, nkb = self.N // self.w, (self.k + 31) // 32
-            hi = view(1).view(torch.bfloat16).to(torch.float32)
-            lo = view(2).view(torch.bfloat16).to(torch.float32)
+            if self.gemm_impl == RBMF_GEMM_SCREEN:       # one fp16 plane
+                hi = view(1).view(torch.float16).to(torch.float32)
+                lo = torch.zeros_like(hi)
+            else:
+                hi = view(1).view(torch.bfloat16).to(torch.float32)
+                lo = view(2).view(torch.bfloat16).to(torch.float32)
             v = (hi + lo).view(nkb, M, 32, 2).permute(1, 0, 2, 3).reshape(M, nkb * 32, 2)[:, : self.k]   # [kb][bin][32]
             return torch.view_as_complex(v.contiguous()).cpu().numpy()
         raise KeyError(which)

@@ -80,11 +80,13 @@ def test_window_capacity_and_workspace_size(binding):
     assert b.rbmf_workspace_bytes(h, ctypes.byref(nbytes)) == b.RBMF_OK
     assert nbytes.value < default_bytes          # smaller lists
     n = ctypes.c_int32()
-    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 4
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 5   # screen mode (default)
     assert b.rbmf_plan_set_window(h, 1) == b.RBMF_OK
-    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 4
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 5
     assert b.rbmf_plan_set_gemm_impl(h, 7) == b.RBMF_ERR_ARG
     assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_SIMT) == b.RBMF_OK
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 4
+    assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_SCREEN) == b.RBMF_OK
     b.rbmf_plan_destroy(h)
 
 

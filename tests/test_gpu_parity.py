@@ -16,9 +16,14 @@ pytestmark = pytest.mark.gpu
 BETA_ATOL = 1e-5
 
 
-def beta_avg_close(got, ref):
-    """bf16 hi + lo keeps 16 mantissa bits: 2^-17 relative per stored value, on top of the FFT's own error."""
-    return np.all(np.abs(got - ref) <= 1e-5 + 2.0 ** -16 * np.abs(ref))
+X3, SIMT, SCREEN = 0, 1, 2       # rbmf_gemm_impl (include/rbmf.h); SCREEN is the library default
+
+
+def beta_avg_close(got, ref, impl=X3):
+    """bf16 hi + lo keeps 16 mantissa bits: 2^-17 relative per stored value, on top of the FFT's own error.
+    The screen's single fp16 plane keeps 11: 2^-11 relative per component."""
+    rel = 2.0 ** -16 if impl != SCREEN else 2.0 ** -10.4
+    return np.all(np.abs(got - ref) <= 1e-5 + rel * np.abs(ref))
 
 
 @pytest.fixture(scope="module")
@@ -40,11 +45,13 @@ def workload(name, **kw):
     return _WL[key]
 
 
-def make_plan(rbmf, wl, w=None, **kw):
+def make_plan(rbmf, wl, w=None, impl=None, **kw):
     import torch
     cfg = wl["config"]
     plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w if w is None else w,
                      max_candidates=kw.pop("max_candidates", 1 << 20), max_triggers=kw.pop("max_triggers", 1 << 20))
+    if impl is not None:
+        plan.set_gemm_impl(impl)
     plan.set_basis(torch.from_numpy(wl["basis"]))
     plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
     return plan
@@ -56,7 +63,7 @@ def oracle(wl, w, thr1, thr2, templates=None):
                              thr1, thr2, templates=templates)
 
 
-def check(rbmf, wl, w, thr1, thr2, impl=0, expect_triggers=True):
+def check(rbmf, wl, w, thr1, thr2, impl=SCREEN, expect_triggers=True):
     import torch
     cfg = wl["config"]
     plan = make_plan(rbmf, wl, w=w)
@@ -80,10 +87,13 @@ def test_beta_matches_oracle_series(rbmf, name):
     import torch
     wl = workload(name)
     cfg = wl["config"]
-    plan = make_plan(rbmf, wl)
+    plan = make_plan(rbmf, wl, impl=X3)
     plan.filter(torch.from_numpy(wl["strain"]), 50.0, 50.0)
     beta = plan.internal("beta")                       # (N, k)
     bavg = plan.internal("beta_avg")                   # (N/w, k)
+    plan.set_gemm_impl(SCREEN)
+    plan.filter(torch.from_numpy(wl["strain"]), 50.0, 50.0)
+    bavg16 = plan.internal("beta_avg")                 # the screen's single fp16 plane
     plan.close()
     ref = orc.basis_series(wl["strain"], wl["basis"], cfg.N, cfg.j_low)   # (k, N) fp64
     assert 1.2 < np.sqrt((np.abs(ref) ** 2).mean()) < 2.0                 # ~unit-variance quadratures (+ injection)
@@ -91,6 +101,7 @@ def test_beta_matches_oracle_series(rbmf, name):
     assert err < BETA_ATOL, err
     ref_avg = orc.bin_average(ref, cfg.w)
     assert beta_avg_close(bavg.T.astype(np.complex128), ref_avg)
+    assert beta_avg_close(bavg16.T.astype(np.complex128), ref_avg, SCREEN)
 
 
 @pytest.mark.parametrize("N,w", [(1024, 1), (2048, 2), (8192, 4), (32768, 16), (65536, 32)])
@@ -99,7 +110,7 @@ def test_beta_all_fft_lengths(rbmf, N, w):
     import torch
     wl = workload("tiny", N=N, T=16, n_inj=0, index=50 + w)
     cfg = wl["config"]
-    plan = make_plan(rbmf, wl, w=w)
+    plan = make_plan(rbmf, wl, w=w, impl=X3)
     plan.filter(torch.from_numpy(wl["strain"]), 50.0, 50.0)
     beta, bavg = plan.internal("beta"), plan.internal("beta_avg")
     plan.close()
@@ -113,7 +124,7 @@ def test_beta_largest_length_sampled(rbmf):
     import torch
     wl = workload("tiny", N=1 << 20, fs=4096.0, f_low=20.0, T=16, n_inj=0, index=60)
     cfg = wl["config"]
-    plan = make_plan(rbmf, wl, w=8)
+    plan = make_plan(rbmf, wl, w=8, impl=X3)
     plan.filter(torch.from_numpy(wl["strain"]), 50.0, 50.0)
     beta, bavg = plan.internal("beta"), plan.internal("beta_avg")
     plan.close()
@@ -124,7 +135,7 @@ def test_beta_largest_length_sampled(rbmf):
 
 
 # ------------------------------------------------------------------------------- whole path, exhaustive
-@pytest.mark.parametrize("impl", [0, 1])
+@pytest.mark.parametrize("impl", [X3, SIMT, SCREEN])
 @pytest.mark.parametrize("thr", [(3.0, 4.0), (5.0, 6.0)])
 def test_tiny_exhaustive(rbmf, impl, thr):
     check(rbmf, workload("tiny"), 4, thr[0], thr[1], impl=impl)
@@ -135,38 +146,71 @@ def test_tiny_narrow_exhaustive(rbmf):
     assert rep["n_got"] > 0
 
 
+@pytest.mark.parametrize("impl", [X3, SCREEN])
 @pytest.mark.parametrize("w", [1, 2, 4, 8, 16])
-def test_mini_all_windows(rbmf, w):
+def test_mini_all_windows(rbmf, w, impl):
     """N = 16384, k = 32, T = 300 (ragged against the 128-template tile), 3 injections."""
     # fs = 1024 Hz: a 16-sample average washes the peaks out, so the coarse threshold drops with w (PAPER.md:300-312)
     thr1 = {1: 4.0, 2: 4.0, 4: 4.0, 8: 3.5, 16: 2.5}[w]
-    check(rbmf, workload("mini"), w, thr1, 5.0)
+    check(rbmf, workload("mini"), w, thr1, 5.0, impl=impl)
+
+
+def test_mini_largest_window(rbmf):
+    # w = 32 at fs = 1024 Hz averages every peak away: the point is the two-slot row layout of kernel 3
+    rep, crep = check(rbmf, workload("mini"), 32, 1.2, 3.5, impl=SCREEN, expect_triggers=False)
+    assert rep["n_got"] > 0
 
 
 def test_mini_simt_and_tensor_core_candidates_agree(rbmf):
+    """The three stage-1 implementations give the same candidate list (threshold ties aside), and the screen's
+    superset really contains it with a modest overhead."""
     import torch
     wl = workload("mini")
     cfg = wl["config"]
-    sets = []
-    for impl in (0, 1):
-        plan = make_plan(rbmf, wl)
-        plan.set_gemm_impl(impl)
-        plan.filter(torch.from_numpy(wl["strain"]), 2.5, 4.5)
+    sets, trig = [], []
+    for impl in (X3, SIMT, SCREEN):
+        plan = make_plan(rbmf, wl, impl=impl)
+        trig.append(plan.filter(torch.from_numpy(wl["strain"]), 2.5, 4.5))
         sets.append(plan.candidates())
         plan.close()
-    a, b = sets
+    a = sets[0]
     ka = a["template"].astype(np.int64) * cfg.N + a["bin"]
-    kb = b["template"].astype(np.int64) * cfg.N + b["bin"]
-    sym = np.setxor1d(ka, kb)
     assert len(ka) > 1000
-    assert len(sym) <= max(2, len(ka) // 2000)          # only threshold ties may differ
-    common, ia, ib = np.intersect1d(ka, kb, return_indices=True)
-    assert np.abs(a["re"][ia] - b["re"][ib]).max() < 2e-4 and np.abs(a["im"][ia] - b["im"][ib]).max() < 2e-4
+    for b in sets[1:]:
+        kb = b["template"].astype(np.int64) * cfg.N + b["bin"]
+        sym = np.setxor1d(ka, kb)
+        assert len(sym) <= max(2, len(ka) // 2000)          # only threshold ties may differ
+        common, ia, ib = np.intersect1d(ka, kb, return_indices=True)
+        assert np.abs(a["re"][ia] - b["re"][ib]).max() < 2e-4 and np.abs(a["im"][ia] - b["im"][ib]).max() < 2e-4
+    # final triggers: identical sets between bf16x3 and screen + fp32 confirm, up to ties at thr1
+    ta = trig[0]["template"].astype(np.int64) * cfg.N + trig[0]["time"]
+    tc = trig[2]["template"].astype(np.int64) * cfg.N + trig[2]["time"]
+    assert len(np.setxor1d(ta, tc)) <= max(2, len(ta) // 500)
 
 
-def test_small_config_exhaustive(rbmf):
+def test_screen_superset_is_tight(rbmf):
+    """How many (template, bin) pairs the fp16 screen passes relative to the confirmed candidates: the rigorous
+    error bound must cost only a modest surplus (it is O(2^-10 ||beta^avg||) ~ 0.01-0.03 in SNR)."""
+    import torch
+    wl = workload("small")
+    cfg = wl["config"]
+    plan = make_plan(rbmf, wl, impl=SCREEN)
+    plan.filter(torch.from_numpy(wl["strain"]), cfg.thr1, cfg.thr2)
+    n_conf = plan.counts()[0]
+    plan.set_gemm_impl(X3)
+    plan.filter(torch.from_numpy(wl["strain"]), cfg.thr1 - 0.05, cfg.thr2)
+    n_loose = plan.counts()[0]
+    plan.filter(torch.from_numpy(wl["strain"]), cfg.thr1, cfg.thr2)
+    n_x3 = plan.counts()[0]
+    plan.close()
+    assert abs(n_conf - n_x3) <= max(3, n_x3 // 500)
+    assert n_conf <= n_loose                       # sanity of the scale: thr1 - 0.05 already admits more
+
+
+@pytest.mark.parametrize("impl", [X3, SCREEN])
+def test_small_config_exhaustive(rbmf, impl):
     """BASELINE.json configs[1]: N = 131072, k = 128, T = 2000, w = 8, thresholds 5.0 / 6.0, 10 injections."""
-    rep, crep = check(rbmf, workload("small"), 8, 5.0, 6.0)
+    rep, crep = check(rbmf, workload("small"), 8, 5.0, 6.0, impl=impl)
     assert rep["n_got"] > 100
 
 
@@ -217,7 +261,12 @@ def test_zero_strain_gives_nothing(rbmf):
 def test_overflow_is_reported_and_bounded(rbmf):
     import torch
     wl = workload("tiny")
-    plan = make_plan(rbmf, wl, max_candidates=64, max_triggers=16)
+    plan = make_plan(rbmf, wl, impl=SCREEN, max_candidates=64, max_triggers=1 << 16)
+    plan.filter_async(torch.from_numpy(wl["strain"]).cuda(), 2.0, 2.0)
+    nc, nt, st = plan.counts(allow_overflow=True)
+    assert st == rbmf.RBMF_ERR_OVERFLOW and nc <= 64      # screened list overflowed; confirmed <= processed
+    plan.close()
+    plan = make_plan(rbmf, wl, impl=X3, max_candidates=64, max_triggers=16)
     plan.filter_async(torch.from_numpy(wl["strain"]).cuda(), 2.0, 2.0)
     nc, nt, st = plan.counts(allow_overflow=True)
     assert st == rbmf.RBMF_ERR_OVERFLOW and nc > 64
@@ -290,14 +339,15 @@ def test_non_default_stream(rbmf):
 
 
 # ------------------------------------------------------------- full size, bench launch configuration
-def test_paper_scale_sampled(rbmf):
+@pytest.mark.parametrize("impl", [SCREEN, X3])
+def test_paper_scale_sampled(rbmf, impl):
     """BASELINE.json configs[2] (N = 524288, k = 256, T = 20000, w = 8; what bench.py times): soundness of sampled
     reported triggers by pointwise O(|B|) re-evaluation (no FFT), completeness on a template subset (all injected
     templates + seeded random ones) by the exhaustive oracle."""
     import torch
     wl = workload("paper")
     cfg = wl["config"]
-    plan = make_plan(rbmf, wl, max_candidates=1 << 22, max_triggers=1 << 22)
+    plan = make_plan(rbmf, wl, impl=impl, max_candidates=1 << 22, max_triggers=1 << 22)
     got = plan.filter(torch.from_numpy(wl["strain"]), cfg.thr1, cfg.thr2)
     nc, nt, _ = plan.counts()
     plan.close()
