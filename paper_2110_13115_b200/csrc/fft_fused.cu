@@ -11,11 +11,12 @@
 // outputs through shared memory before writing the bf16 hi/lo operand planes of kernel 2.
 //
 // Columns are processed in chunks of C = 4 (32-byte row segments).  The work queue is ordered
-//   P1(0) P1(1) P2(0) P1(2) P2(1) ... so that chunk c's intermediate Y (N * 32 bytes, one of kFftRing ring slots) is
-// written and read back while it is still in the 126 MB L2; only the basis (read) and beta / planes (written) touch
-// HBM.  CTAs draw tickets from a global counter; a pass-2 item waits on its chunk's pass-1 completion counter, a
-// pass-1 tile on the completion of the pass-2 items that last read its ring slot.  Every waited-on ticket is lower
-// than the waiting one and already owned by a running CTA, so the scheme cannot deadlock.
+//   P1(0) P1(1) P2(0) P1(2) P2(1) ... so that chunk c's intermediate Y (N * 32 bytes) is written and read back while
+// it is still in the 126 MB L2.  Y lives IN PLACE in the chunk's block of the beta array (Y[n1][j2] at the address
+// of beta[n1 + L1 j2]): a pass-2 item reads exactly the addresses it then overwrites, dirty Y lines are normally
+// overwritten in L2 before they are ever evicted, and only the basis (read) and beta / planes (written) touch HBM.
+// CTAs draw tickets from a global counter; a pass-2 item waits on its chunk's pass-1 completion counter.  Every
+// waited-on ticket is lower than the waiting one and already owned by a running CTA, so the scheme cannot deadlock.
 //
 // Inside a CTA (256 threads) a line of length L = R0 * R1 is two Stockham stages: a thread owns one column and R0
 // elements, computes a radix-R0 butterfly in registers, exchanges through padded shared memory, then R0/R1
@@ -113,13 +114,17 @@ __device__ __forceinline__ float2 ld_stream(const float2* p) {
     return v;
 }
 
+// Poll with relaxed loads (an acquire load would invalidate the SM's L1 on every iteration); the data guarded by
+// the counter (Y) is read with ld.global.cg, i.e. from L2, the point of coherence, after the CTA barrier that
+// follows this wait.
 __device__ __forceinline__ void wait_counter(const unsigned* p, unsigned target) {
     for (;;) {
         unsigned v;
-        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-        if (v >= target) return;
-        __nanosleep(64);
+        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+        if (v >= target) break;
+        __nanosleep(100);
     }
+    __threadfence();
 }
 
 template <int LOGL>
@@ -147,7 +152,6 @@ template <int LOG1, int LOG2>
 __device__ __forceinline__ void p1_tile(const FftArgs& a, int chunk, int tile, float2* smem) {
     using K = Cfg<LOG1>;
     constexpr int L1 = K::L, L2 = 1 << LOG2, R0 = K::R0, R1 = K::R1, W = K::W, H = L1 / 2;
-    constexpr int G = fft_group(LOG2);
     constexpr int RS = region_stride(K::ROWS, K::P1LANES);
     const int tid = threadIdx.x;
     const int col = tid % C, wk = (tid / C) % W, line = tid / (C * W);
@@ -168,15 +172,13 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int chunk, int tile, f
     float2* reg = smem + line * RS;
 #pragma unroll
     for (int m = 0; m < R0; ++m) reg[(wk * (R0 + 1) + m) * C + col] = u[m];
-    // the ring slot this tile writes was last read by pass 2 of chunk - kFftRing
-    if (tid == 0 && chunk >= kFftRing) {
-        const int span = a.w > Cfg<LOG2>::SUB ? a.w : Cfg<LOG2>::SUB;
-        wait_counter(a.sched + 16 + kMaxChunks + (chunk - kFftRing), (unsigned)(L1 / span));
-    }
     __syncthreads();
 
     // ---- stage 1 + inter-pass twiddle + store -----------------------------------------------------
-    float2* yslot = a.Y + (size_t)(chunk % kFftRing) * (size_t)a.N * C;
+    // Y[n1][j2] is stored IN the chunk's beta block, at the address of beta[n1 + L1 j2]: the pass-2 item that owns
+    // lines n1 reads exactly the addresses it later overwrites with beta, so no second buffer (and no buffer
+    // hand-over between chunks) exists, and this tile's 1024 x C outputs are one contiguous run.
+    float2* yrow = a.beta + ((size_t)chunk * (size_t)a.N + (size_t)j2 * L1) * C;
     const float2* tn = a.twN + (size_t)j2 * L1;
 #pragma unroll
     for (int bb = 0; bb < R0 / R1; ++bb) {
@@ -191,7 +193,7 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int chunk, int tile, f
         for (int m = 0; m < R1; ++m) {
             const int n1 = b + m * R0;
             const float2 v = cmul(x[m], __ldg(tn + n1));
-            __stcg(yslot + ((size_t)(n1 / G) * L2 + j2) * (size_t)(G * C) + (n1 % G) * C + col, v);
+            __stcg(yrow + n1 * C + col, v);
         }
     }
     __syncthreads();
@@ -222,7 +224,6 @@ template <int LOG1, int LOG2>
 __device__ __forceinline__ void p2_item(const FftArgs& a, int chunk, int item, float2* smem) {
     using K = Cfg<LOG2>;
     constexpr int L1 = 1 << LOG1, L2 = K::L, R0 = K::R0, R1 = K::R1, W = K::W, SUB = K::SUB;
-    constexpr int G = fft_group(LOG2);
     constexpr int RS = region_stride(K::ROWS, K::P2LANES);
     constexpr int NIT = (L2 * C + NT - 1) / NT;   // reduced outputs per thread and per group of lines
     const int tid = threadIdx.x;
@@ -236,8 +237,7 @@ __device__ __forceinline__ void p2_item(const FftArgs& a, int chunk, int item, f
     if (tid == 0) wait_counter(a.sched + 16 + chunk, (unsigned)(L2 / Cfg<LOG1>::SUB));
     __syncthreads();
 
-    const float2* yslot = a.Y + (size_t)(chunk % kFftRing) * (size_t)a.N * C;
-    float2* bchunk = a.beta + (size_t)chunk * (size_t)a.N * C;
+    float2* bchunk = a.beta + (size_t)chunk * (size_t)a.N * C;   // holds Y on entry, beta on exit (in place)
     float2* reg = smem + line * RS;
     float2 acc[NIT];
 #pragma unroll
@@ -247,9 +247,9 @@ __device__ __forceinline__ void p2_item(const FftArgs& a, int chunk, int item, f
         const int n1 = n1_0 + rd * SUB + line;
         float2 u[R0];
         {
-            const float2* yp = yslot + (size_t)(n1 / G) * L2 * (size_t)(G * C) + (n1 % G) * C + col;
+            const float2* yp = bchunk + (size_t)n1 * C + col;
 #pragma unroll
-            for (int q = 0; q < R0; ++q) u[q] = __ldcg(yp + (size_t)(wk + q * W) * (G * C));
+            for (int q = 0; q < R0; ++q) u[q] = __ldcg(yp + (size_t)(wk + q * W) * (L1 * C));
         }
         dft<R0>(u);
 #pragma unroll
@@ -308,10 +308,6 @@ __device__ __forceinline__ void p2_item(const FftArgs& a, int chunk, int item, f
         }
         __syncthreads();
     }
-    if (tid == 0) {
-        __threadfence();
-        atomicAdd(a.sched + 16 + kMaxChunks + chunk, 1u);
-    }
 }
 
 // ------------------------------------------------------------------------------------------- kernel
@@ -342,18 +338,16 @@ __global__ void __launch_bounds__(NT, 2) fft_fused_kernel(const FftArgs a) {
         // draw the next ticket early; every tile has a barrier between this write and the read below
         if (threadIdx.x == 0) s_next[(it + 1) & 1] = (int)atomicAdd(a.sched, 1u);
         // queue order: P1(0) | P1(1) P2(0) | P1(2) P2(1) | ... | P1(n-1) P2(n-2) | P2(n-1)
-        if (t < n1t) {
-            p1_tile<LOG1, LOG2>(a, 0, t, smem);
-        } else {
+        int chunk = 0, idx = t;
+        bool first = true;
+        if (t >= n1t) {
             const int u = t - n1t;
             const int blk = u / per, v = u - blk * per;
-            if (blk < a.nchunk - 1) {
-                if (v < n1t) p1_tile<LOG1, LOG2>(a, blk + 1, v, smem);
-                else p2_item<LOG1, LOG2>(a, blk, v - n1t, smem);
-            } else {
-                p2_item<LOG1, LOG2>(a, a.nchunk - 1, v, smem);
-            }
+            if (blk < a.nchunk - 1 && v < n1t) { chunk = blk + 1; idx = v; }
+            else { first = false; chunk = blk; idx = blk < a.nchunk - 1 ? v - n1t : v; }
         }
+        if (first) p1_tile<LOG1, LOG2>(a, chunk, idx, smem);
+        else p2_item<LOG1, LOG2>(a, chunk, idx, smem);
         t = s_next[(it + 1) & 1];
     }
 }

@@ -16,7 +16,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 inline int ilog2(int64_t x) { int l = 0; while ((int64_t(1) << l) < x) ++l; return l; }
 
 struct Layout {
-    size_t basisP, Y, beta, bavg_hi, bavg_lo, c_hi, c_lo, c_h16, tnorm_blk, bin_norm, cs, tw1_a, tw1_b, twN, dsT,
+    size_t basisP, beta, bavg_hi, bavg_lo, c_hi, c_lo, c_h16, tnorm_blk, bin_norm, cs, tw1_a, tw1_b, twN, dsT,
         cand, cand2, counters, sched, strain_stage, trig_stage, total;
     size_t plane_bytes;
 };
@@ -59,7 +59,6 @@ Layout make_layout(const rbmf_plan* p) {
     const size_t nkb = (k + 31) / 32;
     L.plane_bytes = nkb * M * 64 * 2;
     L.basisP = take((size_t)p->n_half * k * 8);
-    L.Y = take((size_t)kFftRing * N * kFftC * 8);
     L.beta = take(N * k * 8);
     L.bavg_hi = take(L.plane_bytes);
     L.bavg_lo = take(L.plane_bytes);
@@ -299,7 +298,7 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     memset(&a, 0, sizeof(a));
     a.basisP = at<float2>(plan, L.basisP); a.dsT = at<float2>(plan, L.dsT);
     a.tw1_a = at<float2>(plan, L.tw1_a); a.tw1_b = at<float2>(plan, L.tw1_b); a.twN = at<float2>(plan, L.twN);
-    a.Y = at<float2>(plan, L.Y); a.beta = at<float2>(plan, L.beta);
+    a.beta = at<float2>(plan, L.beta);
     a.plane_hi = at<uint16_t>(plan, L.bavg_hi); a.plane_lo = at<uint16_t>(plan, L.bavg_lo);
     a.sched = at<unsigned>(plan, L.sched);
     a.N = plan->N; a.M = (int)plan->M; a.nchunk = plan->k / kFftC; a.w = plan->w; a.inv_w = 1.0f / (float)plan->w;

@@ -11,7 +11,6 @@ namespace rbmf {
 
 constexpr int kFftC = 4;           // basis columns per FFT chunk (32-byte row segments)
 constexpr int kFftThreads = 256;   // threads per FFT CTA
-constexpr int kFftRing = 3;        // chunk slots of the L2-resident intermediate Y
 constexpr int kMaxChunks = 256;    // k <= 1024
 constexpr int kGemmBM = 128;       // time bins per GEMM tile (UMMA M)
 constexpr int kGemmTT = 128;       // templates per GEMM tile (UMMA N = 2*kGemmTT: re | im rows)
@@ -23,12 +22,9 @@ __host__ __device__ constexpr int fft_r0(int logL) { return logL >= 9 ? 32 : (lo
 __host__ __device__ constexpr int fft_r1(int logL) { return (1 << logL) / fft_r0(logL); }
 // lines (independent transforms) a 256-thread CTA works on in lockstep
 __host__ __device__ constexpr int fft_sub(int logL) { return kFftThreads / (fft_r1(logL) * kFftC); }
-// inner row group of the Y layout: Y[slot][n1 / g][j2][n1 % g][C]
-__host__ __device__ constexpr int fft_group(int logL2) { return fft_sub(logL2) < 8 ? fft_sub(logL2) : 8; }
 
-// Scheduler words (uint32) in the workspace: [0] ticket, [16 + c] pass-1 tiles done of chunk c,
-// [16 + kMaxChunks + c] pass-2 items done of chunk c.
-constexpr int kSchedWords = 16 + 2 * kMaxChunks;
+// Scheduler words (uint32) in the workspace: [0] ticket, [16 + c] pass-1 tiles done of chunk c.
+constexpr int kSchedWords = 16 + kMaxChunks;
 
 // Device views handed to the fused FFT kernel.
 struct FftArgs {
@@ -37,8 +33,7 @@ struct FftArgs {
     const float2* tw1_a;     // pass 1 stage-1 twiddles  [q < R1][b < R0] = e^{2 pi i q b / L1}
     const float2* tw1_b;     // pass 2 stage-1 twiddles, same for L2
     const float2* twN;       // inter-pass twiddles [j2 < L2][n1 < L1] = e^{2 pi i j2 n1 / N}
-    float2* Y;               // ring of kFftRing chunk slots, N * C entries each
-    float2* beta;            // [chunk][n < N][C]
+    float2* beta;            // [chunk][n < N][C]; between the passes it holds Y[n1][j2] at index n1 + L1 j2
     uint16_t* plane_hi;      // [kb = col / 32][bin < M][64]: bf16 (re, im) of column col % 32
     uint16_t* plane_lo;
     unsigned* sched;         // kSchedWords
