@@ -40,8 +40,28 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
 __device__ __forceinline__ float2 cmul_conj(float2 d, float2 b) {   // d * conj(b)
     return make_float2(d.x * b.x + d.y * b.y, d.y * b.x - d.x * b.y);
 }
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// Complex add / subtract as ONE packed fp32x2 instruction (FADD2 on sm_100): the butterflies are ~2/3 additions, and
+// the kernel is bound by instruction issue, not by the fp32 lanes (a packed op does two lanes' work per issue slot).
+__device__ __forceinline__ unsigned long long pk2(float2 a) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y));
+    return r;
+}
+__device__ __forceinline__ float2 upk2(unsigned long long r) {
+    float2 a;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r));
+    return a;
+}
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) {
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a)), "l"(pk2(b)));
+    return upk2(r);
+}
+__device__ __forceinline__ float2 csub(float2 a, float2 b) {
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a)), "l"(pk2(b)));
+    return upk2(r);
+}
 
 // v * e^{+2 pi i m / 32}, 0 <= m < 16; m is a compile-time constant after unrolling.
 __device__ __forceinline__ float2 mul_w32(float2 v, int m) {
@@ -243,14 +263,18 @@ __device__ __forceinline__ void p2_item(const FftArgs& a, int chunk, int item, f
 #pragma unroll
     for (int i = 0; i < NIT; ++i) acc[i] = make_float2(0.f, 0.f);
 
+    // Y loads of line n1 (stage-0 inputs).  The loads of round rd + 1 are issued as soon as u[] is free in round rd
+    // (after its outputs went to shared memory for the bin sums), so their L2 latency overlaps the summation.
+    float2 u[R0];
+    auto load_line = [&](int n1) {
+        const float2* yp = bchunk + (size_t)n1 * C + col;
+#pragma unroll
+        for (int q = 0; q < R0; ++q) u[q] = __ldcg(yp + (size_t)(wk + q * W) * (L1 * C));
+    };
+    load_line(n1_0 + line);
+
     for (int rd = 0; rd < rounds; ++rd) {
         const int n1 = n1_0 + rd * SUB + line;
-        float2 u[R0];
-        {
-            const float2* yp = bchunk + (size_t)n1 * C + col;
-#pragma unroll
-            for (int q = 0; q < R0; ++q) u[q] = __ldcg(yp + (size_t)(wk + q * W) * (L1 * C));
-        }
         dft<R0>(u);
 #pragma unroll
         for (int m = 0; m < R0; ++m) reg[(wk * (R0 + 1) + m) * C + col] = u[m];
@@ -269,41 +293,44 @@ __device__ __forceinline__ void p2_item(const FftArgs& a, int chunk, int item, f
                 const int n2 = b + m * R0;
                 const size_t n = (size_t)n1 + (size_t)L1 * n2;
                 __stcs(bchunk + n * C + col, x[m]);
-                if (w == 1) store_planes(a, (int)n, gcol, x[m]);
                 u[bb * R1 + m] = x[m];
             }
         }
-        if (w > 1) {
-            // ---- a3: sum the outputs of gs = min(w, SUB) consecutive lines at equal n2 --------------------
-            __syncthreads();   // every stage-1 read of the exchange regions is done
+        // ---- a3: sum the outputs of gs = min(w, SUB) consecutive lines at equal n2 ------------------------
+        __syncthreads();   // every stage-1 read of the exchange regions is done
 #pragma unroll
-            for (int bb = 0; bb < R0 / R1; ++bb)
+        for (int bb = 0; bb < R0 / R1; ++bb)
 #pragma unroll
-                for (int m = 0; m < R1; ++m) reg[((wk + bb * W) + m * R0) * C + col] = u[bb * R1 + m];
-            __syncthreads();
-            const int gs = w < SUB ? w : SUB;
-            const int nb = SUB / gs;   // bins (per n2) completed by this round when w <= SUB
+            for (int m = 0; m < R1; ++m) reg[((wk + bb * W) + m * R0) * C + col] = u[bb * R1 + m];
+        if (rd + 1 < rounds) load_line(n1 + SUB);
+        __syncthreads();
+        if (w >= SUB) {
+            // all SUB lines of this round fall into one bin per n2; a bin spans `rounds` rounds
 #pragma unroll
-            for (int it = 0; it < SUB * NIT; ++it) {
-                const int e = tid + it * NT;                // (rb, n2, col): col is this thread's own
-                if (e < nb * L2 * C) {
-                    const int rb = e / (L2 * C), n2 = (e % (L2 * C)) / C;
-                    float2 s = make_float2(0.f, 0.f);
+            for (int it = 0; it < NIT; ++it) {
+                const int e = tid + it * NT;   // (n2, col): col is this thread's own
+                if (L2 * C >= NT || e < L2 * C) {
+                    const int n2 = e / C;
+                    float2 sum = smem[n2 * C + col];
 #pragma unroll
-                    for (int rr = 0; rr < SUB; ++rr)
-                        if (rr < gs) s = cadd(s, smem[(rb * gs + rr) * RS + n2 * C + col]);
-                    if (w > SUB) {
-                        if (it < NIT) {
-                            acc[it] = cadd(acc[it], s);
-                            if (rd == rounds - 1)
-                                store_planes(a, n1_0 / w + (L1 / w) * n2, gcol,
-                                             make_float2(acc[it].x * a.inv_w, acc[it].y * a.inv_w));
-                        }
-                    } else {
-                        store_planes(a, (n1_0 + rb * gs) / w + (L1 / w) * n2, gcol,
-                                     make_float2(s.x * a.inv_w, s.y * a.inv_w));
-                    }
+                    for (int rr = 1; rr < SUB; ++rr) sum = cadd(sum, smem[rr * RS + n2 * C + col]);
+                    acc[it] = cadd(acc[it], sum);
+                    if (rd == rounds - 1)
+                        store_planes(a, n1_0 / w + (L1 / w) * n2, gcol,
+                                     make_float2(acc[it].x * a.inv_w, acc[it].y * a.inv_w));
                 }
+            }
+        } else {
+            // w < SUB (including w = 1): this round completes SUB / w bins per n2; compact, not unrolled
+            const int nb = SUB / w;
+#pragma unroll 1
+            for (int e = tid; e < nb * L2 * C; e += NT) {
+                const int rb = e / (L2 * C), n2 = (e % (L2 * C)) / C;
+                float2 sum = smem[(rb * w) * RS + n2 * C + col];
+#pragma unroll 1
+                for (int rr = 1; rr < w; ++rr) sum = cadd(sum, smem[(rb * w + rr) * RS + n2 * C + col]);
+                store_planes(a, (n1_0 + rd * SUB + rb * w) / w + (L1 / w) * n2, gcol,
+                             make_float2(sum.x * a.inv_w, sum.y * a.inv_w));
             }
         }
         __syncthreads();
