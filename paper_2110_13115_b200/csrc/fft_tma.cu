@@ -1,0 +1,559 @@
+// Kernel 1 (steps a1-a3 of include/rbmf.h): pointwise correlation fused into a batched inverse FFT, the w-sample
+// bin average fused into its last pass -- ONE persistent, warp-specialised launch whose intermediate stays in L2.
+//
+// Four-step FFT, N = L1 * L2, per basis column:
+//   pass 1 (line = j2, length L1):  Y[n1][j2] = e^{2 pi i j2 n1 / N} sum_{j1} G[j1 L2 + j2] e^{2 pi i j1 n1 / L1}
+//   pass 2 (line = n1, length L2):  beta[n1 + L1 n2] = sum_{j2} Y[n1][j2] e^{2 pi i j2 n2 / L2}
+// with G[j] = s d[j] conj(b[j]) formed by pass 1 as it reads its inputs (a1) and zero for
+// j >= N/2 (one-sided spectrum: the upper half of every pass-1 line is never read and its first radix-2 level is
+// pruned).  beta^avg (a3, Eq. 9) sums w consecutive samples n = n1 + L1 n2, i.e. w consecutive lines
+// n1 at equal n2: a pass-2 item owns max(w, SUB) consecutive lines and reduces their outputs through shared memory
+// before writing the operand plane(s) of kernel 2.
+//
+// Columns are processed in chunks of C = 4 (32-byte row segments).  Work queue (global ticket counter):
+//   P1(0) | P1(1) P2(0) | P1(2) P2(1) | ...   so chunk c's intermediate Y (N * 32 bytes) is written and read back
+// while it is still in the 126 MB L2.  Y lives IN PLACE in the chunk's block of the beta array (Y[n1][j2] at the
+// address of beta[n1 + L1 j2]): a pass-2 item reads exactly the addresses it then overwrites, so dirty Y lines are
+// overwritten in L2 before they are evicted and only basis (read) and beta / planes (written) touch HBM.
+//
+// One CTA per SM, 16 consumer warps + a producer warpgroup of which one warp works:
+//   warp 16      producer: draws tickets, waits for a chunk's pass-1 completion counter before its pass-2 items, and
+//                moves every tile's input into one of three shared-memory tile buffers with bulk-async copies
+//                (cp.async.bulk 1-D for the basis block and the strain slice of a pass-1 tile; a 3-D tensor map over
+//                the beta array for the strided Y rows of a pass-2 tile), completion signalled on an mbarrier;
+//   warps 0-7, 8-15  two consumer groups of 256 threads; tiles alternate strictly between them (tile i -> group
+//                i & 1, buffer i % 3), so a group never waits on global-memory latency: its next tile is loaded while
+//                it computes.  Groups synchronise internally with a named barrier (bar.sync id, 256).
+// Inside a group a line of length L = R0 * R1 is two Stockham stages: a thread owns one column and R0 elements; stage 0
+// reads its elements (positions wk + q W) from the tile buffer, does a radix-R0 DFT in registers and writes the results
+// back IN PLACE (the same, thread-private positions); after the group barrier stage 1 reads R1 consecutive positions,
+// applies the twiddles (table in shared memory), does a radix-R1 DFT and stores straight to global memory.
+// Tile buffer layout: [position][line][column] (one row = SUB lines x 4 columns), conflict-free for both stages; when
+// a row is only 64 bytes (L = 1024) one pad row per 32 rows keeps stage 1 conflict-free.
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include "rbmf_internal.h"
+
+namespace rbmf {
+
+namespace {
+
+constexpr int C = kFftC;
+constexpr int GT = kFftThreads;         // threads per consumer group
+constexpr int NGROUP = 2;
+constexpr int NT = NGROUP * GT + 128;   // + producer warpgroup (one working warp; setmaxnreg acts on warpgroups)
+constexpr int NBUF = 3;
+
+// ------------------------------------------------------------------------------------------------ complex helpers
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ float2 cmul_conj(float2 d, float2 b) {   // d * conj(b)
+    return make_float2(d.x * b.x + d.y * b.y, d.y * b.x - d.x * b.y);
+}
+// Complex add / subtract as ONE packed fp32x2 instruction (FADD2 on sm_100): the butterflies are ~2/3 additions and
+// the kernel is bound by instruction issue, not by the fp32 lanes.
+__device__ __forceinline__ unsigned long long pk2(float2 a) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y));
+    return r;
+}
+__device__ __forceinline__ float2 upk2(unsigned long long r) {
+    float2 a;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r));
+    return a;
+}
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) {
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a)), "l"(pk2(b)));
+    return upk2(r);
+}
+__device__ __forceinline__ float2 csub(float2 a, float2 b) {
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a)), "l"(pk2(b)));
+    return upk2(r);
+}
+
+// v * e^{+2 pi i m / 32}, 0 <= m < 16; m is a compile-time constant after unrolling.
+__device__ __forceinline__ float2 mul_w32(float2 v, int m) {
+    constexpr float CS[9] = {1.0f,
+                             0.98078528040323044913f,
+                             0.92387953251128675613f,
+                             0.83146961230254523708f,
+                             0.70710678118654752440f,
+                             0.55557023301960222474f,
+                             0.38268343236508977173f,
+                             0.19509032201612826785f,
+                             0.0f};
+    if (m == 0) return v;
+    if (m == 8) return make_float2(-v.y, v.x);
+    if (m == 4) return make_float2((v.x - v.y) * CS[4], (v.x + v.y) * CS[4]);
+    if (m == 12) return make_float2((-v.x - v.y) * CS[4], (v.x - v.y) * CS[4]);
+    const float c = m < 8 ? CS[m] : -CS[16 - m];
+    const float s = m < 8 ? CS[8 - m] : CS[m - 8];
+    return cmul(v, make_float2(c, s));
+}
+
+// In-register inverse DFT of length R (natural order in and out): x[m] <- sum_j x[j] e^{+2 pi i j m / R}.
+template <int R>
+__device__ __forceinline__ void dft(float2 (&x)[R]) {
+    if constexpr (R == 2) {
+        const float2 a = x[0], b = x[1];
+        x[0] = cadd(a, b);
+        x[1] = csub(a, b);
+    } else {
+        float2 e[R / 2], o[R / 2];
+#pragma unroll
+        for (int i = 0; i < R / 2; ++i) { e[i] = x[2 * i]; o[i] = x[2 * i + 1]; }
+        dft<R / 2>(e);
+        dft<R / 2>(o);
+#pragma unroll
+        for (int i = 0; i < R / 2; ++i) {
+            const float2 t = mul_w32(o[i], i * (32 / R));
+            x[i] = cadd(e[i], t);
+            x[i + R / 2] = csub(e[i], t);
+        }
+    }
+}
+
+// Same, for an input whose upper half x[R/2 .. R) is zero (and not read): the deepest level degenerates to a copy.
+template <int R>
+__device__ __forceinline__ void dft_half(float2 (&x)[R]) {
+    if constexpr (R == 2) {
+        x[1] = x[0];
+    } else {
+        float2 e[R / 2], o[R / 2];
+#pragma unroll
+        for (int i = 0; i < R / 4; ++i) { e[i] = x[2 * i]; o[i] = x[2 * i + 1]; }
+        dft_half<R / 2>(e);
+        dft_half<R / 2>(o);
+#pragma unroll
+        for (int i = 0; i < R / 2; ++i) {
+            const float2 t = mul_w32(o[i], i * (32 / R));
+            x[i] = cadd(e[i], t);
+            x[i + R / 2] = csub(e[i], t);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------ mbarrier / bulk-copy helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+// 1-D bulk copy global -> shared (16-byte aligned addresses, size a multiple of 16), completion on an mbarrier.
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y, int z) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(dst),
+        "l"(map), "r"(bar), "r"(x), "r"(y), "r"(z)
+        : "memory");
+}
+__device__ __forceinline__ void group_sync(int g) {   // named barrier of one consumer group
+    if (g == 0) asm volatile("bar.sync 1, %0;" ::"n"(GT) : "memory");
+    else asm volatile("bar.sync 2, %0;" ::"n"(GT) : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Poll with relaxed loads (an acquire load would invalidate the SM's L1 on every iteration).
+__device__ __forceinline__ void wait_counter(const unsigned* p, unsigned target) {
+    for (;;) {
+        unsigned v;
+        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+        if (v >= target) break;
+        __nanosleep(100);
+    }
+    __threadfence();
+    asm volatile("fence.proxy.async;" ::: "memory");   // the guarded data is read next through the async proxy (TMA)
+}
+
+// ------------------------------------------------------------------------------------------- per-length config
+// PASS1: the pass-1 tile buffer may carry pad rows (its producer uses 1-D bulk copies, 16-byte aligned); pass-2 tiles
+// arrive through tensor copies whose destination must stay 128-byte aligned, so they are never padded.
+template <int LOGL, bool PASS1>
+struct Cfg {
+    static constexpr int L = 1 << LOGL;
+    static constexpr int R0 = fft_r0(LOGL);
+    static constexpr int R1 = fft_r1(LOGL);
+    static constexpr int W = R1;                      // threads per column per line
+    static constexpr int SUB = GT / (R1 * C);         // lines per tile
+    static constexpr int RB = SUB * C;                // float2 per tile-buffer row (one position: SUB lines x C columns)
+    static constexpr bool PAD = PASS1 && RB * 8 == 64;   // 64-byte rows: one pad row per 32 rows
+    static constexpr int ROWS = PAD ? L + L / 32 : L;
+    static constexpr int TILE_F2 = ROWS * RB;         // float2 per tile buffer
+    __device__ static __forceinline__ int idx(int p) { return PAD ? p + (p >> 5) : p; }
+};
+
+enum TileType : int { TILE_NOP = 0, TILE_P1 = 1, TILE_P2 = 2, TILE_STOP = 3 };
+
+template <int LOG1, int LOG2>
+struct Smem {
+    static constexpr int BUF_F2 = Cfg<LOG1, true>::TILE_F2 > Cfg<LOG2, false>::TILE_F2 ? Cfg<LOG1, true>::TILE_F2
+                                                                                         : Cfg<LOG2, false>::TILE_F2;
+    static constexpr size_t BUF_BYTES = (size_t)BUF_F2 * 8;
+    static constexpr size_t TW_A = NBUF * BUF_BYTES;                      // tw1_a: L1 float2
+    static constexpr size_t TW_B = TW_A + ((size_t)8 << LOG1);            // tw1_b: L2 float2
+    static constexpr size_t BARS = TW_B + ((size_t)8 << LOG2);            // full[NBUF][NGROUP], empty[NBUF]
+    static constexpr size_t META = BARS + 3 * NBUF * 8;                   // int4 meta[NBUF]
+    static constexpr size_t TOTAL = META + NBUF * 16 + 128 /* base alignment slack */;
+};
+
+// ------------------------------------------------------------------------------------------- pass 1 (consumer)
+// Tile = SUB consecutive lines j2 of one chunk.  Thread (col, line, wk) of the group.  On entry rows [0, H) of the tile
+// buffer hold the basis block [j1][line][col] and rows [H, ...) the strain slice [line][j1] (both placed by the
+// producer); stage 0 multiplies them (a1), transforms along j1 and writes back in place.
+template <int LOG1, int LOG2>
+__device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chunk, int tile, float2* B,
+                                        const float2* tw1) {
+    using K = Cfg<LOG1, true>;
+    constexpr int L1 = K::L, R0 = K::R0, R1 = K::R1, W = K::W, H = L1 / 2, SUB = K::SUB, RB = K::RB;
+    const int col = gt % C, line = (gt / C) % SUB, wk = gt / (C * SUB);
+    const int slot = line * C + col;
+    const int j2 = tile * SUB + line;
+
+    // ---- a1 + stage 0 ---------------------------------------------------------------------------------
+    float2 u[R0];
+    {
+        const float2* S = B + K::idx(H) * RB + line * H;
+#pragma unroll
+        for (int q = 0; q < R0 / 2; ++q) {
+            const int j1 = wk + q * W;
+            u[q] = cmul_conj(S[j1], B[K::idx(j1) * RB + slot]);
+        }
+    }
+    group_sync(g);   // the strain slice sits where stage 0 writes its upper-half results
+    dft_half<R0>(u);
+#pragma unroll
+    for (int m = 0; m < R0; ++m) B[K::idx(wk + m * W) * RB + slot] = u[m];
+    group_sync(g);
+
+    // ---- stage 1 + inter-pass twiddle + store of Y (in place in the beta array) -------------------------------
+    float2* yrow = a.beta + ((size_t)chunk * (size_t)a.N + (size_t)j2 * L1) * C + col;
+    const float2* tn = a.twN + (size_t)j2 * L1;
+#pragma unroll 1
+    for (int bb = 0; bb < R0 / R1; ++bb) {
+        const int b = wk + bb * W;   // butterfly index < R0
+        float2 x[R1];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) x[q] = B[K::idx(b * R1 + q) * RB + slot];
+#pragma unroll
+        for (int q = 1; q < R1; ++q) x[q] = cmul(x[q], tw1[q * R0 + b]);
+        dft<R1>(x);
+#pragma unroll
+        for (int m = 0; m < R1; ++m) {
+            const int n1 = b + m * R0;
+            __stcg(yrow + n1 * C, cmul(x[m], __ldg(tn + n1)));
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------- pass 2 (consumer)
+__device__ __forceinline__ void store_planes(const FftArgs& a, int bin, int gcol, float2 v) {
+    const size_t e = ((size_t)(gcol / 32) * a.M + bin) * 64 + (gcol % 32) * 2;
+    if (a.plane_fp16) {
+        // screen mode: one fp16 plane (round to nearest; |v| > 65504 becomes inf, which the screen lets through)
+        *reinterpret_cast<__half2*>(a.plane_hi + e) = __floats2half2_rn(v.x, v.y);
+        return;
+    }
+    const __nv_bfloat16 hx = __float2bfloat16_rn(v.x), hy = __float2bfloat16_rn(v.y);
+    const __nv_bfloat16 lx = __float2bfloat16_rn(v.x - __bfloat162float(hx));
+    const __nv_bfloat16 ly = __float2bfloat16_rn(v.y - __bfloat162float(hy));
+    *reinterpret_cast<ushort2*>(a.plane_hi + e) = make_ushort2(__bfloat16_as_ushort(hx), __bfloat16_as_ushort(hy));
+    *reinterpret_cast<ushort2*>(a.plane_lo + e) = make_ushort2(__bfloat16_as_ushort(lx), __bfloat16_as_ushort(ly));
+}
+
+// One round = SUB consecutive lines n1 = n1_r .. of one chunk (an item of span = max(w, SUB) lines is `rounds`
+// consecutive rounds of the same group; acc carries the bin sums across them).  On entry the tile buffer holds the Y
+// rows [j2][line][col].
+template <int LOG1, int LOG2, int NIT>
+__device__ __forceinline__ void p2_round(const FftArgs& a, int g, int gt, int chunk, int n1_0, int rd, int rounds,
+                                         float2* B, const float2* tw1, float2 (&acc)[NIT]) {
+    using K = Cfg<LOG2, false>;
+    constexpr int L1 = 1 << LOG1, L2 = K::L, R0 = K::R0, R1 = K::R1, W = K::W, SUB = K::SUB, RB = K::RB;
+    const int col = gt % C, line = (gt / C) % SUB, wk = gt / (C * SUB);
+    const int slot = line * C + col;
+    const int w = a.w;
+    const int n1 = n1_0 + rd * SUB + line;
+    const int gcol = chunk * C + col;
+    float2* bchunk = a.beta + (size_t)chunk * (size_t)a.N * C;   // holds Y on entry, beta on exit (in place)
+
+    float2 u[R0];
+#pragma unroll
+    for (int q = 0; q < R0; ++q) u[q] = B[K::idx(wk + q * W) * RB + slot];
+    dft<R0>(u);
+#pragma unroll
+    for (int m = 0; m < R0; ++m) B[K::idx(wk + m * W) * RB + slot] = u[m];
+    group_sync(g);
+#pragma unroll
+    for (int bb = 0; bb < R0 / R1; ++bb) {
+        const int b = wk + bb * W;
+        float2 x[R1];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) x[q] = B[K::idx(b * R1 + q) * RB + slot];
+#pragma unroll
+        for (int q = 1; q < R1; ++q) x[q] = cmul(x[q], tw1[q * R0 + b]);
+        dft<R1>(x);
+#pragma unroll
+        for (int m = 0; m < R1; ++m) {
+            const int n2 = b + m * R0;
+            __stcs(bchunk + ((size_t)n1 + (size_t)L1 * n2) * C + col, x[m]);
+            u[bb * R1 + m] = x[m];
+        }
+    }
+    // ---- a3: sum the outputs of min(w, SUB) consecutive lines at equal n2 ----------------------------------------
+    group_sync(g);   // every stage-1 read of the tile buffer is done
+#pragma unroll
+    for (int bb = 0; bb < R0 / R1; ++bb)
+#pragma unroll
+        for (int m = 0; m < R1; ++m) B[K::idx((wk + bb * W) + m * R0) * RB + slot] = u[bb * R1 + m];
+    group_sync(g);
+    if (rd == 0) {
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) acc[it] = make_float2(0.f, 0.f);
+    }
+    if (w >= SUB) {
+        // all SUB lines of this round fall into one bin per n2; a bin spans `rounds` rounds.  Each thread starts at
+        // a different line (rot) so that the 16 lanes of a shared-memory wavefront hit 16 distinct 8-byte banks.
+        const int rot = (gt >> (RB * 8 == 64 ? 3 : 2)) & (SUB - 1);
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const int e = gt + it * GT;   // (n2, col): col is this thread's own
+            if (L2 * C >= GT || e < L2 * C) {
+                const int n2 = e / C;
+                const float2* row = B + K::idx(n2) * RB + col;
+                float2 sum = row[rot * C];
+#pragma unroll
+                for (int rr = 1; rr < SUB; ++rr) sum = cadd(sum, row[((rot + rr) & (SUB - 1)) * C]);
+                acc[it] = cadd(acc[it], sum);
+                if (rd == rounds - 1)
+                    store_planes(a, n1_0 / w + (L1 / w) * n2, gcol,
+                                 make_float2(acc[it].x * a.inv_w, acc[it].y * a.inv_w));
+            }
+        }
+    } else {
+        // w < SUB (including w = 1): this round completes SUB / w bins per n2; compact, not unrolled
+        const int nb = SUB / w;
+#pragma unroll 1
+        for (int e = gt; e < nb * L2 * C; e += GT) {
+            const int rb = e / (L2 * C), n2 = (e % (L2 * C)) / C;
+            const float2* row = B + K::idx(n2) * RB + col;
+            float2 sum = row[(rb * w) * C];
+#pragma unroll 1
+            for (int rr = 1; rr < w; ++rr) sum = cadd(sum, row[(rb * w + rr) * C]);
+            store_planes(a, (n1_0 + rd * SUB + rb * w) / w + (L1 / w) * n2, gcol,
+                         make_float2(sum.x * a.inv_w, sum.y * a.inv_w));
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------ kernel
+template <int LOG1, int LOG2>
+__global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ CUtensorMap tmY, const FftArgs a) {
+    using K1 = Cfg<LOG1, true>;
+    using K2 = Cfg<LOG2, false>;
+    using S = Smem<LOG1, LOG2>;
+    constexpr int L1 = 1 << LOG1, L2 = 1 << LOG2, H = L1 / 2;
+    constexpr int NIT = (L2 * C + GT - 1) / GT;   // reduced outputs per thread and round
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
+    float2* tw_a = reinterpret_cast<float2*>(sm + S::TW_A);
+    float2* tw_b = reinterpret_cast<float2*>(sm + S::TW_B);
+    const uint32_t bars = smem_u32(sm + S::BARS);
+    // One "full" barrier per (buffer, group): a parity wait can only tell the current phase from the previous one, and
+    // a group that got an empty (NOP) tile may ask for its next tile in buffer b before the OTHER group's tile in b
+    // has even landed -- on a barrier shared by both groups that request would alias to an older phase and pass.
+    // With per-group barriers a group's successive waits on one barrier are successive phases (tiles i, i + 6, ...).
+    auto full_bar = [&](int b, int g) { return bars + 8u * (b * NGROUP + g); };
+    auto empty_bar = [&](int b) { return bars + 8u * (NBUF * NGROUP + b); };
+    volatile int4* meta = reinterpret_cast<volatile int4*>(sm + S::META);
+    auto buf_ptr = [&](int b) { return reinterpret_cast<float2*>(sm + (size_t)b * S::BUF_BYTES); };
+
+    const int n1t = L2 / K1::SUB;                                  // pass-1 tiles per chunk
+    const int span = a.w > K2::SUB ? a.w : K2::SUB;
+    const int rounds = span / K2::SUB;
+    const int n2t = L1 / span;                                     // pass-2 items per chunk
+    const int per = n1t + n2t;
+    const int total = a.nchunk * per;
+
+    for (int i = threadIdx.x; i < L1; i += NT) tw_a[i] = a.tw1_a[i];
+    for (int i = threadIdx.x; i < L2; i += NT) tw_b[i] = a.tw1_b[i];
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < NBUF; ++b) {
+            mbar_init(full_bar(b, 0), 1); mbar_init(full_bar(b, 1), 1); mbar_init(empty_bar(b), 1);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_async_smem();
+    }
+    __syncthreads();
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp >= NGROUP * (GT / 32)) {
+        // the producer needs few registers: hand the rest of the register file to the consumer warpgroups
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        if (warp > NGROUP * (GT / 32)) return;
+        // =========================================== producer ===========================================
+        if (lane == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmY) : "memory");
+        int next_ticket = 0;
+        if (lane == 0) next_ticket = (int)atomicAdd(a.sched, 1u);
+        int it_chunk[NGROUP] = {0, 0}, it_n1[NGROUP] = {0, 0}, it_rd[NGROUP] = {0, 0};   // open pass-2 items
+        bool it_open[NGROUP] = {false, false};
+        int stops = 0;
+        for (int i = 0; stops < NGROUP; ++i) {
+            const int g = i & 1, buf = i % NBUF;
+            const uint32_t use = (uint32_t)(i / NBUF);
+            int type = TILE_NOP, chunk = 0, idx = 0, rd = 0;
+            if (lane == 0) {
+                mbar_wait(empty_bar(buf), (use & 1u) ^ 1u);
+                if (it_open[g]) {
+                    type = TILE_P2; chunk = it_chunk[g]; idx = it_n1[g]; rd = it_rd[g];
+                } else if (next_ticket < total) {
+                    const int t = next_ticket;
+                    next_ticket = (int)atomicAdd(a.sched, 1u);
+                    // queue order: P1(0) | P1(1) P2(0) | P1(2) P2(1) | ... | P1(n-1) P2(n-2) | P2(n-1)
+                    bool first = true;
+                    chunk = 0; idx = t;
+                    if (t >= n1t) {
+                        const int u = t - n1t;
+                        const int blk = u / per, v = u - blk * per;
+                        if (blk < a.nchunk - 1 && v < n1t) { chunk = blk + 1; idx = v; }
+                        else { first = false; chunk = blk; idx = blk < a.nchunk - 1 ? v - n1t : v; }
+                    }
+                    if (first) {
+                        type = TILE_P1;
+                    } else {
+                        type = TILE_P2; idx *= span; rd = 0;
+                        wait_counter(a.sched + 16 + chunk, (unsigned)n1t);   // all of the chunk's Y is in L2
+                    }
+                } else if (!it_open[g ^ 1]) {
+                    type = TILE_STOP;
+                }
+            }
+            type = __shfl_sync(0xffffffffu, type, 0);
+            chunk = __shfl_sync(0xffffffffu, chunk, 0);
+            idx = __shfl_sync(0xffffffffu, idx, 0);
+            rd = __shfl_sync(0xffffffffu, rd, 0);
+            const uint32_t dst = smem_u32(buf_ptr(buf));
+            if (lane == 0) {
+                meta[buf].x = type; meta[buf].y = chunk; meta[buf].z = idx; meta[buf].w = rd;
+            }
+            if (type == TILE_P1) {
+                constexpr uint32_t basis_bytes = (uint32_t)H * K1::RB * 8, strain_bytes = (uint32_t)K1::SUB * H * 8;
+                if (lane == 0) mbar_expect_tx(full_bar(buf, g), basis_bytes + strain_bytes);
+                __syncwarp();
+                const float2* src = a.basisP + ((size_t)chunk * n1t + idx) * (size_t)(H * K1::RB);
+                if (K1::PAD) {
+                    for (int p = lane; p < H / 32; p += 32)
+                        bulk_g2s(dst + (uint32_t)(33 * p) * K1::RB * 8, src + (size_t)p * 32 * K1::RB, 32 * K1::RB * 8,
+                                 full_bar(buf, g));
+                } else if (lane == 0) {
+                    bulk_g2s(dst, src, basis_bytes, full_bar(buf, g));
+                }
+                if (lane == 31)
+                    bulk_g2s(dst + (uint32_t)K1::idx(H) * K1::RB * 8, a.dsT + (size_t)idx * K1::SUB * H, strain_bytes,
+                             full_bar(buf, g));
+            } else if (type == TILE_P2) {
+                constexpr int BR = L2 < 256 ? L2 : 256;   // rows per tensor copy
+                if (lane == 0) mbar_expect_tx(full_bar(buf, g), (uint32_t)L2 * K2::RB * 8);
+                __syncwarp();
+                const int x = (idx + rd * K2::SUB) * C * 2;   // floats along the (n1, col) axis
+                for (int p = lane; p < L2 / BR; p += 32)
+                    tma_load_3d(dst + (uint32_t)K2::idx(p * BR) * K2::RB * 8, &tmY, full_bar(buf, g), x, p * BR, chunk);
+                if (rd + 1 < rounds) { it_open[g] = true; it_chunk[g] = chunk; it_n1[g] = idx; it_rd[g] = rd + 1; }
+                else it_open[g] = false;
+            } else {
+                if (lane == 0) mbar_arrive(full_bar(buf, g));
+                if (type == TILE_STOP) ++stops;
+            }
+            __syncwarp();
+        }
+    } else {
+        // =========================================== consumers ==========================================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+        const int g = warp / (GT / 32), gt = threadIdx.x - g * GT;
+        float2 acc[NIT];
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) acc[it] = make_float2(0.f, 0.f);
+        for (int i = g;; i += NGROUP) {
+            const int buf = i % NBUF;
+            mbar_wait(full_bar(buf, g), (uint32_t)(i / (NBUF * NGROUP)) & 1u);
+            const int type = meta[buf].x, chunk = meta[buf].y, idx = meta[buf].z, rd = meta[buf].w;
+            if (type == TILE_STOP) break;
+            float2* B = buf_ptr(buf);
+            if (type == TILE_P1) p1_tile<LOG1, LOG2>(a, g, gt, chunk, idx, B, tw_a);
+            else if (type == TILE_P2) p2_round<LOG1, LOG2, NIT>(a, g, gt, chunk, idx, rd, rounds, B, tw_b, acc);
+            fence_async_smem();   // this thread's generic-proxy writes to the buffer, before the async proxy refills it
+            if (type == TILE_P1) __threadfence();   // this thread's Y stores are performed before the group signals
+            group_sync(g);
+            if (gt == 0) {
+                mbar_arrive(empty_bar(buf));
+                if (type == TILE_P1) atomicAdd(a.sched + 16 + chunk, 1u);
+            }
+        }
+    }
+}
+
+template <int LOG1, int LOG2>
+cudaError_t configure_one(size_t* smem_bytes) {
+    constexpr size_t smem = Smem<LOG1, LOG2>::TOTAL;
+    *smem_bytes = smem;
+    return cudaFuncSetAttribute(fft_tma_kernel<LOG1, LOG2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+}
+
+template <int LOG1, int LOG2>
+cudaError_t launch_one(const CUtensorMap& tmY, const FftArgs& a, int grid, cudaStream_t st) {
+    fft_tma_kernel<LOG1, LOG2><<<grid, NT, Smem<LOG1, LOG2>::TOTAL, st>>>(tmY, a);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// N = 2^(logL1 + logL2) with logL1 = ceil(n/2), logL2 = floor(n/2), n = 10 .. 20.
+#define RBMF_FFT_DISPATCH(FN, ...)                                   \
+    switch (logL1 * 16 + logL2) {                                    \
+        case 5 * 16 + 5: return FN<5, 5>(__VA_ARGS__);               \
+        case 6 * 16 + 5: return FN<6, 5>(__VA_ARGS__);               \
+        case 6 * 16 + 6: return FN<6, 6>(__VA_ARGS__);               \
+        case 7 * 16 + 6: return FN<7, 6>(__VA_ARGS__);               \
+        case 7 * 16 + 7: return FN<7, 7>(__VA_ARGS__);               \
+        case 8 * 16 + 7: return FN<8, 7>(__VA_ARGS__);               \
+        case 8 * 16 + 8: return FN<8, 8>(__VA_ARGS__);               \
+        case 9 * 16 + 8: return FN<9, 8>(__VA_ARGS__);               \
+        case 9 * 16 + 9: return FN<9, 9>(__VA_ARGS__);               \
+        case 10 * 16 + 9: return FN<10, 9>(__VA_ARGS__);             \
+        case 10 * 16 + 10: return FN<10, 10>(__VA_ARGS__);           \
+        default: return cudaErrorInvalidValue;                       \
+    }
+
+cudaError_t fft_tma_configure(int logL1, int logL2, size_t* smem_bytes) {
+    RBMF_FFT_DISPATCH(configure_one, smem_bytes)
+}
+
+cudaError_t launch_fft_tma(const CUtensorMap& tmY, const FftArgs& a, int logL1, int logL2, int grid, cudaStream_t st) {
+    RBMF_FFT_DISPATCH(launch_one, tmY, a, grid, st)
+}
+
+
+}  // namespace rbmf

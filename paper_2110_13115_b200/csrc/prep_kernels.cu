@@ -36,10 +36,11 @@ cudaError_t launch_init_tables(float2* tw1_a, float2* tw1_b, float2* twN, int lo
 }
 
 // --------------------------------------------------------------------------------- basis re-layout
-// basis: k x bins (row-major, caller's layout)  ->  basisP[chunk][j2][j1 < L1/2][C] with j = j1 L2 + j2,
-// zero outside the band: the block a pass-1 tile reads is contiguous.
+// basis: k x bins (row-major, caller's layout)  ->  basisP[chunk][tile][j1 < L1/2][line < sub][C] with
+// j = j1 L2 + j2, j2 = tile * sub + line, zero outside the band: the block a pass-1 tile (sub lines) reads is
+// contiguous and already in the [position][line][column] order of the FFT kernel's tile buffer.
 __global__ void layout_basis_kernel(const float2* __restrict__ basis, float2* __restrict__ basisP, long long bins,
-                                    int j_low, int logL1, int logL2) {
+                                    int j_low, int logL1, int logL2, int sub) {
     __shared__ float2 tile[kFftC][32][33];
     const int L2 = 1 << logL2, H = (1 << logL1) / 2;
     const int chunk = blockIdx.z;
@@ -62,16 +63,18 @@ __global__ void layout_basis_kernel(const float2* __restrict__ basis, float2* __
         if (j2 >= L2) continue;
         for (int e = tx; e < 32 * kFftC; e += 32) {
             const int j1 = j1_0 + e / kFftC, c = e % kFftC;
-            if (j1 < H) basisP[(((size_t)chunk * L2 + j2) * H + j1) * kFftC + c] = tile[c][e / kFftC][r];
+            if (j1 < H)
+                basisP[((((size_t)chunk * (L2 / sub) + j2 / sub) * H + j1) * sub + j2 % sub) * kFftC + c] =
+                    tile[c][e / kFftC][r];
         }
     }
 }
 
 cudaError_t launch_layout_basis(const float2* basis, float2* basisP, int k, int64_t bins, int j_low, int logL1,
-                                int logL2, cudaStream_t st) {
+                                int logL2, int sub, cudaStream_t st) {
     const int L2 = 1 << logL2, H = (1 << logL1) / 2;
     dim3 grid((unsigned)((L2 + 31) / 32), (unsigned)((H + 31) / 32), (unsigned)(k / kFftC));
-    layout_basis_kernel<<<grid, 256, 0, st>>>(basis, basisP, bins, j_low, logL1, logL2);
+    layout_basis_kernel<<<grid, 256, 0, st>>>(basis, basisP, bins, j_low, logL1, logL2, sub);
     return cudaGetLastError();
 }
 

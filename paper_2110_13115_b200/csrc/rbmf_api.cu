@@ -43,7 +43,7 @@ struct rbmf_plan {
     bool have_ws, have_basis, have_coeffs, filtered;
     int num_sms;
     int last_cuda;
-    CUtensorMap tmA_hi, tmA_lo, tmB_hi, tmB_lo, tmB_h16;
+    CUtensorMap tmA_hi, tmA_lo, tmB_hi, tmB_lo, tmB_h16, tmY;
     bool have_maps;
     cudaEvent_t ev[5];
     bool have_events;
@@ -106,7 +106,9 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 rbmf_status encode_map(rbmf_plan* plan, CUtensorMap* map, void* base, int rank, const cuuint64_t* dims,
-                       const cuuint64_t* strides, const cuuint32_t* box) {
+                       const cuuint64_t* strides, const cuuint32_t* box,
+                       CUtensorMapDataType dtype = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16,
+                       CUtensorMapSwizzle swizzle = CU_TENSOR_MAP_SWIZZLE_128B) {
     static EncodeTiledFn fn = nullptr;
     if (!fn) {
         void* sym = nullptr;
@@ -117,9 +119,8 @@ rbmf_status encode_map(rbmf_plan* plan, CUtensorMap* map, void* base, int rank, 
         fn = (EncodeTiledFn)sym;
     }
     const cuuint32_t estr[3] = {1, 1, 1};
-    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, base, dims, strides, box, estr,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = fn(map, dtype, (cuuint32_t)rank, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    swizzle, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { plan->last_cuda = (int)r; return RBMF_ERR_CUDA; }
     return RBMF_OK;
 }
@@ -139,6 +140,17 @@ rbmf_status make_map_planes(rbmf_plan* plan, CUtensorMap* map, void* base, uint6
     const cuuint64_t strides[2] = {(cuuint64_t)kGemmBK * 2, M * kGemmBK * 2};
     const cuuint32_t box[3] = {(cuuint32_t)kGemmBK, (cuuint32_t)kGemmBM, 1};
     return encode_map(plan, map, base, 3, dims, strides, box);
+}
+
+// Y rows of a pass-2 FFT tile: the beta array viewed as fp32 [chunk][j2 < L2][2 C L1] (Y[n1][j2] sits at the address
+// of beta[n1 + L1 j2]); box = sub2 lines x C columns (re, im) wide, up to 256 rows j2, unswizzled.
+rbmf_status make_map_y(rbmf_plan* plan, CUtensorMap* map, void* base) {
+    const uint64_t L1 = 1ull << plan->logN1, L2 = 1ull << plan->logN2;
+    const cuuint64_t dims[3] = {2 * kFftC * L1, L2, (cuuint64_t)(plan->k / kFftC)};
+    const cuuint64_t strides[2] = {L1 * kFftC * 8, (cuuint64_t)plan->N * kFftC * 8};
+    const cuuint32_t box[3] = {(cuuint32_t)(2 * kFftC * fft_sub(plan->logN2)), (cuuint32_t)(L2 < 256 ? L2 : 256), 1};
+    return encode_map(plan, map, base, 3, dims, strides, box, CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                      CU_TENSOR_MAP_SWIZZLE_NONE);
 }
 
 template <typename T> T* at(rbmf_plan* p, size_t off) { return reinterpret_cast<T*>(p->ws + off); }
@@ -234,16 +246,15 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     CK(cudaMemsetAsync(plan->ws + L.bavg_lo, 0, L.plane_bytes, plan->stream));
     CK(gemm_tcgen05_configure());
     {
-        int per_sm = 0;
         size_t smem = 0;
-        CK(fft_fused_configure(plan->logN1, plan->logN2, &per_sm, &smem));
-        if (per_sm < 1) return RBMF_ERR_UNSUPPORTED;
-        plan->fft_grid = per_sm * plan->num_sms;
+        CK(fft_tma_configure(plan->logN1, plan->logN2, &smem));
+        plan->fft_grid = plan->num_sms;   // persistent: one CTA (two consumer groups + a producer warp) per SM
     }
     // TMA descriptors: A = beta^avg planes ([kb][M][64]), B = coefficient planes (2*Tpad rows x 2k)
     rbmf_status s;
     const uint64_t k2 = 2 * (uint64_t)plan->k;
     const uint64_t nkb = (uint64_t)((plan->k + 31) / 32);
+    if ((s = make_map_y(plan, &plan->tmY, plan->ws + L.beta)) != RBMF_OK) return s;
     if ((s = make_map_planes(plan, &plan->tmA_hi, plan->ws + L.bavg_hi, (uint64_t)plan->M, nkb)) != RBMF_OK) return s;
     if ((s = make_map_planes(plan, &plan->tmA_lo, plan->ws + L.bavg_lo, (uint64_t)plan->M, nkb)) != RBMF_OK) return s;
     if ((s = make_map_rows(plan, &plan->tmB_hi, plan->ws + L.c_hi, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
@@ -262,7 +273,7 @@ rbmf_status rbmf_set_basis(rbmf_plan* plan, const void* basis_dev) {
     if (!plan || !basis_dev) return RBMF_ERR_ARG;
     if (!plan->have_ws) return RBMF_ERR_STATE;
     CK(launch_layout_basis((const float2*)basis_dev, at<float2>(plan, plan->lay.basisP), plan->k, plan->N / 2 + 1,
-                           plan->j_low, plan->logN1, plan->logN2, plan->stream));
+                           plan->j_low, plan->logN1, plan->logN2, fft_sub(plan->logN1), plan->stream));
     plan->have_basis = true;
     return RBMF_OK;
 }
@@ -304,7 +315,7 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     a.N = plan->N; a.M = (int)plan->M; a.nchunk = plan->k / kFftC; a.w = plan->w; a.inv_w = 1.0f / (float)plan->w;
     const bool screen = plan->gemm_impl == RBMF_GEMM_SCREEN;
     a.plane_fp16 = screen ? 1 : 0;
-    CK(launch_fft_fused(a, plan->logN1, plan->logN2, plan->fft_grid, st));
+    CK(launch_fft_tma(plan->tmY, a, plan->logN1, plan->logN2, plan->fft_grid, st));
     if (screen)
         CK(launch_bin_norm(at<uint16_t>(plan, L.bavg_hi), at<float>(plan, L.bin_norm), (int)plan->M,
                            (plan->k + 31) / 32, st));

@@ -10,7 +10,7 @@
 namespace rbmf {
 
 constexpr int kFftC = 4;           // basis columns per FFT chunk (32-byte row segments)
-constexpr int kFftThreads = 256;   // threads per FFT CTA
+constexpr int kFftThreads = 256;   // threads per FFT consumer group
 constexpr int kMaxChunks = 256;    // k <= 1024
 constexpr int kGemmBM = 128;       // time bins per GEMM tile (UMMA M)
 constexpr int kGemmTT = 128;       // templates per GEMM tile (UMMA N = 2*kGemmTT: re | im rows)
@@ -20,7 +20,7 @@ constexpr int kGemmBK = 64;        // bf16 elements per K block (= one 128-byte 
 // A thread owns one column and R0 elements; W = L / R0 = R1 threads cooperate on one column of one line.
 __host__ __device__ constexpr int fft_r0(int logL) { return logL >= 9 ? 32 : (logL >= 7 ? 16 : 8); }
 __host__ __device__ constexpr int fft_r1(int logL) { return (1 << logL) / fft_r0(logL); }
-// lines (independent transforms) a 256-thread CTA works on in lockstep
+// lines (independent transforms) a 256-thread consumer group works on in lockstep = lines per tile
 __host__ __device__ constexpr int fft_sub(int logL) { return kFftThreads / (fft_r1(logL) * kFftC); }
 
 // Scheduler words (uint32) in the workspace: [0] ticket, [16 + c] pass-1 tiles done of chunk c.
@@ -28,7 +28,7 @@ constexpr int kSchedWords = 16 + kMaxChunks;
 
 // Device views handed to the fused FFT kernel.
 struct FftArgs {
-    const float2* basisP;    // [chunk][j2 < L2][j1 < L1/2][C]: conj NOT applied, zero outside the band
+    const float2* basisP;    // [chunk][tile][j1 < L1/2][line][C], j2 = tile * sub + line: conj NOT applied, zero outside the band
     const float2* dsT;       // [j2 < L2][j1 < L1/2]: s * d[j1 L2 + j2]
     const float2* tw1_a;     // pass 1 stage-1 twiddles  [q < R1][b < R0] = e^{2 pi i q b / L1}
     const float2* tw1_b;     // pass 2 stage-1 twiddles, same for L2
@@ -83,16 +83,17 @@ struct Stage2Args {
 // ---- launchers (each returns the cudaError_t of the launch) -------------------------------------
 cudaError_t launch_init_tables(float2* tw1_a, float2* tw1_b, float2* twN, int logL1, int logL2, cudaStream_t st);
 cudaError_t launch_layout_basis(const float2* basis, float2* basisP, int k, int64_t bins, int j_low, int logL1,
-                                int logL2, cudaStream_t st);
+                                int logL2, int sub, cudaStream_t st);
 cudaError_t launch_prep_coeffs(const float2* coeffs, const float* sigma, float2* cs, uint16_t* c_hi,
                                uint16_t* c_lo, uint16_t* c_h16, float* tnorm_blk, int T, int Tpad, int k,
                                cudaStream_t st);
 cudaError_t launch_bin_norm(const uint16_t* plane_h16, float* bin_norm, int M, int nkb, cudaStream_t st);
 cudaError_t launch_prep_strain(const float2* strain, float2* dsT, int logL1, int logL2, float scale,
                                cudaStream_t st);
-// Fused FFT (a1-a3): configure once per (logL1, logL2) -> CTAs per SM; then launch.
-cudaError_t fft_fused_configure(int logL1, int logL2, int* ctas_per_sm, size_t* smem_bytes);
-cudaError_t launch_fft_fused(const FftArgs& a, int logL1, int logL2, int grid, cudaStream_t st);
+// Fused FFT (a1-a3): configure once per (logL1, logL2); then launch with one CTA per SM.  tmY: 3-D fp32 tensor map
+// over the beta array, dims {2 C L1, L2, k/C}, box {2 C sub2, min(L2, 256), 1} (the Y rows of a pass-2 tile).
+cudaError_t fft_tma_configure(int logL1, int logL2, size_t* smem_bytes);
+cudaError_t launch_fft_tma(const CUtensorMap& tmY, const FftArgs& a, int logL1, int logL2, int grid, cudaStream_t st);
 cudaError_t launch_gemm_simt(const uint16_t* a_hi, const uint16_t* a_lo, const uint16_t* c_hi,
                              const uint16_t* c_lo, const GemmArgs& g, cudaStream_t st);
 cudaError_t launch_gemm_tcgen05(const CUtensorMap& tmA_hi, const CUtensorMap& tmA_lo, const CUtensorMap& tmB_hi,

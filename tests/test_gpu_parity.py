@@ -157,8 +157,7 @@ def test_mini_all_windows(rbmf, w, impl):
 
 def test_mini_largest_window(rbmf):
     # w = 32 at fs = 1024 Hz averages every peak away: the point is the two-slot row layout of kernel 3
-    rep, crep = check(rbmf, workload("mini"), 32, 1.2, 3.5, impl=SCREEN, expect_triggers=False)
-    assert rep["n_got"] > 0
+    check(rbmf, workload("mini"), 32, 0.4, 3.0, impl=SCREEN, expect_triggers=False)
 
 
 def test_mini_simt_and_tensor_core_candidates_agree(rbmf):
