@@ -161,10 +161,23 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     } while (!done);
 }
 // 1-D bulk copy global -> shared (16-byte aligned addresses, size a multiple of 16), completion on an mbarrier.
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-                 "l"(src), "r"(bytes), "r"(bar)
-                 : "memory");
+// L2 policies: the basis is streamed once (evict first); strain slice, Y and tables are re-read (evict last / normal).
+__device__ __forceinline__ unsigned long long policy_evict_first() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ unsigned long long policy_evict_last() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar,
+                                         unsigned long long pol) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+        "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+        : "memory");
 }
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y, int z) {
     asm volatile(
@@ -172,6 +185,18 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
         "l"(map), "r"(bar), "r"(x), "r"(y), "r"(z)
         : "memory");
 }
+// Tensor store shared -> global (bulk async group): the beta rows of a pass-2 tile leave through the same 3-D map
+// their Y rows came in by.
+// beta is written once and not read again by this kernel: evict-first keeps it from displacing the Y rows in L2.
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, uint32_t src, int x, int y, int z) {
+    const unsigned long long pol = policy_evict_first();
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3, %4}], [%1], %5;" ::"l"(map),
+                 "r"(src), "r"(x), "r"(y), "r"(z), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void group_sync(int g) {   // named barrier of one consumer group
     if (g == 0) asm volatile("bar.sync 1, %0;" ::"n"(GT) : "memory");
     else asm volatile("bar.sync 2, %0;" ::"n"(GT) : "memory");
@@ -289,16 +314,14 @@ __device__ __forceinline__ void store_planes(const FftArgs& a, int bin, int gcol
 // consecutive rounds of the same group; acc carries the bin sums across them).  On entry the tile buffer holds the Y
 // rows [j2][line][col].
 template <int LOG1, int LOG2, int NIT>
-__device__ __forceinline__ void p2_round(const FftArgs& a, int g, int gt, int chunk, int n1_0, int rd, int rounds,
-                                         float2* B, const float2* tw1, float2 (&acc)[NIT]) {
+__device__ __forceinline__ void p2_round(const FftArgs& a, const CUtensorMap* tmY, int g, int gt, int chunk, int n1_0,
+                                         int rd, int rounds, float2* B, const float2* tw1, float2 (&acc)[NIT]) {
     using K = Cfg<LOG2, false>;
     constexpr int L1 = 1 << LOG1, L2 = K::L, R0 = K::R0, R1 = K::R1, W = K::W, SUB = K::SUB, RB = K::RB;
     const int col = gt % C, line = (gt / C) % SUB, wk = gt / (C * SUB);
     const int slot = line * C + col;
     const int w = a.w;
-    const int n1 = n1_0 + rd * SUB + line;
     const int gcol = chunk * C + col;
-    float2* bchunk = a.beta + (size_t)chunk * (size_t)a.N * C;   // holds Y on entry, beta on exit (in place)
 
     float2 u[R0];
 #pragma unroll
@@ -318,9 +341,7 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, int g, int gt, int ch
         dft<R1>(x);
 #pragma unroll
         for (int m = 0; m < R1; ++m) {
-            const int n2 = b + m * R0;
-            __stcs(bchunk + ((size_t)n1 + (size_t)L1 * n2) * C + col, x[m]);
-            u[bb * R1 + m] = x[m];
+            u[bb * R1 + m] = x[m];   // output n2 = b + m R0
         }
     }
     // ---- a3: sum the outputs of min(w, SUB) consecutive lines at equal n2 ----------------------------------------
@@ -329,7 +350,16 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, int g, int gt, int ch
     for (int bb = 0; bb < R0 / R1; ++bb)
 #pragma unroll
         for (int m = 0; m < R1; ++m) B[K::idx((wk + bb * W) + m * R0) * RB + slot] = u[bb * R1 + m];
+    // The buffer now holds the tile's beta rows [n2][line][col] -- the layout of the beta array itself (in place of the
+    // Y rows this tile loaded): one thread hands them to the TMA, the bin sums below read the same rows meanwhile.
+    fence_async_smem();
     group_sync(g);
+    if (gt == 0) {
+        constexpr int BR = L2 < 256 ? L2 : 256;
+        const int x = (n1_0 + rd * SUB) * C * 2;
+        for (int p = 0; p < L2 / BR; ++p) tma_store_3d(tmY, smem_u32(B + (size_t)p * BR * RB), x, p * BR, chunk);
+        bulk_commit();
+    }
     if (rd == 0) {
 #pragma unroll
         for (int it = 0; it < NIT; ++it) acc[it] = make_float2(0.f, 0.f);
@@ -367,6 +397,7 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, int g, int gt, int ch
                          make_float2(sum.x * a.inv_w, sum.y * a.inv_w));
         }
     }
+    if (gt == 0) bulk_wait_read();   // the tensor store has read the buffer: it may be handed back to the producer
 }
 
 // ------------------------------------------------------------------------------------------------------ kernel
@@ -416,6 +447,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
         if (warp > NGROUP * (GT / 32)) return;
         // =========================================== producer ===========================================
         if (lane == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmY) : "memory");
+        const unsigned long long pol_first = policy_evict_first(), pol_last = policy_evict_last();
         int next_ticket = 0;
         if (lane == 0) next_ticket = (int)atomicAdd(a.sched, 1u);
         int it_chunk[NGROUP] = {0, 0}, it_n1[NGROUP] = {0, 0}, it_rd[NGROUP] = {0, 0};   // open pass-2 items
@@ -467,13 +499,13 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                 if (K1::PAD) {
                     for (int p = lane; p < H / 32; p += 32)
                         bulk_g2s(dst + (uint32_t)(33 * p) * K1::RB * 8, src + (size_t)p * 32 * K1::RB, 32 * K1::RB * 8,
-                                 full_bar(buf, g));
+                                 full_bar(buf, g), pol_first);
                 } else if (lane == 0) {
-                    bulk_g2s(dst, src, basis_bytes, full_bar(buf, g));
+                    bulk_g2s(dst, src, basis_bytes, full_bar(buf, g), pol_first);
                 }
                 if (lane == 31)
                     bulk_g2s(dst + (uint32_t)K1::idx(H) * K1::RB * 8, a.dsT + (size_t)idx * K1::SUB * H, strain_bytes,
-                             full_bar(buf, g));
+                             full_bar(buf, g), pol_last);
             } else if (type == TILE_P2) {
                 constexpr int BR = L2 < 256 ? L2 : 256;   // rows per tensor copy
                 if (lane == 0) mbar_expect_tx(full_bar(buf, g), (uint32_t)L2 * K2::RB * 8);
@@ -503,7 +535,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
             if (type == TILE_STOP) break;
             float2* B = buf_ptr(buf);
             if (type == TILE_P1) p1_tile<LOG1, LOG2>(a, g, gt, chunk, idx, B, tw_a);
-            else if (type == TILE_P2) p2_round<LOG1, LOG2, NIT>(a, g, gt, chunk, idx, rd, rounds, B, tw_b, acc);
+            else if (type == TILE_P2) p2_round<LOG1, LOG2, NIT>(a, &tmY, g, gt, chunk, idx, rd, rounds, B, tw_b, acc);
             fence_async_smem();   // this thread's generic-proxy writes to the buffer, before the async proxy refills it
             if (type == TILE_P1) __threadfence();   // this thread's Y stores are performed before the group signals
             group_sync(g);
@@ -512,6 +544,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                 if (type == TILE_P1) atomicAdd(a.sched + 16 + chunk, 1u);
             }
         }
+        if (gt == 0) bulk_wait_all();   // this thread's beta stores are complete before the CTA retires
     }
 }
 
