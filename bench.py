@@ -28,6 +28,11 @@ import numpy as np  # noqa: E402
 METRIC = "template_seconds_filtered_per_second"
 UNIT = "template-seconds/s"
 
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the `ncu --set full` captures summarised
+# under profiles/ (r01_launches.md); known only for the configuration that was profiled, else reported as null.
+NCU_TRAFFIC = {("paper", 8, "screen", "gemm"): 290.4e6 + 2.0e6, ("paper", 8, "screen", "fft"): 551.6e6 + 1232.5e6,
+               ("paper", 8, "screen", "stage2"): 178.5e6 + 4.4e6}
+
 
 # ------------------------------------------------------------------------------------------------- clocks
 class ClockSampler:
@@ -272,14 +277,16 @@ def main():
     fft_alg_bytes = cfg.k * band * 8 + (cfg.N // 2 + 1) * 8 + cfg.k * cfg.N * 8 + cfg.k * M * 8
     fft_gbs = fft_alg_bytes / (fft_ms * 1e-3) / 1e9
     roofline = {"kernel": "gemm_tcgen05_kernel (a4-a5)", "bound": "tensor", "achieved": gemm_tflops,
-                "peak": tensor_peak, "unit": "TFLOP/s", "frac": gemm_tflops / tensor_peak, "traffic": None,
+                "peak": tensor_peak, "unit": "TFLOP/s", "frac": gemm_tflops / tensor_peak,
+                "traffic": NCU_TRAFFIC.get((args.config, cfg.w, args.gemm, "gemm")),
                 "peak_source": peak_src, "flops_counted": "executed 16-bit MMA flops = %d x 8 T k N/w (%s)" % (
                     int(products), "one fp16 product: rigorous-bound screen, fp32 confirm in kernel 3"
                     if args.gemm == "screen" else "bf16x3 split precision"),
                 "useful_tflops": useful_flops / (gemm_ms * 1e-3) / 1e12, "avg_kernel_ms": gemm_ms}
     stages = {"fft_ms": fft_ms, "gemm_ms": gemm_ms, "stage2_ms": s2_ms, "total_ms": statistics.mean(stage["total"]),
               "fft": {"bound": "hbm", "algorithmic_GBps": fft_gbs, "peak": hbm_peak, "frac": fft_gbs / hbm_peak,
-                      "algorithmic_bytes": fft_alg_bytes},
+                      "algorithmic_bytes": fft_alg_bytes,
+                      "traffic": NCU_TRAFFIC.get((args.config, cfg.w, args.gemm, "fft"))},
               "n_candidates": nc, "n_triggers": nt, "gemm_mode": args.gemm}
     if other_stage is not None:
         stages["other_mode"] = dict(other_stage, gemm_mode=other)
