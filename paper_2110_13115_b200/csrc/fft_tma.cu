@@ -296,6 +296,16 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chu
 }
 
 // ------------------------------------------------------------------------------------------- pass 2 (consumer)
+__device__ __forceinline__ void store_plane_fp16(uint16_t* p, float2 v) {
+    *reinterpret_cast<__half2*>(p) = __floats2half2_rn(v.x, v.y);
+}
+__device__ __forceinline__ void store_planes_bf16(uint16_t* phi, uint16_t* plo, float2 v) {
+    const __nv_bfloat16 hx = __float2bfloat16_rn(v.x), hy = __float2bfloat16_rn(v.y);
+    const __nv_bfloat16 lx = __float2bfloat16_rn(v.x - __bfloat162float(hx));
+    const __nv_bfloat16 ly = __float2bfloat16_rn(v.y - __bfloat162float(hy));
+    *reinterpret_cast<ushort2*>(phi) = make_ushort2(__bfloat16_as_ushort(hx), __bfloat16_as_ushort(hy));
+    *reinterpret_cast<ushort2*>(plo) = make_ushort2(__bfloat16_as_ushort(lx), __bfloat16_as_ushort(ly));
+}
 __device__ __forceinline__ void store_planes(const FftArgs& a, int bin, int gcol, float2 v) {
     const size_t e = ((size_t)(gcol / 32) * a.M + bin) * 64 + (gcol % 32) * 2;
     if (a.plane_fp16) {
@@ -378,9 +388,24 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, const CUtensorMap* tm
 #pragma unroll
                 for (int rr = 1; rr < SUB; ++rr) sum = cadd(sum, row[((rot + rr) & (SUB - 1)) * C]);
                 acc[it] = cadd(acc[it], sum);
-                if (rd == rounds - 1)
-                    store_planes(a, n1_0 / w + (L1 / w) * n2, gcol,
-                                 make_float2(acc[it].x * a.inv_w, acc[it].y * a.inv_w));
+            }
+        }
+        if (rd == rounds - 1) {
+            // bins n1_0 / w + (L1 / w) n2, n2 = gt / C + it GT / C: a constant element stride between iterations
+            const size_t e0 = ((size_t)(gcol / 32) * a.M + n1_0 / w + (size_t)(L1 / w) * (gt / C)) * 64 + (gcol % 32) * 2;
+            const size_t es = (size_t)(L1 / w) * (GT / C) * 64;
+            const float iw = a.inv_w;
+            if (a.plane_fp16) {
+#pragma unroll
+                for (int it = 0; it < NIT; ++it)
+                    if (L2 * C >= GT || gt + it * GT < L2 * C)
+                        store_plane_fp16(a.plane_hi + e0 + it * es, make_float2(acc[it].x * iw, acc[it].y * iw));
+            } else {
+#pragma unroll
+                for (int it = 0; it < NIT; ++it)
+                    if (L2 * C >= GT || gt + it * GT < L2 * C)
+                        store_planes_bf16(a.plane_hi + e0 + it * es, a.plane_lo + e0 + it * es,
+                                          make_float2(acc[it].x * iw, acc[it].y * iw));
             }
         }
     } else {
@@ -409,7 +434,9 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
     constexpr int L1 = 1 << LOG1, L2 = 1 << LOG2, H = L1 / 2;
     constexpr int NIT = (L2 * C + GT - 1) / GT;   // reduced outputs per thread and round
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
+    // 128-byte aligned base, derived by pointer arithmetic so that the compiler keeps the shared address space
+    // (LDS / STS instead of generic loads and stores)
+    uint8_t* sm = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
     float2* tw_a = reinterpret_cast<float2*>(sm + S::TW_A);
     float2* tw_b = reinterpret_cast<float2*>(sm + S::TW_B);
     const uint32_t bars = smem_u32(sm + S::BARS);
