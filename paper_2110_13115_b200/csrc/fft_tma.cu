@@ -564,11 +564,15 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
             if (type == TILE_P1) p1_tile<LOG1, LOG2>(a, g, gt, chunk, idx, B, tw_a);
             else if (type == TILE_P2) p2_round<LOG1, LOG2, NIT>(a, &tmY, g, gt, chunk, idx, rd, rounds, B, tw_b, acc);
             fence_async_smem();   // this thread's generic-proxy writes to the buffer, before the async proxy refills it
-            if (type == TILE_P1) __threadfence();   // this thread's Y stores are performed before the group signals
             group_sync(g);
             if (gt == 0) {
                 mbar_arrive(empty_bar(buf));
-                if (type == TILE_P1) atomicAdd(a.sched + 16 + chunk, 1u);
+                if (type == TILE_P1) {
+                    // release: the group's Y stores happen before this fence through the barrier above (bar.sync
+                    // orders them at CTA scope, the gpu-scope fence is cumulative), then the counter is bumped
+                    __threadfence();
+                    atomicAdd(a.sched + 16 + chunk, 1u);
+                }
             }
         }
         if (gt == 0) bulk_wait_all();   // this thread's beta stores are complete before the CTA retires

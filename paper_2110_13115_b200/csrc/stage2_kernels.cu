@@ -25,16 +25,46 @@ __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
         const float2* __restrict__ crow = a.cs + (size_t)cd.template_id * k;
         const float2* __restrict__ brow = a.beta + (size_t)cd.bin_index * w * kFftC;
         float re0 = 0.f, im0 = 0.f, re1 = 0.f, im1 = 0.f;
-        int par = 0;
-        for (int e = lane; e < total; e += 32, par ^= 1) {
-            const int ch = e / per_chunk, rem = e % per_chunk;
+        // per_chunk = 2w is a power of two: shifts instead of divisions; four items per lane in flight (the loop is
+        // bound by the latency of its two loads, not by their bandwidth)
+        const int lg = 31 - __clz(per_chunk);
+        auto item = [&](int e, float& ar, float& ai) {
+            const int ch = e >> lg, rem = e & (per_chunk - 1);
             const int r = rem >> 1, h = rem & 1;
             const float4 p = __ldg(reinterpret_cast<const float4*>(crow + ch * kFftC + 2 * h));
             const float4 x = __ldg(reinterpret_cast<const float4*>(brow + ch * chunk_stride + r * kFftC + 2 * h));
             float vr = p.x * x.x, vi = p.x * x.y;
             vr = fmaf(-p.y, x.y, vr); vr = fmaf(p.z, x.z, vr); vr = fmaf(-p.w, x.w, vr);
             vi = fmaf(p.y, x.x, vi); vi = fmaf(p.z, x.w, vi); vi = fmaf(p.w, x.z, vi);
-            if (per_chunk > 32 && par) { re1 += vr; im1 += vi; } else { re0 += vr; im0 += vi; }
+            ar += vr; ai += vi;
+        };
+        int e = lane;
+        if (per_chunk > 32) {   // w = 32: consecutive items of a lane alternate between rows r and r + 16
+            for (; e + 96 < total; e += 128) {
+                item(e, re0, im0); item(e + 32, re1, im1); item(e + 64, re0, im0); item(e + 96, re1, im1);
+            }
+            for (int par = 0; e < total; e += 32, par ^= 1) { if (par) item(e, re1, im1); else item(e, re0, im0); }
+        } else {
+            // a lane keeps its (row r, half h) and walks the chunks ch0, ch0 + dch, ...: two pointers, constant strides
+            const int rem = lane & (per_chunk - 1), dch = 32 >> lg, nch = k / kFftC;
+            const float4* pc = reinterpret_cast<const float4*>(crow + (lane >> lg) * kFftC + 2 * (rem & 1));
+            const float4* px = reinterpret_cast<const float4*>(brow + (size_t)(lane >> lg) * chunk_stride +
+                                                               (rem >> 1) * kFftC + 2 * (rem & 1));
+            const size_t sc = (size_t)dch * kFftC / 2, sx = (size_t)dch * chunk_stride / 2;   // float4 strides
+            auto mac = [&](const float4 p, const float4 x, float& ar, float& ai) {
+                ar = fmaf(p.x, x.x, ar); ar = fmaf(-p.y, x.y, ar); ar = fmaf(p.z, x.z, ar); ar = fmaf(-p.w, x.w, ar);
+                ai = fmaf(p.x, x.y, ai); ai = fmaf(p.y, x.x, ai); ai = fmaf(p.z, x.w, ai); ai = fmaf(p.w, x.z, ai);
+            };
+            float r2 = 0.f, i2 = 0.f, r3 = 0.f, i3 = 0.f;
+            int ch = lane >> lg;
+            for (; ch + 3 * dch < nch; ch += 4 * dch, pc += 4 * sc, px += 4 * sx) {
+                const float4 p0 = __ldg(pc), p1 = __ldg(pc + sc), p2 = __ldg(pc + 2 * sc), p3 = __ldg(pc + 3 * sc);
+                const float4 x0 = __ldg(px), x1 = __ldg(px + sx), x2 = __ldg(px + 2 * sx), x3 = __ldg(px + 3 * sx);
+                mac(p0, x0, re0, im0); mac(p1, x1, re1, im1); mac(p2, x2, r2, i2); mac(p3, x3, r3, i3);
+            }
+            for (; ch < nch; ch += dch, pc += sc, px += sx) mac(__ldg(pc), __ldg(px), re0, im0);
+            re0 += re1 + r2 + r3; im0 += im1 + i2 + i3;
+            re1 = 0.f; im1 = 0.f;
         }
         // lanes that share a row differ in bit 0 (half) and in the bits >= log2(2w)
         for (int o = 1; o < 32; o <<= 1) {
