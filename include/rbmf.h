@@ -89,7 +89,9 @@ rbmf_status rbmf_plan_set_window(rbmf_plan* plan, int32_t w);
  * before rbmf_workspace_bytes / rbmf_plan_set_workspace. */
 rbmf_status rbmf_plan_set_capacity(rbmf_plan* plan, int64_t max_candidates, int64_t max_triggers);
 
-/* Select the stage-1 kernel (default RBMF_GEMM_SCREEN).  May be called at any time. */
+/* Select the stage-1 kernel (default RBMF_GEMM_SCREEN).  May be called at any time.
+ * (Diagnostics: with the environment variable RBMF_NO_CLUSTER set when rbmf_plan_set_workspace runs, screen mode uses
+ * its single-CTA kernel instead of the 2-CTA cluster kernel that multicasts the coefficient tile.) */
 rbmf_status rbmf_plan_set_gemm_impl(rbmf_plan* plan, int32_t impl);
 
 /* Bytes of device workspace the plan needs (depends on N, k, T, w, capacities). */

@@ -16,6 +16,16 @@
 // Split precision (bf16x3): every fp32 operand value v is stored as hi = bf16(v), lo = bf16(v - hi); the product is
 // accumulated in fp32 as  A_hi B_hi + A_hi B_lo + A_lo B_hi  (the lo*lo term, ~2^-16 relative, is dropped).
 //
+// Screen mode (MODE 1, RBMF_GEMM_SCREEN, the default).  ONE product with both operands rounded once to fp16, and the
+// threshold of every (time bin i, template block) lowered by a bound of the error this can cause, so that the hit list
+// is a superset of the true candidates; kernel 3 repeats the test in fp32 (see stage2_kernels.cu).  With a = c_t/sigma_t,
+// b = beta^avg[i] (the fp32 values), u = 2^-11 and eta = sqrt(2) 2^-25 (fp16 subnormal range):
+//     |delta a_k| <= u |a_k| + eta,  |delta b_k| <= u |b_k| + eta        (each complex component rounded to nearest)
+//     |R_16 - R| <= (2u + u^2) ||a|| ||b|| + eta sqrt(k) (||a|| + ||b||)                       (Cauchy-Schwarz)
+//                   + (2k + 64) 2^-22 sqrt(2) ||a|| ||b||        (fp32 accumulation of the 2k exact fp16 products)
+// ||b|| comes from bin_norm_kernel (GemmArgs::bin_norm, inflated for the rounding of the plane it reads), ||a|| as the
+// maximum over the tile's 128 templates (GemmArgs::tnorm_blk); kappa1, kappa2, slack are set in rbmf_api.cu.
+//
 // Warp roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + single-thread tcgen05.mma issuer,
 // warps 2-5 = epilogue (one TMEM lane quadrant each).  Two TMEM accumulator buffers (2 x 256 columns) let the epilogue
 // of tile n overlap the main loop of tile n+1.  The kernel is persistent: grid = #SMs, static round-robin over tiles in
@@ -141,6 +151,56 @@ __device__ __forceinline__ void decode_tile(const GemmArgs& g, int tile, int& ib
 }
 
 __device__ __forceinline__ int num_tiles(const GemmArgs& g) { return g.num_tb * g.num_ib; }
+
+// Epilogue of one 128-bin x 128-template tile for one warp (its 32 TMEM lanes = 32 time bins): |R|^2 against the
+// threshold of this bin, warp vote, and -- only where something hit -- a warp-aggregated append to the candidate list.
+__device__ __forceinline__ void epilogue_tile(const GemmArgs& g, uint32_t taddr, int bin, int tb, int lane,
+                                              float thr_sq) {
+#pragma unroll 1
+    for (int ch = 0; ch < kGemmTT / 32; ++ch) {
+        uint32_t re[32], im[32];
+        tmem_ld32(taddr + ch * 32, re);
+        tmem_ld32(taddr + kGemmTT + ch * 32, im);
+        tmem_ld_wait();
+        uint32_t mask = 0;
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
+            mask |= (!(fmaf(x, x, y * y) < thr_sq) ? 1u : 0u) << j;   // NaN (fp16 overflow) passes
+        }
+        if (bin >= g.M) mask = 0;
+        if (__any_sync(0xffffffffu, mask != 0)) {
+            // rare path: warp-aggregated append, one atomic per (warp, template column) with hits
+#pragma unroll 1
+            for (int j = 0; j < 32; ++j) {
+                const bool hit = (mask >> j) & 1u;
+                const unsigned ballot = __ballot_sync(0xffffffffu, hit);
+                if (ballot == 0) continue;
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(g.counters, (unsigned long long)__popc(ballot));
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (hit) {
+                    const unsigned long long idx = base + __popc(ballot & ((1u << lane) - 1u));
+                    const int t = tb * kGemmTT + ch * 32 + j;
+                    if (idx < g.cand_cap && t < g.T) {
+                        rbmf_candidate cd;
+                        cd.template_id = t;
+                        cd.bin_index = bin;
+                        // dynamic register index -> select through a small unrolled search
+                        float x = 0.f, y = 0.f;
+#pragma unroll
+                        for (int jj = 0; jj < 32; ++jj)
+                            if (jj == j) { x = __uint_as_float(re[jj]); y = __uint_as_float(im[jj]); }
+                        cd.avg_re = x;
+                        cd.avg_im = y;
+                        g.cand[idx] = cd;
+                    }
+                }
+            }
+        }
+    }
+}
+
 
 }  // namespace
 
@@ -274,49 +334,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
                 const float te = g.thr1 - (g.kappa1 * nmax * Bn + g.kappa2 * (Bn + nmax) + g.slack);
                 thr_sq = te > 0.f ? te * te : 0.f;
             }
-#pragma unroll 1
-            for (int ch = 0; ch < kGemmTT / 32; ++ch) {
-                uint32_t re[32], im[32];
-                tmem_ld32(taddr + ch * 32, re);
-                tmem_ld32(taddr + kGemmTT + ch * 32, im);
-                tmem_ld_wait();
-                uint32_t mask = 0;
-#pragma unroll
-                for (int j = 0; j < 32; ++j) {
-                    const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
-                    mask |= (!(fmaf(x, x, y * y) < thr_sq) ? 1u : 0u) << j;   // NaN (fp16 overflow) passes
-                }
-                if (bin >= g.M) mask = 0;
-                if (__any_sync(0xffffffffu, mask != 0)) {
-                    // rare path: warp-aggregated append, one atomic per (warp, template column) with hits
-#pragma unroll 1
-                    for (int j = 0; j < 32; ++j) {
-                        const bool hit = (mask >> j) & 1u;
-                        const unsigned ballot = __ballot_sync(0xffffffffu, hit);
-                        if (ballot == 0) continue;
-                        unsigned long long base = 0;
-                        if (lane == 0) base = atomicAdd(g.counters, (unsigned long long)__popc(ballot));
-                        base = __shfl_sync(0xffffffffu, base, 0);
-                        if (hit) {
-                            const unsigned long long idx = base + __popc(ballot & ((1u << lane) - 1u));
-                            const int t = tb * kGemmTT + ch * 32 + j;
-                            if (idx < g.cand_cap && t < g.T) {
-                                rbmf_candidate cd;
-                                cd.template_id = t;
-                                cd.bin_index = bin;
-                                // dynamic register index -> select through a small unrolled search
-                                float x = 0.f, y = 0.f;
-#pragma unroll
-                                for (int jj = 0; jj < 32; ++jj)
-                                    if (jj == j) { x = __uint_as_float(re[jj]); y = __uint_as_float(im[jj]); }
-                                cd.avg_re = x;
-                                cd.avg_im = y;
-                                g.cand[idx] = cd;
-                            }
-                        }
-                    }
-                }
-            }
+            epilogue_tile(g, taddr, bin, tb, lane, thr_sq);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty_bar(buf));
@@ -331,12 +349,203 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// Screen mode on CTA PAIRS (thread-block clusters of 2).  The two CTAs of a cluster work on the two halves of a
+// 256-bin x 128-template super-tile: same coefficient tile (B operand, 32 KB per K block), different beta^avg rows
+// (A operand).  Each CTA fetches only HALF of B and multicasts it into both CTAs' shared memory, so a CTA pulls
+// 16 + 16 KB instead of 16 + 32 KB per K block from L2 -- the single-CTA kernel runs at 15 TB/s of L2 reads, which,
+// not the MMA rate, is what limits it.  A stage may be refilled only when BOTH CTAs' MMAs have drained it: the
+// tcgen05.commit that frees a stage arrives on the "empty" barrier of both CTAs (count 2).
+namespace {
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t cluster_id_x() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t num_clusters_x() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%nclusterid.x;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tma_load_2d_mc(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y,
+                                               uint16_t mask) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster"
+        " [%0], [%1, {%3, %4}], [%2], %5;" ::"r"(dst),
+        "l"(map), "r"(bar), "r"(x), "r"(y), "h"(mask)
+        : "memory");
+}
+__device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t mask) {
+    asm volatile(
+        "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+        "h"(mask)
+        : "memory");
+}
+
+}  // namespace
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
+gemm_screen_pair_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmBh,
+                        const GemmArgs g) {
+    constexpr int STAGES = ModeCfg<1>::STAGES;
+    constexpr uint32_t STAGE_BYTES = ModeCfg<1>::STAGE_BYTES;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+    auto tfull_bar = [&](int b) { return bar_base + 8u * (2 * STAGES + b); };
+    auto tempty_bar = [&](int b) { return bar_base + 8u * (2 * STAGES + 2 + b); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
+    volatile uint32_t* tmem_slot_ptr =
+        reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmBh) : "memory");
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 2); }
+        for (int b = 0; b < 2; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "n"(TMEM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();   // the peer's barriers are initialised before anything is multicast to them
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    // super-tiles: pairs of time-bin blocks; both CTAs of a cluster walk the same sequence (lock step by construction)
+    GemmArgs gp = g;
+    gp.num_ib = (g.num_ib + 1) / 2;
+    const int npairs = gp.num_tb * gp.num_ib;
+    const int num_kb = (g.k2 + BK - 1) / BK;
+    const int first = (int)cluster_id_x(), step = (int)num_clusters_x();
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int pair = first; pair < npairs; pair += step) {
+                int ibp, tb;
+                decode_tile(gp, pair, ibp, tb);
+                const int ib = 2 * ibp + (int)rank;   // may be one past the last block: TMA zero-fills, epilogue masks
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
+                    const uint32_t sbase = smem_base + stage * STAGE_BYTES;
+                    mbar_expect_tx(full_bar(stage), STAGE_BYTES);
+                    tma_load_3d(sbase, &tmA, full_bar(stage), 0, ib * BM, kb);
+                    // my half of the coefficient tile (128 of its 256 rows), into both CTAs
+                    tma_load_2d_mc(sbase + A_BYTES + rank * (B_BYTES / 2), &tmBh, full_bar(stage), kb * BK,
+                                   tb * BN + (int)rank * (BN / 2), (uint16_t)3);
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int it = 0;
+            for (int pair = first; pair < npairs; pair += step, ++it) {
+                const int buf = it & 1;
+                mbar_wait(tempty_bar(buf), ((uint32_t)(it >> 1) & 1u) ^ 1u);
+                tc_fence_after();
+                const uint32_t tmem_d = tmem_base + (uint32_t)(buf * BN);
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    mbar_wait(full_bar(stage), phase);
+                    tc_fence_after();
+                    const uint32_t sbase = smem_base + stage * STAGE_BYTES;
+#pragma unroll
+                    for (int k4 = 0; k4 < BK / UMMA_K; ++k4) {
+                        const uint32_t koff = k4 * UMMA_K * 2;
+                        const uint64_t a_h = make_smem_desc(sbase + koff);
+                        const uint64_t b_h = make_smem_desc(sbase + A_BYTES + koff);
+                        umma_f16<kInstrDescF16>(tmem_d, a_h, b_h, (kb | k4) != 0 ? 1u : 0u);
+                    }
+                    umma_commit_mc(empty_bar(stage), (uint16_t)3);       // frees the slot in BOTH CTAs
+                    if (kb == num_kb - 1) umma_commit(tfull_bar(buf));
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else {
+        const int quad = warp & 3;
+        const int row = quad * 32 + lane;
+        int it = 0;
+        for (int pair = first; pair < npairs; pair += step, ++it) {
+            int ibp, tb;
+            decode_tile(gp, pair, ibp, tb);
+            const int ib = 2 * ibp + (int)rank;
+            const int buf = it & 1;
+            mbar_wait(tfull_bar(buf), (uint32_t)(it >> 1) & 1u);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(buf * BN);
+            const int bin = ib * BM + row;
+            const float Bn = bin < g.M ? __ldg(g.bin_norm + bin) : 0.f;
+            const float nmax = __ldg(g.tnorm_blk + tb);
+            const float te = g.thr1 - (g.kappa1 * nmax * Bn + g.kappa2 * (Bn + nmax) + g.slack);
+            const float thr_sq = te > 0.f ? te * te : 0.f;
+            epilogue_tile(g, taddr, bin, tb, lane, thr_sq);
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar(buf));
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();   // no CTA retires while its peer may still multicast into it or arrive on its barriers
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TMEM_COLS) : "memory");
+    }
+}
+
 cudaError_t gemm_tcgen05_configure() {
     cudaError_t e = cudaFuncSetAttribute(gemm_tcgen05_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)ModeCfg<0>::SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(gemm_tcgen05_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    e = cudaFuncSetAttribute(gemm_tcgen05_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)ModeCfg<1>::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(gemm_screen_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)ModeCfg<1>::SMEM_BYTES);
+}
+
+// How many 2-CTA clusters of the pair kernel the device can hold at once (0: use the single-CTA kernel).
+cudaError_t gemm_screen_pair_clusters(int num_sms, int* clusters) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(num_sms / 2 * 2));
+    cfg.blockDim = dim3(NUM_THREADS);
+    cfg.dynamicSmemBytes = ModeCfg<1>::SMEM_BYTES;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = 2; attr.val.clusterDim.y = 1; attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    int n = 0;
+    cudaError_t e = cudaOccupancyMaxActiveClusters(&n, gemm_screen_pair_kernel, &cfg);
+    if (e != cudaSuccess) { cudaGetLastError(); n = 0; }
+    *clusters = n;
+    return cudaSuccess;
 }
 
 cudaError_t launch_gemm_tcgen05(const CUtensorMap& tmA_hi, const CUtensorMap& tmA_lo, const CUtensorMap& tmB_hi,
@@ -347,8 +556,14 @@ cudaError_t launch_gemm_tcgen05(const CUtensorMap& tmA_hi, const CUtensorMap& tm
     return cudaGetLastError();
 }
 
-cudaError_t launch_gemm_screen(const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmArgs& g, int num_sms,
-                               cudaStream_t st) {
+cudaError_t launch_gemm_screen(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmB_half,
+                               int pair_clusters, const GemmArgs& g, int num_sms, cudaStream_t st) {
+    if (pair_clusters > 0) {
+        const int npairs = g.num_tb * ((g.num_ib + 1) / 2);
+        const int nc = npairs < pair_clusters ? npairs : pair_clusters;
+        gemm_screen_pair_kernel<<<2 * nc, NUM_THREADS, ModeCfg<1>::SMEM_BYTES, st>>>(tmA, tmB_half, g);
+        return cudaGetLastError();
+    }
     const int ntiles = g.num_tb * g.num_ib;
     const int grid = ntiles < num_sms ? ntiles : num_sms;
     gemm_tcgen05_kernel<1><<<grid, NUM_THREADS, ModeCfg<1>::SMEM_BYTES, st>>>(tmA, tmA, tmB, tmB, g);

@@ -43,7 +43,8 @@ struct rbmf_plan {
     bool have_ws, have_basis, have_coeffs, filtered;
     int num_sms;
     int last_cuda;
-    CUtensorMap tmA_hi, tmA_lo, tmB_hi, tmB_lo, tmB_h16, tmY;
+    CUtensorMap tmA_hi, tmA_lo, tmB_hi, tmB_lo, tmB_h16, tmB_h16half, tmY;
+    int pair_clusters;   // 2-CTA clusters of the screen GEMM the device holds (0: single-CTA kernel)
     bool have_maps;
     cudaEvent_t ev[5];
     bool have_events;
@@ -261,6 +262,9 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     if ((s = make_map_rows(plan, &plan->tmB_lo, plan->ws + L.c_lo, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
     // fp16 data through a 16-bit tensor map: TMA only moves bytes, the element type is irrelevant without OOB fill
     if ((s = make_map_rows(plan, &plan->tmB_h16, plan->ws + L.c_h16, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
+    if ((s = make_map_rows(plan, &plan->tmB_h16half, plan->ws + L.c_h16, 2 * (uint64_t)plan->Tpad, k2, kGemmTT)) != RBMF_OK) return s;
+    CK(gemm_screen_pair_clusters(plan->num_sms, &plan->pair_clusters));
+    if (getenv("RBMF_NO_CLUSTER")) plan->pair_clusters = 0;
     plan->have_maps = true;
     if (!plan->have_events) {
         for (int i = 0; i < 5; ++i) CK(cudaEventCreate(&plan->ev[i]));
@@ -331,7 +335,7 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     g.T = plan->T; g.M = (int)plan->M; g.k2 = 2 * plan->k;
     g.num_tb = plan->Tpad / kGemmTT;
     g.num_ib = (int)(plan->M / kGemmBM);
-    g.group = 16;
+    g.group = 32;   // template blocks per raster group: 32 coefficient tiles (8 MB fp16) stay L2-resident
     if (screen) {
         // Rigorous bound of |R_fp16 - R| for the one-product fp16 screen (derivation: gemm_tcgen05.cu header):
         // operand rounding u = 2^-11 relative (+ eta = 2^-25 sqrt(2) absolute per complex value in the subnormal
@@ -344,7 +348,7 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
         g.kappa1 = (float)((2.0 * u + u * u + (2.0 * k + 64.0) * ldexp(1.0, -22) * 1.4142135623730951) * 1.001);
         g.kappa2 = (float)(eta * sqrt(k) * 1.001);
         g.slack = 1e-4f;   // fp32 rounding of the confirm step and of this threshold arithmetic
-        CK(launch_gemm_screen(plan->tmA_hi, plan->tmB_h16, g, plan->num_sms, st));
+        CK(launch_gemm_screen(plan->tmA_hi, plan->tmB_h16, plan->tmB_h16half, plan->pair_clusters, g, plan->num_sms, st));
     } else if (plan->gemm_impl == RBMF_GEMM_TCGEN05) {
         CK(launch_gemm_tcgen05(plan->tmA_hi, plan->tmA_lo, plan->tmB_hi, plan->tmB_lo, g, plan->num_sms, st));
     } else {

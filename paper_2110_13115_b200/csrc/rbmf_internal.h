@@ -99,8 +99,11 @@ cudaError_t launch_gemm_simt(const uint16_t* a_hi, const uint16_t* a_lo, const u
 cudaError_t launch_gemm_tcgen05(const CUtensorMap& tmA_hi, const CUtensorMap& tmA_lo, const CUtensorMap& tmB_hi,
                                 const CUtensorMap& tmB_lo, const GemmArgs& g, int num_sms, cudaStream_t st);
 // screen mode: one fp16 product; tmA = beta^avg fp16 plane, tmB = coefficient fp16 plane
-cudaError_t launch_gemm_screen(const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmArgs& g, int num_sms,
-                               cudaStream_t st);
+// (pair_clusters > 0: the 2-CTA cluster kernel, which multicasts the coefficient tile and needs tmB_half, the same
+// plane with a 128-row box)
+cudaError_t launch_gemm_screen(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmB_half,
+                               int pair_clusters, const GemmArgs& g, int num_sms, cudaStream_t st);
+cudaError_t gemm_screen_pair_clusters(int num_sms, int* clusters);
 cudaError_t gemm_tcgen05_configure();   // sets the dynamic shared memory attribute once
 cudaError_t launch_stage2(const Stage2Args& a, int num_sms, cudaStream_t st);
 

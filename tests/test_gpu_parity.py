@@ -160,6 +160,20 @@ def test_mini_largest_window(rbmf):
     check(rbmf, workload("mini"), 32, 0.4, 3.0, impl=SCREEN, expect_triggers=False)
 
 
+def test_screen_single_cta_kernel(rbmf, monkeypatch):
+    """The screen's fallback kernel (no thread-block clusters) gives the same lists as the 2-CTA one."""
+    monkeypatch.setenv("RBMF_NO_CLUSTER", "1")
+    check(rbmf, workload("mini"), 8, 3.5, 5.0, impl=SCREEN)
+
+
+def test_single_bin_block(rbmf):
+    """N/w = 128: one time-bin block.  The 2-CTA screen kernel then has a partner CTA whose block lies entirely
+    past the end (TMA zero fill + bin mask)."""
+    wl = workload("tiny", N=1024, T=40, n_inj=1, index=71)
+    for impl in (SCREEN, X3):
+        check(rbmf, wl, 8, 1.5, 3.0, impl=impl, expect_triggers=False)
+
+
 def test_mini_simt_and_tensor_core_candidates_agree(rbmf):
     """The three stage-1 implementations give the same candidate list (threshold ties aside), and the screen's
     superset really contains it with a modest overhead."""
