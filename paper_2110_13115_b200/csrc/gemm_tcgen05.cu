@@ -162,14 +162,31 @@ __device__ __forceinline__ void epilogue_tile(const GemmArgs& g, uint32_t taddr,
         tmem_ld32(taddr + ch * 32, re);
         tmem_ld32(taddr + kGemmTT + ch * 32, im);
         tmem_ld_wait();
-        uint32_t mask = 0;
+        // Common case (no hit in 32 bins x 32 templates): two packed fp32x2 ops and one max per two values, then one
+        // warp vote.  NaN (an fp16 overflow upstream) must pass the screen: fmaxf drops NaN operands, so the squares'
+        // plain sum is tracked too -- it stays NaN or inf if anything was.
+        float vmax = 0.f, vsum = 0.f;
 #pragma unroll
-        for (int j = 0; j < 32; ++j) {
-            const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
-            mask |= (!(fmaf(x, x, y * y) < thr_sq) ? 1u : 0u) << j;   // NaN (fp16 overflow) passes
+        for (int j = 0; j < 32; j += 2) {
+            unsigned long long xx, yy, m2;
+            asm("mov.b64 %0, {%1, %2};" : "=l"(xx) : "r"(re[j]), "r"(re[j + 1]));
+            asm("mov.b64 %0, {%1, %2};" : "=l"(yy) : "r"(im[j]), "r"(im[j + 1]));
+            asm("mul.rn.f32x2 %0, %1, %1;" : "=l"(m2) : "l"(yy));
+            asm("fma.rn.f32x2 %0, %1, %1, %2;" : "=l"(m2) : "l"(xx), "l"(m2));
+            float m0, m1;
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(m0), "=f"(m1) : "l"(m2));
+            vmax = fmaxf(vmax, fmaxf(m0, m1));
+            vsum += m0 + m1;
         }
-        if (bin >= g.M) mask = 0;
-        if (__any_sync(0xffffffffu, mask != 0)) {
+        const bool maybe = bin < g.M && !(vmax < thr_sq && vsum < 3.0e38f);
+        if (__any_sync(0xffffffffu, maybe)) {
+            uint32_t mask = 0;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+                const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
+                mask |= (!(fmaf(x, x, y * y) < thr_sq) ? 1u : 0u) << j;   // NaN (fp16 overflow) passes
+            }
+            if (bin >= g.M) mask = 0;
             // rare path: warp-aggregated append, one atomic per (warp, template column) with hits
 #pragma unroll 1
             for (int j = 0; j < 32; ++j) {
