@@ -242,7 +242,8 @@ struct Smem {
     static constexpr size_t TW_A = NBUF * BUF_BYTES;                      // tw1_a: L1 float2
     static constexpr size_t TW_B = TW_A + ((size_t)8 << LOG1);            // tw1_b: L2 float2
     static constexpr size_t BARS = TW_B + ((size_t)8 << LOG2);            // full[NBUF][NGROUP], empty[NBUF]
-    static constexpr size_t META = BARS + 3 * NBUF * 8;                   // int4 meta[NBUF]
+    static constexpr size_t E2S = BARS + 3 * NBUF * 8;                    // float2 e2s[NGROUP][GT / C]
+    static constexpr size_t META = E2S + NGROUP * (GT / C) * 8;           // int4 meta[NBUF]
     static constexpr size_t TOTAL = META + NBUF * 16 + 128 /* base alignment slack */;
 };
 
@@ -252,12 +253,20 @@ struct Smem {
 // producer); stage 0 multiplies them (a1), transforms along j1 and writes back in place.
 template <int LOG1, int LOG2>
 __device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chunk, int tile, float2* B,
-                                        const float2* tw1) {
+                                        const float2* tw1, float2* e2s) {
     using K = Cfg<LOG1, true>;
     constexpr int L1 = K::L, R0 = K::R0, R1 = K::R1, W = K::W, H = L1 / 2, SUB = K::SUB, RB = K::RB;
     const int col = gt % C, line = (gt / C) % SUB, wk = gt / (C * SUB);
     const int slot = line * C + col;
     const int j2 = tile * SUB + line;
+
+    // Inter-pass twiddle e^{2 pi i j2 n1 / N}, n1 = b + m R0, as the product E1[j2][b] E2[j2][m]: this thread's E1
+    // factors are fetched now and used in stage 1; the SUB x R1 = 64 E2 factors of the tile go to shared memory.
+    constexpr int NB = R0 / R1, L2 = 1 << LOG2;
+    float2 e1[NB];
+#pragma unroll
+    for (int bb = 0; bb < NB; ++bb) e1[bb] = __ldg(a.twN + (size_t)j2 * R0 + wk + bb * W);
+    if (gt < SUB * R1) e2s[gt] = __ldg(a.twN + (size_t)L2 * R0 + (size_t)(tile * SUB) * R1 + gt);
 
     // ---- a1 + stage 0 ---------------------------------------------------------------------------------
     float2 u[R0];
@@ -277,9 +286,9 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chu
 
     // ---- stage 1 + inter-pass twiddle + store of Y (in place in the beta array) -------------------------------
     float2* yrow = a.beta + ((size_t)chunk * (size_t)a.N + (size_t)j2 * L1) * C + col;
-    const float2* tn = a.twN + (size_t)j2 * L1;
-#pragma unroll 1
-    for (int bb = 0; bb < R0 / R1; ++bb) {
+    const float2* e2 = e2s + line * R1;
+#pragma unroll
+    for (int bb = 0; bb < NB; ++bb) {
         const int b = wk + bb * W;   // butterfly index < R0
         float2 x[R1];
 #pragma unroll
@@ -290,7 +299,7 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chu
 #pragma unroll
         for (int m = 0; m < R1; ++m) {
             const int n1 = b + m * R0;
-            __stcg(yrow + n1 * C, cmul(x[m], __ldg(tn + n1)));
+            __stcg(yrow + n1 * C, cmul(cmul(x[m], e2[m]), e1[bb]));
         }
     }
 }
@@ -447,6 +456,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
     auto full_bar = [&](int b, int g) { return bars + 8u * (b * NGROUP + g); };
     auto empty_bar = [&](int b) { return bars + 8u * (NBUF * NGROUP + b); };
     volatile int4* meta = reinterpret_cast<volatile int4*>(sm + S::META);
+    float2* e2s_all = reinterpret_cast<float2*>(sm + S::E2S);
     auto buf_ptr = [&](int b) { return reinterpret_cast<float2*>(sm + (size_t)b * S::BUF_BYTES); };
 
     const int n1t = L2 / K1::SUB;                                  // pass-1 tiles per chunk
@@ -561,7 +571,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
             const int type = meta[buf].x, chunk = meta[buf].y, idx = meta[buf].z, rd = meta[buf].w;
             if (type == TILE_STOP) break;
             float2* B = buf_ptr(buf);
-            if (type == TILE_P1) p1_tile<LOG1, LOG2>(a, g, gt, chunk, idx, B, tw_a);
+            if (type == TILE_P1) p1_tile<LOG1, LOG2>(a, g, gt, chunk, idx, B, tw_a, e2s_all + g * (GT / C));
             else if (type == TILE_P2) p2_round<LOG1, LOG2, NIT>(a, &tmY, g, gt, chunk, idx, rd, rounds, B, tw_b, acc);
             fence_async_smem();   // this thread's generic-proxy writes to the buffer, before the async proxy refills it
             group_sync(g);

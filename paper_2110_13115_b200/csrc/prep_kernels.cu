@@ -18,14 +18,18 @@ __device__ __forceinline__ float2 unit_root(long long num, long long den) {
 }
 
 // tw1[q * R0 + b] = e^{2 pi i q b / L} (stage-1 twiddles of a length-L = R0 * R1 line, q < R1, b < R0);
-// twN[j2 * L1 + n1] = e^{2 pi i j2 n1 / N} (inter-pass twiddles of the four-step FFT).
+// Inter-pass twiddles of the four-step FFT, e^{2 pi i j2 n1 / N} with n1 = b + m R0 (b < R0, m < R1), as two small
+// tables whose product they are:  twN[j2 * R0 + b] = e^{2 pi i j2 b / N}  (L2 x R0 entries), followed by
+// twN[L2 * R0 + j2 * R1 + m] = e^{2 pi i j2 m R0 / N}  (L2 x R1 entries): 256 KB instead of N entries.
 __global__ void init_tables_kernel(float2* tw1_a, float2* tw1_b, float2* twN, int logL1, int logL2) {
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     const int L1 = 1 << logL1, L2 = 1 << logL2;
     const long long N = (long long)L1 * L2;
     if (i < L1) { const int R0 = fft_r0(logL1); tw1_a[i] = unit_root((i / R0) * (i % R0), L1); }
     if (i < L2) { const int R0 = fft_r0(logL2); tw1_b[i] = unit_root((i / R0) * (i % R0), L2); }
-    if (i < N) twN[i] = unit_root((i / L1) * (i % L1), N);
+    const int R0 = fft_r0(logL1), R1 = fft_r1(logL1);
+    if (i < (long long)L2 * R0) twN[i] = unit_root((i / R0) * (i % R0), N);
+    if (i < (long long)L2 * R1) twN[(long long)L2 * R0 + i] = unit_root((i / R1) * (i % R1) * R0, N);
 }
 
 cudaError_t launch_init_tables(float2* tw1_a, float2* tw1_b, float2* twN, int logL1, int logL2, cudaStream_t st) {

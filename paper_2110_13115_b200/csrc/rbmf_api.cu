@@ -71,7 +71,7 @@ Layout make_layout(const rbmf_plan* p) {
     L.cs = take((size_t)p->T * k * 8);
     L.tw1_a = take(((size_t)1 << p->logN1) * 8);
     L.tw1_b = take(((size_t)1 << p->logN2) * 8);
-    L.twN = take(N * 8);
+    L.twN = take(((size_t)1 << p->logN2) * (size_t)(fft_r0(p->logN1) + fft_r1(p->logN1)) * 8);   // two factor tables
     L.dsT = take((size_t)p->n_half * 8);
     L.cand = take((size_t)p->max_cand * sizeof(rbmf_candidate));
     L.cand2 = take((size_t)p->max_cand * sizeof(rbmf_candidate));

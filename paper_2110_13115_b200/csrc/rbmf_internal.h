@@ -32,7 +32,7 @@ struct FftArgs {
     const float2* dsT;       // [j2 < L2][j1 < L1/2]: s * d[j1 L2 + j2]
     const float2* tw1_a;     // pass 1 stage-1 twiddles  [q < R1][b < R0] = e^{2 pi i q b / L1}
     const float2* tw1_b;     // pass 2 stage-1 twiddles, same for L2
-    const float2* twN;       // inter-pass twiddles [j2 < L2][n1 < L1] = e^{2 pi i j2 n1 / N}
+    const float2* twN;       // inter-pass twiddles as two factor tables, [j2][b < R0] then [j2][m < R1] (prep_kernels.cu)
     float2* beta;            // [chunk][n < N][C]; between the passes it holds Y[n1][j2] at index n1 + L1 j2
     uint16_t* plane_hi;      // [kb = col / 32][bin < M][64]: bf16 (re, im) of column col % 32
     uint16_t* plane_lo;
