@@ -30,8 +30,8 @@ UNIT = "template-seconds/s"
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the `ncu --set full` captures summarised
 # under profiles/ (r01_launches.md); known only for the configuration that was profiled, else reported as null.
-NCU_TRAFFIC = {("paper", 8, "screen", "gemm"): 290.4e6 + 2.0e6, ("paper", 8, "screen", "fft"): 551.6e6 + 1232.5e6,
-               ("paper", 8, "screen", "stage2"): 178.5e6 + 4.4e6}
+NCU_TRAFFIC = {("paper", 8, "screen", "gemm"): 365.7e6 + 1.6e6, ("paper", 8, "screen", "fft"): 541.7e6 + 1175.5e6,
+               ("paper", 8, "screen", "stage2"): 180.6e6 + 8.7e6}
 
 
 # ------------------------------------------------------------------------------------------------- clocks
@@ -276,7 +276,7 @@ def main():
     band = cfg.N // 2 - cfg.j_low
     fft_alg_bytes = cfg.k * band * 8 + (cfg.N // 2 + 1) * 8 + cfg.k * cfg.N * 8 + cfg.k * M * 8
     fft_gbs = fft_alg_bytes / (fft_ms * 1e-3) / 1e9
-    roofline = {"kernel": "gemm_tcgen05_kernel (a4-a5)", "bound": "tensor", "achieved": gemm_tflops,
+    roofline = {"kernel": ("gemm_screen_pair_kernel" if args.gemm == "screen" else "gemm_tcgen05_kernel") + " (a4-a5)", "bound": "tensor", "achieved": gemm_tflops,
                 "peak": tensor_peak, "unit": "TFLOP/s", "frac": gemm_tflops / tensor_peak,
                 "traffic": NCU_TRAFFIC.get((args.config, cfg.w, args.gemm, "gemm")),
                 "peak_source": peak_src, "flops_counted": "executed 16-bit MMA flops = %d x 8 T k N/w (%s)" % (
