@@ -183,24 +183,30 @@ def main():
     strain_np, _ = workloads.make_strain(wl, seg)
     stream = torch.cuda.Stream(device=device)
     with torch.cuda.stream(stream):
-        plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, device=str(device), stream=stream)
         impls = {"screen": rbmf.RBMF_GEMM_SCREEN, "bf16x3": rbmf.RBMF_GEMM_TCGEN05, "simt": rbmf.RBMF_GEMM_SIMT}
-        plan.set_gemm_impl(impls[args.gemm])
-        plan.set_basis(torch.from_numpy(wl["basis"]))
-        plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
         strain_dev = torch.from_numpy(strain_np).to(device)
         strain_pinned = torch.from_numpy(strain_np).pin_memory()
+        capacity = 1 << 22
+        while True:
+            # list capacities grow until one warm-up pass fits (dense banks give 1e6-1e7 records)
+            plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, device=str(device), stream=stream,
+                             max_candidates=capacity, max_triggers=capacity)
+            plan.set_gemm_impl(impls[args.gemm])
+            plan.set_basis(torch.from_numpy(wl["basis"]))
+            plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+            torch.cuda.empty_cache()
+            for _ in range(args.warmup):
+                plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
+            stream.synchronize()
+            nc, nt, st = plan.counts(allow_overflow=True)
+            if st != rbmf.RBMF_ERR_OVERFLOW or capacity >= (1 << 26):
+                break
+            plan.close()
+            capacity <<= 2
         out_host = np.empty(plan.max_triggers, dtype=rbmf.TRIGGER_DTYPE)
-        torch.cuda.empty_cache()
         plan.set_timing(True)
         sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
                                int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
-
-        # ---- device-resident leg
-        for _ in range(args.warmup):
-            plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
-        stream.synchronize()
-        nc, nt, _ = plan.counts(allow_overflow=True)
         rdist.barrier(device)
         torch.cuda.synchronize(device)
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -287,7 +293,8 @@ def main():
               "fft": {"bound": "hbm", "algorithmic_GBps": fft_gbs, "peak": hbm_peak, "frac": fft_gbs / hbm_peak,
                       "algorithmic_bytes": fft_alg_bytes,
                       "traffic": NCU_TRAFFIC.get((args.config, cfg.w, args.gemm, "fft"))},
-              "n_candidates": nc, "n_triggers": nt, "gemm_mode": args.gemm}
+              "n_candidates": nc, "n_triggers": nt, "gemm_mode": args.gemm, "list_capacity": capacity,
+              "lists_overflowed": bool(nc > capacity or nt > capacity)}
     if other_stage is not None:
         stages["other_mode"] = dict(other_stage, gemm_mode=other)
 

@@ -11,10 +11,11 @@
 // before writing the operand plane(s) of kernel 2.
 //
 // Columns are processed in chunks of C = 4 (32-byte row segments).  Work queue (global ticket counter):
-//   P1(0) | P1(1) P2(0) | P1(2) P2(1) | ...   so chunk c's intermediate Y (N * 32 bytes) is written and read back
-// while it is still in the 126 MB L2.  Y lives IN PLACE in the chunk's block of the beta array (Y[n1][j2] at the
-// address of beta[n1 + L1 j2]): a pass-2 item reads exactly the addresses it then overwrites, so dirty Y lines are
-// overwritten in L2 before they are evicted and only basis (read) and beta / planes (written) touch HBM.
+//   P1(0) | P1(1) P2(0) | P1(2) P2(1) | ...   (pass 1 runs kFftLookahead chunks ahead; two were measured: no gain) so
+// chunk c's intermediate Y (N * 32 bytes) is written and read back while it is still in the 126 MB L2.  Y lives IN
+// PLACE in the chunk's block of the beta array (Y[n1][j2] at the address of beta[n1 + L1 j2]): a pass-2 item reads
+// exactly the addresses it then overwrites, so dirty Y lines are overwritten in L2 before they are evicted and only
+// basis (read) and beta / planes (written) touch HBM.
 //
 // One CTA per SM, 16 consumer warps + a producer warpgroup of which one warp works:
 //   warp 16      producer: draws tickets, waits for a chunk's pass-1 completion counter before its pass-2 items, and
@@ -501,14 +502,23 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                 } else if (next_ticket < total) {
                     const int t = next_ticket;
                     next_ticket = (int)atomicAdd(a.sched, 1u);
-                    // queue order: P1(0) | P1(1) P2(0) | P1(2) P2(1) | ... | P1(n-1) P2(n-2) | P2(n-1)
+                    // queue order, pass 1 running LA chunks ahead of pass 2:
+                    //   P1(0) .. P1(LA-1) | P1(LA) P2(0) | P1(LA+1) P2(1) | ... | P2(n-LA) | ... | P2(n-1)
+                    constexpr int LA = kFftLookahead;
+                    const int la = a.nchunk < LA ? a.nchunk : LA, nfull = a.nchunk - la;
                     bool first = true;
-                    chunk = 0; idx = t;
-                    if (t >= n1t) {
-                        const int u = t - n1t;
-                        const int blk = u / per, v = u - blk * per;
-                        if (blk < a.nchunk - 1 && v < n1t) { chunk = blk + 1; idx = v; }
-                        else { first = false; chunk = blk; idx = blk < a.nchunk - 1 ? v - n1t : v; }
+                    if (t < la * n1t) {
+                        chunk = t / n1t; idx = t - chunk * n1t;
+                    } else {
+                        const int u = t - la * n1t;
+                        if (u < nfull * per) {
+                            const int blk = u / per, v = u - blk * per;
+                            if (v < n1t) { chunk = blk + la; idx = v; }
+                            else { first = false; chunk = blk; idx = v - n1t; }
+                        } else {
+                            const int u2 = u - nfull * per;
+                            first = false; chunk = nfull + u2 / n2t; idx = u2 % n2t;
+                        }
                     }
                     if (first) {
                         type = TILE_P1;

@@ -152,19 +152,25 @@ __device__ __forceinline__ void decode_tile(const GemmArgs& g, int tile, int& ib
 
 __device__ __forceinline__ int num_tiles(const GemmArgs& g) { return g.num_tb * g.num_ib; }
 
-// Epilogue of one 128-bin x 128-template tile for one warp (its 32 TMEM lanes = 32 time bins): |R|^2 against the
-// threshold of this bin, warp vote, and -- only where something hit -- a warp-aggregated append to the candidate list.
+// Epilogue of one 128-bin x 128-template tile for one warp (its 32 TMEM lanes = 32 time bins).
+// Pass 1 (every tile): |R|^2 against the threshold of this bin -- two packed fp32x2 ops and one max per two values --
+// and one warp vote per 32 templates; the per-value hit masks are built only where the vote fired.
+// Pass 2 (only if something hit): ONE atomicAdd per warp and tile reserves the list space for all its hits (a loud
+// injection fires in thousands of tiles at once: per-column atomics on the single counter serialise in L2), then the
+// chunks that hit are read from TMEM again and written out.
 __device__ __forceinline__ void epilogue_tile(const GemmArgs& g, uint32_t taddr, int bin, int tb, int lane,
                                               float thr_sq) {
-#pragma unroll 1
-    for (int ch = 0; ch < kGemmTT / 32; ++ch) {
+    constexpr int NCH = kGemmTT / 32;
+    uint32_t mask[NCH];
+    bool any = false;
+#pragma unroll
+    for (int ch = 0; ch < NCH; ++ch) {
         uint32_t re[32], im[32];
         tmem_ld32(taddr + ch * 32, re);
         tmem_ld32(taddr + kGemmTT + ch * 32, im);
         tmem_ld_wait();
-        // Common case (no hit in 32 bins x 32 templates): two packed fp32x2 ops and one max per two values, then one
-        // warp vote.  NaN (an fp16 overflow upstream) must pass the screen: fmaxf drops NaN operands, so the squares'
-        // plain sum is tracked too -- it stays NaN or inf if anything was.
+        // NaN (an fp16 overflow upstream) must pass the screen: fmaxf drops NaN operands, so the plain sum of the
+        // squares is tracked too -- it stays NaN or inf if anything was.
         float vmax = 0.f, vsum = 0.f;
 #pragma unroll
         for (int j = 0; j < 32; j += 2) {
@@ -179,45 +185,60 @@ __device__ __forceinline__ void epilogue_tile(const GemmArgs& g, uint32_t taddr,
             vsum += m0 + m1;
         }
         const bool maybe = bin < g.M && !(vmax < thr_sq && vsum < 3.0e38f);
+        uint32_t m = 0;
         if (__any_sync(0xffffffffu, maybe)) {
-            uint32_t mask = 0;
 #pragma unroll
             for (int j = 0; j < 32; ++j) {
                 const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
-                mask |= (!(fmaf(x, x, y * y) < thr_sq) ? 1u : 0u) << j;   // NaN (fp16 overflow) passes
+                const bool hit = !(fmaf(x, x, y * y) < thr_sq) && (tb * kGemmTT + ch * 32 + j) < g.T;
+                m |= (hit ? 1u : 0u) << j;
             }
-            if (bin >= g.M) mask = 0;
-            // rare path: warp-aggregated append, one atomic per (warp, template column) with hits
-#pragma unroll 1
-            for (int j = 0; j < 32; ++j) {
-                const bool hit = (mask >> j) & 1u;
-                const unsigned ballot = __ballot_sync(0xffffffffu, hit);
-                if (ballot == 0) continue;
-                unsigned long long base = 0;
-                if (lane == 0) base = atomicAdd(g.counters, (unsigned long long)__popc(ballot));
-                base = __shfl_sync(0xffffffffu, base, 0);
-                if (hit) {
-                    const unsigned long long idx = base + __popc(ballot & ((1u << lane) - 1u));
-                    const int t = tb * kGemmTT + ch * 32 + j;
-                    if (idx < g.cand_cap && t < g.T) {
-                        rbmf_candidate cd;
-                        cd.template_id = t;
-                        cd.bin_index = bin;
-                        // dynamic register index -> select through a small unrolled search
-                        float x = 0.f, y = 0.f;
+            if (bin >= g.M) m = 0;
+        }
+        mask[ch] = m;
+        any |= m != 0;
+    }
+    if (!__any_sync(0xffffffffu, any)) return;
+
+    // ---- rare path: reserve, then write ------------------------------------------------------------------------
+    int cnt = 0;
 #pragma unroll
-                        for (int jj = 0; jj < 32; ++jj)
-                            if (jj == j) { x = __uint_as_float(re[jj]); y = __uint_as_float(im[jj]); }
-                        cd.avg_re = x;
-                        cd.avg_im = y;
-                        g.cand[idx] = cd;
-                    }
+    for (int ch = 0; ch < NCH; ++ch) cnt += __popc(mask[ch]);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    unsigned long long base = 0;
+    if (lane == 0) base = atomicAdd(g.counters, (unsigned long long)total);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    unsigned long long idx = base + (unsigned long long)(incl - cnt);
+#pragma unroll 1
+    for (int ch = 0; ch < NCH; ++ch) {
+        const uint32_t m = mask[ch];
+        if (__ballot_sync(0xffffffffu, m != 0) == 0) continue;
+        uint32_t re[32], im[32];
+        tmem_ld32(taddr + ch * 32, re);
+        tmem_ld32(taddr + kGemmTT + ch * 32, im);
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            if ((m >> j) & 1u) {
+                if (idx < g.cand_cap) {
+                    rbmf_candidate cd;
+                    cd.template_id = tb * kGemmTT + ch * 32 + j;
+                    cd.bin_index = bin;
+                    cd.avg_re = __uint_as_float(re[j]);
+                    cd.avg_im = __uint_as_float(im[j]);
+                    g.cand[idx] = cd;
                 }
+                ++idx;
             }
         }
     }
 }
-
 
 }  // namespace
 

@@ -10,7 +10,33 @@ namespace rbmf {
 // beta is chunk-blocked, [chunk][n][C = 4]: per chunk the candidate's w rows are one contiguous block of w * 32
 // bytes.  The warp walks float4 items e = (chunk, r, half) in this order, e = lane, lane + 32, ...: with 2w <= 32 a
 // lane always sees the same (r, half), so it accumulates one row's partial sum; w = 32 alternates between two rows.
+// Outputs are staged per warp in shared memory and flushed with ONE atomicAdd per 32+ records: with millions of
+// candidates (a loud injection in a dense bank) per-candidate atomics on the two list counters serialise in L2.
 __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
+    __shared__ rbmf_trigger tbuf_all[8][64];
+    __shared__ rbmf_candidate cbuf_all[8][32];
+    rbmf_trigger* tbuf = tbuf_all[threadIdx.x >> 5];
+    rbmf_candidate* cbuf = cbuf_all[threadIdx.x >> 5];
+    int tcount = 0, ccount = 0;   // warp-uniform fill levels
+    auto flush_triggers = [&](int lane_) {
+        unsigned long long base = 0;
+        if (lane_ == 0) base = atomicAdd(a.counters + 1, (unsigned long long)tcount);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        __syncwarp();
+        for (int i = lane_; i < tcount; i += 32)
+            if (base + i < a.trig_cap) a.out[base + i] = tbuf[i];
+        __syncwarp();
+        tcount = 0;
+    };
+    auto flush_confirmed = [&](int lane_) {
+        unsigned long long base = 0;
+        if (lane_ == 0) base = atomicAdd(a.counters + 2, (unsigned long long)ccount);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        __syncwarp();
+        if (lane_ < ccount && base + lane_ < a.cand_cap) a.confirmed[base + lane_] = cbuf[lane_];
+        __syncwarp();
+        ccount = 0;
+    };
     const int lane = threadIdx.x & 31;
     const unsigned long long warp0 = (unsigned long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const unsigned long long nwarps = (unsigned long long)gridDim.x * (blockDim.x >> 5);
@@ -89,13 +115,11 @@ __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
             sr *= inv_w; si *= inv_w;
             if (!(sr * sr + si * si >= a.thr1_sq)) continue;   // warp-uniform
             if (lane == 0) {
-                const unsigned long long idx = atomicAdd(a.counters + 2, 1ULL);
-                if (idx < a.cand_cap) {
-                    rbmf_candidate c2;
-                    c2.template_id = cd.template_id; c2.bin_index = cd.bin_index; c2.avg_re = sr; c2.avg_im = si;
-                    a.confirmed[idx] = c2;
-                }
+                rbmf_candidate c2;
+                c2.template_id = cd.template_id; c2.bin_index = cd.bin_index; c2.avg_re = sr; c2.avg_im = si;
+                cbuf[ccount] = c2;
             }
+            if (++ccount == 32) flush_confirmed(lane);
         }
         for (int s = 0; s < nslot; ++s) {
             const int r = (lane >> 1) + 16 * s;
@@ -104,23 +128,21 @@ __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
             const bool hit = owner && (vr * vr + vi * vi >= a.thr2_sq);
             const unsigned ballot = __ballot_sync(0xffffffffu, hit);
             if (ballot) {
-                unsigned long long base = 0;
-                if (lane == 0) base = atomicAdd(a.counters + 1, (unsigned long long)__popc(ballot));
-                base = __shfl_sync(0xffffffffu, base, 0);
                 if (hit) {
-                    const unsigned long long idx = base + __popc(ballot & ((1u << lane) - 1u));
-                    if (idx < a.trig_cap) {
-                        rbmf_trigger t;
-                        t.template_id = cd.template_id;
-                        t.time_index = cd.bin_index * w + r;
-                        t.snr_re = vr;
-                        t.snr_im = vi;
-                        a.out[idx] = t;
-                    }
+                    rbmf_trigger t;
+                    t.template_id = cd.template_id;
+                    t.time_index = cd.bin_index * w + r;
+                    t.snr_re = vr;
+                    t.snr_im = vi;
+                    tbuf[tcount + __popc(ballot & ((1u << lane) - 1u))] = t;
                 }
+                tcount += __popc(ballot);          // at most 16 per slot: 32 + 16 <= 64 entries
+                if (tcount > 32) flush_triggers(lane);
             }
         }
     }
+    if (tcount > 0) flush_triggers(lane);
+    if (ccount > 0) flush_confirmed(lane);
 }
 
 cudaError_t launch_stage2(const Stage2Args& a, int num_sms, cudaStream_t st) {
