@@ -30,8 +30,8 @@ UNIT = "template-seconds/s"
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the `ncu --set full` captures summarised
 # under profiles/ (r01_launches.md); known only for the configuration that was profiled, else reported as null.
-NCU_TRAFFIC = {("paper", 8, "screen", "gemm"): 365.7e6 + 1.6e6, ("paper", 8, "screen", "fft"): 541.7e6 + 1175.5e6,
-               ("paper", 8, "screen", "stage2"): 180.6e6 + 8.7e6}
+NCU_TRAFFIC = {("paper", 8, "screen", "gemm"): 359.5e6 + 2.5e6, ("paper", 8, "screen", "fft"): 542.8e6 + 1181.2e6,
+               ("paper", 8, "screen", "stage2"): 186.0e6 + 3.9e6}
 
 
 # ------------------------------------------------------------------------------------------------- clocks
