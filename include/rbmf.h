@@ -13,8 +13,9 @@
  *
  * with s = sqrt(2/N), d = unnormalised forward DFT of the whitened unit-variance strain, b_k orthonormal
  * over the band, c_tk the decomposition coefficients.  Every step runs in hand-written CUDA
- * kernels for sm_100a (batched Stockham FFT; tcgen05/TMEM split-bf16 GEMM with a fused threshold/compaction
- * epilogue; a warp-per-candidate re-scoring kernel).  There is no CPU fallback.
+ * kernels for sm_100a (a persistent, TMA-fed batched four-step Stockham FFT; a tcgen05/TMEM GEMM -- fp16 screen with a
+ * proven error bound by default, split-bf16 on request -- with a fused threshold/compaction epilogue; a
+ * warp-per-candidate re-scoring kernel that also confirms the screen's hits in fp32).  There is no CPU fallback.
  *
  * Conventions
  *  - "dev" pointers are CUDA device memory owned by the caller; "host" pointers are ordinary host memory.
