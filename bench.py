@@ -203,7 +203,9 @@ def main():
                 break
             plan.close()
             capacity <<= 2
-        out_host = np.empty(plan.max_triggers, dtype=rbmf.TRIGGER_DTYPE)
+        # pinned host array for the trigger list (the end-to-end leg copies into it every step)
+        out_pinned = torch.empty(plan.max_triggers * 4, dtype=torch.int32).pin_memory()
+        out_host = out_pinned.numpy().view(rbmf.TRIGGER_DTYPE)
         plan.set_timing(True)
         sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
                                int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
