@@ -45,6 +45,7 @@ constexpr int GT = kFftThreads;         // threads per consumer group
 constexpr int NGROUP = 2;
 constexpr int NT = NGROUP * GT + 128;   // + producer warpgroup (one working warp; setmaxnreg acts on warpgroups)
 constexpr int NBUF = 3;
+constexpr int kE2Stride = GT / C + 2 * 16;   // per-group E2 factors: SUB lines of R1 entries, each line padded by 2
 
 // ------------------------------------------------------------------------------------------------ complex helpers
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
@@ -243,8 +244,8 @@ struct Smem {
     static constexpr size_t TW_A = NBUF * BUF_BYTES;                      // tw1_a: L1 float2
     static constexpr size_t TW_B = TW_A + ((size_t)8 << LOG1);            // tw1_b: L2 float2
     static constexpr size_t BARS = TW_B + ((size_t)8 << LOG2);            // full[NBUF][NGROUP], empty[NBUF]
-    static constexpr size_t E2S = BARS + 3 * NBUF * 8;                    // float2 e2s[NGROUP][GT / C]
-    static constexpr size_t META = E2S + NGROUP * (GT / C) * 8;           // int4 meta[NBUF]
+    static constexpr size_t E2S = BARS + 3 * NBUF * 8;                    // float2 e2s[NGROUP][kE2Stride]
+    static constexpr size_t META = E2S + NGROUP * kE2Stride * 8;          // int4 meta[NBUF]
     static constexpr size_t TOTAL = META + NBUF * 16 + 128 /* base alignment slack */;
 };
 
@@ -267,7 +268,8 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chu
     float2 e1[NB];
 #pragma unroll
     for (int bb = 0; bb < NB; ++bb) e1[bb] = __ldg(a.twN + (size_t)j2 * R0 + wk + bb * W);
-    if (gt < SUB * R1) e2s[gt] = __ldg(a.twN + (size_t)L2 * R0 + (size_t)(tile * SUB) * R1 + gt);
+    // (lines are padded by two entries: the lanes of a warp read the same entry of 2+ different lines at once)
+    if (gt < SUB * R1) e2s[gt + 2 * (gt / R1)] = __ldg(a.twN + (size_t)L2 * R0 + (size_t)(tile * SUB) * R1 + gt);
 
     // ---- a1 + stage 0 ---------------------------------------------------------------------------------
     float2 u[R0];
@@ -287,7 +289,7 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chu
 
     // ---- stage 1 + inter-pass twiddle + store of Y (in place in the beta array) -------------------------------
     float2* yrow = a.beta + ((size_t)chunk * (size_t)a.N + (size_t)j2 * L1) * C + col;
-    const float2* e2 = e2s + line * R1;
+    const float2* e2 = e2s + line * (R1 + 2);
 #pragma unroll
     for (int bb = 0; bb < NB; ++bb) {
         const int b = wk + bb * W;   // butterfly index < R0
@@ -581,7 +583,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
             const int type = meta[buf].x, chunk = meta[buf].y, idx = meta[buf].z, rd = meta[buf].w;
             if (type == TILE_STOP) break;
             float2* B = buf_ptr(buf);
-            if (type == TILE_P1) p1_tile<LOG1, LOG2>(a, g, gt, chunk, idx, B, tw_a, e2s_all + g * (GT / C));
+            if (type == TILE_P1) p1_tile<LOG1, LOG2>(a, g, gt, chunk, idx, B, tw_a, e2s_all + g * kE2Stride);
             else if (type == TILE_P2) p2_round<LOG1, LOG2, NIT>(a, &tmY, g, gt, chunk, idx, rd, rounds, B, tw_b, acc);
             fence_async_smem();   // this thread's generic-proxy writes to the buffer, before the async proxy refills it
             group_sync(g);
