@@ -11,7 +11,7 @@
 // before writing the operand plane(s) of kernel 2.
 //
 // Columns are processed in chunks of C = 4 (32-byte row segments).  Work queue (global ticket counter):
-//   P1(0) | P1(1) P2(0) | P1(2) P2(1) | ...   (pass 1 runs kFftLookahead chunks ahead; two were measured: no gain) so
+//   P1(0) | P1(1) P2(0) | P1(2) P2(1) | ...   (pass 1 runs FftArgs::lookahead chunks ahead, see rbmf_api.cu) so
 // chunk c's intermediate Y (N * 32 bytes) is written and read back while it is still in the 126 MB L2.  Y lives IN
 // PLACE in the chunk's block of the beta array (Y[n1][j2] at the address of beta[n1 + L1 j2]): a pass-2 item reads
 // exactly the addresses it then overwrites, so dirty Y lines are overwritten in L2 before they are evicted and only
@@ -506,7 +506,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                     next_ticket = (int)atomicAdd(a.sched, 1u);
                     // queue order, pass 1 running LA chunks ahead of pass 2:
                     //   P1(0) .. P1(LA-1) | P1(LA) P2(0) | P1(LA+1) P2(1) | ... | P2(n-LA) | ... | P2(n-1)
-                    constexpr int LA = kFftLookahead;
+                    const int LA = a.lookahead;
                     const int la = a.nchunk < LA ? a.nchunk : LA, nfull = a.nchunk - la;
                     bool first = true;
                     if (t < la * n1t) {

@@ -319,6 +319,17 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     a.N = plan->N; a.M = (int)plan->M; a.nchunk = plan->k / kFftC; a.w = plan->w; a.inv_w = 1.0f / (float)plan->w;
     const bool screen = plan->gemm_impl == RBMF_GEMM_SCREEN;
     a.plane_fp16 = screen ? 1 : 0;
+    {
+        // Pass-1 lookahead: a chunk's pass 2 needs ALL of its pass-1 tiles, so enough pass-1 tiles of later chunks
+        // must be queued to keep every consumer group (2 per SM) busy meanwhile -- about two tiles per group --,
+        // limited by what Y (N x 32 bytes per chunk, lookahead + 1 chunks alive) may occupy in L2 (48 MB).
+        const long long n1t = (1ll << plan->logN2) / fft_sub(plan->logN1);
+        long long la = (4ll * plan->fft_grid + n1t - 1) / n1t;
+        const long long cap = (48ll << 20) / ((long long)plan->N * kFftC * 8) - 1;
+        if (la > cap) la = cap;
+        if (la < 1) la = 1;
+        a.lookahead = (int)la;
+    }
     CK(launch_fft_tma(plan->tmY, a, plan->logN1, plan->logN2, plan->fft_grid, st));
     if (screen)
         CK(launch_bin_norm(at<uint16_t>(plan, L.bavg_hi), at<float>(plan, L.bin_norm), (int)plan->M,

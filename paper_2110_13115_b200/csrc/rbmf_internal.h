@@ -12,7 +12,6 @@ namespace rbmf {
 constexpr int kFftC = 4;           // basis columns per FFT chunk (32-byte row segments)
 constexpr int kFftThreads = 256;   // threads per FFT consumer group
 constexpr int kMaxChunks = 256;    // k <= 1024
-constexpr int kFftLookahead = 1;   // chunks pass 1 runs ahead of pass 2 in the FFT work queue (their Y must fit in L2)
 constexpr int kGemmBM = 128;       // time bins per GEMM tile (UMMA M)
 constexpr int kGemmTT = 128;       // templates per GEMM tile (UMMA N = 2*kGemmTT: re | im rows)
 constexpr int kGemmBK = 64;        // bf16 elements per K block (= one 128-byte swizzle row = 32 basis columns)
@@ -43,6 +42,7 @@ struct FftArgs {
     int nchunk;              // k / C
     int w;
     float inv_w;
+    int lookahead;           // chunks pass 1 runs ahead of pass 2 in the work queue (their Y must fit in L2)
     int plane_fp16;          // 1: write ONE fp16 plane (screen mode) into plane_hi; 0: bf16 hi + lo planes
 };
 
