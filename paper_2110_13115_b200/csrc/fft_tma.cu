@@ -28,7 +28,9 @@
 // Inside a group a line of length L = R0 * R1 is two Stockham stages: a thread owns one column and R0 elements; stage 0
 // reads its elements (positions wk + q W) from the tile buffer, does a radix-R0 DFT in registers and writes the results
 // back IN PLACE (the same, thread-private positions); after the group barrier stage 1 reads R1 consecutive positions,
-// applies the twiddles (table in shared memory), does a radix-R1 DFT and stores straight to global memory.
+// applies the twiddles (table in shared memory) and does a radix-R1 DFT.  Pass 1 then multiplies by the inter-pass
+// twiddle (product of two small tables) and stores Y straight to global memory; pass 2 writes its rows back to the tile
+// buffer, where the bin sums read them, and one TMA tensor store moves them to the beta array.
 // Tile buffer layout: [position][line][column] (one row = SUB lines x 4 columns), conflict-free for both stages; when
 // a row is only 64 bytes (L = 1024) one pad row per 32 rows keeps stage 1 conflict-free.
 #include <cuda_bf16.h>
