@@ -233,6 +233,9 @@ struct Cfg {
     static constexpr bool PAD = PASS1 && RB * 8 == 64;   // 64-byte rows: one pad row per 32 rows
     static constexpr int ROWS = PAD ? L + L / 32 : L;
     static constexpr int TILE_F2 = ROWS * RB;         // float2 per tile buffer
+    // strain slice of a pass-1 tile: one row of H values per line, rows offset so that the SUB lines a warp reads at
+    // once fall into different banks
+    static constexpr int SPAD = 16 / SUB > 2 ? 16 / SUB : 2;
     __device__ static __forceinline__ int idx(int p) { return PAD ? p + (p >> 5) : p; }
 };
 
@@ -276,7 +279,7 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chu
     // ---- a1 + stage 0 ---------------------------------------------------------------------------------
     float2 u[R0];
     {
-        const float2* S = B + K::idx(H) * RB + line * H;
+        const float2* S = B + K::idx(H) * RB + line * (H + K::SPAD);
 #pragma unroll
         for (int q = 0; q < R0 / 2; ++q) {
             const int j1 = wk + q * W;
@@ -554,9 +557,11 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                 } else if (lane == 0) {
                     bulk_g2s(dst, src, basis_bytes, full_bar(buf, g), pol_first);
                 }
-                if (lane == 31)
-                    bulk_g2s(dst + (uint32_t)K1::idx(H) * K1::RB * 8, a.dsT + (size_t)idx * K1::SUB * H, strain_bytes,
-                             full_bar(buf, g), pol_last);
+                if (lane >= 32 - K1::SUB) {   // one copy per line (padded rows, see Cfg::SPAD)
+                    const int l = 31 - lane;
+                    bulk_g2s(dst + (uint32_t)(K1::idx(H) * K1::RB + l * (H + K1::SPAD)) * 8,
+                             a.dsT + ((size_t)idx * K1::SUB + l) * H, (uint32_t)H * 8, full_bar(buf, g), pol_last);
+                }
             } else if (type == TILE_P2) {
                 constexpr int BR = L2 < 256 ? L2 : 256;   // rows per tensor copy
                 if (lane == 0) mbar_expect_tx(full_bar(buf, g), (uint32_t)L2 * K2::RB * 8);
