@@ -39,21 +39,8 @@ def compare_triggers(got, oracle_result, N, thr1, thr2, tau=TAU, snr_rtol=1e-3, 
     extra = np.setdiff1d(k_got, k_all)
 
     # per-trigger values against the oracle's value at the same (template, time)
-    order = np.argsort(k_all)
-    pos = np.searchsorted(k_all[order], k_got)
-    pos = np.clip(pos, 0, max(len(k_all) - 1, 0))
-    matched = len(k_all) > 0
-    max_rel, max_phase, bad_val = 0.0, 0.0, 0
-    if matched and len(k_got):
-        idx = order[pos]
-        hit = k_all[idx] == k_got
-        ref = allowed["re"][idx[hit]] + 1j * allowed["im"][idx[hit]]
-        val = got["re"][hit].astype(np.float64) + 1j * got["im"][hit].astype(np.float64)
-        rel = np.abs(np.abs(val) - np.abs(ref)) / np.abs(ref)
-        ph = np.abs(np.angle(val * np.conj(ref)))
-        if len(rel):
-            max_rel, max_phase = float(rel.max()), float(ph.max())
-            bad_val = int(((rel > snr_rtol) | (ph > phase_atol)).sum())
+    max_rel, max_phase, bad_val = _match_values(k_got, got["re"], got["im"], k_all, allowed["re"], allowed["im"],
+                                                snr_rtol, phase_atol)
     ok = dup == 0 and len(missing) == 0 and len(extra) == 0 and bad_val == 0
     return {
         "ok": bool(ok), "n_got": int(len(k_got)), "n_oracle": int(len(trig)), "n_mandatory": int(len(k_man)),
@@ -63,16 +50,43 @@ def compare_triggers(got, oracle_result, N, thr1, thr2, tau=TAU, snr_rtol=1e-3, 
     }
 
 
-def compare_candidates(got, oracle_result, n_bins, thr1, tau=TAU):
-    """First-stage candidate sets: oracle candidates with margin > tau must be present; every reported candidate must
-    have an oracle averaged SNR within tau of the threshold or above.  `got` has fields template, bin, re, im.
-    The allowed side needs |rho_bar| of bins just below thr1, which `oracle_filter` does not keep, so the caller
-    passes `oracle_result['cand_near']` when available; otherwise only the mandatory side is checked."""
+def _match_values(k_got, got_re, got_im, k_ref, ref_re, ref_im, snr_rtol, phase_atol):
+    """For every got key present in k_ref: relative modulus error and phase error against the reference value."""
+    if len(k_ref) == 0 or len(k_got) == 0:
+        return 0.0, 0.0, 0
+    order = np.argsort(k_ref)
+    pos = np.clip(np.searchsorted(k_ref[order], k_got), 0, len(k_ref) - 1)
+    idx = order[pos]
+    hit = k_ref[idx] == k_got
+    ref = np.asarray(ref_re)[idx[hit]] + 1j * np.asarray(ref_im)[idx[hit]]
+    val = np.asarray(got_re)[hit].astype(np.float64) + 1j * np.asarray(got_im)[hit].astype(np.float64)
+    if len(ref) == 0:
+        return 0.0, 0.0, 0
+    rel = np.abs(np.abs(val) - np.abs(ref)) / np.abs(ref)
+    ph = np.abs(np.angle(val * np.conj(ref)))
+    return float(rel.max()), float(ph.max()), int(((rel > snr_rtol) | (ph > phase_atol)).sum())
+
+
+def compare_candidates(got, oracle_result, n_bins, thr1, tau=TAU, snr_rtol=1e-3, phase_atol=1e-3):
+    """First-stage candidate sets, two-sided and value-checked, same rule as the triggers:
+      mandatory M = oracle bins with |rho_bar|/thr1 - 1 >  tau   (from oracle_result['candidates'])
+      allowed   A = oracle bins with |rho_bar|/thr1 - 1 > -tau   (from oracle_result['cand_near'])
+      pass iff M subset-of GOT subset-of A, no duplicates, and every reported averaged SNR is within 1e-3 (relative
+      modulus) and 1e-3 rad of the oracle's rho_bar of that bin.
+    `got` has fields template, bin, re, im."""
     cand = oracle_result["candidates"]
-    mod = np.hypot(cand["re"], cand["im"])
-    man = cand[mod / thr1 - 1.0 > tau]
+    near = oracle_result["cand_near"]
+    man = cand[np.hypot(cand["re"], cand["im"]) / thr1 - 1.0 > tau]
+    allowed = near[np.hypot(near["re"], near["im"]) / thr1 - 1.0 > -tau]
     k_got = _keys(got["template"], got["bin"], n_bins)
     k_man = _keys(man["template"], man["bin"], n_bins)
+    k_all = _keys(allowed["template"], allowed["bin"], n_bins)
+    dup = len(k_got) - len(np.unique(k_got))
     missing = np.setdiff1d(k_man, k_got)
-    return {"n_got": int(len(k_got)), "n_oracle": int(len(cand)), "n_missing": int(len(missing)),
-            "ok": len(missing) == 0}
+    extra = np.setdiff1d(k_got, k_all)
+    max_rel, max_phase, bad_val = _match_values(k_got, got["re"], got["im"], k_all, allowed["re"], allowed["im"],
+                                                snr_rtol, phase_atol)
+    ok = dup == 0 and len(missing) == 0 and len(extra) == 0 and bad_val == 0
+    return {"ok": bool(ok), "n_got": int(len(k_got)), "n_oracle": int(len(cand)), "n_mandatory": int(len(k_man)),
+            "n_allowed": int(len(k_all)), "n_missing": int(len(missing)), "n_extra": int(len(extra)),
+            "n_duplicates": int(dup), "n_bad_values": bad_val, "max_rel_err": max_rel, "max_phase_err": max_phase}

@@ -180,6 +180,8 @@ def oracle_filter(strain, basis, coeffs, sigma, N, fs, f_low, w, thr1, thr2, tem
       n_flat     number of flat triggers |rho| >= thr2 over the same templates
       near       structured array of every (template, time, re, im, avg_abs) with
                  |rho| >= thr2 (1 - 2e-3) and |rho_bar| >= thr1 (1 - 2e-3): superset used for the allowed set
+      cand_near  structured array (template, bin, re, im) of every bin with |rho_bar| >= thr1 (1 - 2e-3):
+                 superset of `candidates` used for the allowed set of the first stage (keep_margins only)
     """
     j_low, _ = band(N, fs, f_low)
     T = np.asarray(coeffs).shape[0]
@@ -187,7 +189,7 @@ def oracle_filter(strain, basis, coeffs, sigma, N, fs, f_low, w, thr1, thr2, tem
     trig_dt = np.dtype([("template", np.int64), ("time", np.int64), ("re", np.float64), ("im", np.float64),
                         ("avg_abs", np.float64)])
     cand_dt = np.dtype([("template", np.int64), ("bin", np.int64), ("re", np.float64), ("im", np.float64)])
-    trig_parts, cand_parts, near_parts = [], [], []
+    trig_parts, cand_parts, near_parts, cnear_parts = [], [], [], []
     n_flat = 0
     slack = 1.0 - 2e-3
     for a in range(0, len(tids), chunk):
@@ -209,6 +211,12 @@ def oracle_filter(strain, basis, coeffs, sigma, N, fs, f_low, w, thr1, thr2, tem
                 r["avg_abs"] = np.abs(rho_bar[trig // w])
                 trig_parts.append(r)
             if keep_margins:
+                cn = np.nonzero(np.abs(rho_bar) >= thr1 * slack)[0]
+                if len(cn):
+                    c = np.empty(len(cn), dtype=cand_dt)
+                    c["template"], c["bin"] = t, cn
+                    c["re"], c["im"] = rho_bar[cn].real, rho_bar[cn].imag
+                    cnear_parts.append(c)
                 mod = np.abs(rho[m])
                 nn = np.nonzero(mod >= thr2 * slack)[0]
                 nn = nn[np.abs(rho_bar[nn // w]) >= thr1 * slack]
@@ -220,7 +228,7 @@ def oracle_filter(strain, basis, coeffs, sigma, N, fs, f_low, w, thr1, thr2, tem
                     near_parts.append(r)
     cat = lambda parts, dt: np.concatenate(parts) if parts else np.empty(0, dtype=dt)
     return {"triggers": cat(trig_parts, trig_dt), "candidates": cat(cand_parts, cand_dt),
-            "near": cat(near_parts, trig_dt), "n_flat": n_flat}
+            "near": cat(near_parts, trig_dt), "cand_near": cat(cnear_parts, cand_dt), "n_flat": n_flat}
 
 
 def evaluate_points(strain, basis, coeffs, sigma, N, fs, f_low, w, template, times):

@@ -174,6 +174,23 @@ def test_single_bin_block(rbmf):
         check(rbmf, wl, 8, 1.5, 3.0, impl=impl, expect_triggers=False)
 
 
+@pytest.mark.parametrize("impl", [X3, SCREEN])
+def test_non_integer_band_edge_and_out_of_band_values_ignored(rbmf, impl):
+    """f_low N / fs = 121.2: the band starts at bin 122 (ceil).  Basis and strain carry garbage below the band and in
+    the Nyquist bin; the library must ignore it exactly as the oracle's definition does (include/rbmf.h, rbmf_set_basis)."""
+    wl = dict(workload("tiny", f_low=30.3, index=72))
+    cfg = wl["config"]
+    assert cfg.j_low == 122 and orc.band(cfg.N, cfg.fs, cfg.f_low) == (122, cfg.N // 2)
+    rng = np.random.default_rng(3)
+    basis, strain = wl["basis"].copy(), wl["strain"].copy()
+    basis[:, :122] = (rng.standard_normal((cfg.k, 122)) + 1j * rng.standard_normal((cfg.k, 122))).astype(np.complex64)
+    basis[:, cfg.N // 2] = 7.0
+    strain[:122] = strain[:122] * 3 + 50.0
+    strain[cfg.N // 2] = 1000.0
+    wl["basis"], wl["strain"] = basis, strain
+    check(rbmf, wl, 4, 3.0, 4.0, impl=impl)
+
+
 def test_mini_simt_and_tensor_core_candidates_agree(rbmf):
     """The three stage-1 implementations give the same candidate list (threshold ties aside), and the screen's
     superset really contains it with a modest overhead."""

@@ -93,6 +93,48 @@ def test_direct_and_fft_routes_match_time_domain_bruteforce():
     assert np.abs(orc.snr_series_fft(d, u, 2.5, N, j_low) * 2.5 - ref).max() < 1e-11
 
 
+def test_band_edges_with_non_integer_cutoff():
+    """Band = [ceil(f_low N / fs), N/2): with f_low N / fs = 9.3 the first bin is 10 (not 9), and the Nyquist bin is
+    excluded (PAPER.md:175-177 filters above the lower cutoff only).  The reference writes the band
+    out by hand in a time-domain correlation; the template has power in bin 9 and in the Nyquist bin, so a floor
+    instead of a ceil, or an inclusive upper edge, changes the result by O(1)."""
+    N, fs, f_low = 128, 128.0, 9.3
+    assert orc.band(N, fs, f_low) == (10, 64)
+    assert orc.band(N, fs, 9.0) == (9, 64) and orc.band(N, fs, 8.999999) == (9, 64) and orc.band(N, fs, 9.0001) == (10, 64)
+    assert wlm.band_start(N, fs, f_low) == 10            # the generator's own statement of the same edge
+    rng = np.random.default_rng(11)
+    x = rng.standard_normal(N)
+    u = rng.standard_normal(N // 2 + 1) + 1j * rng.standard_normal(N // 2 + 1)      # power in EVERY bin 0..N/2
+    d = np.fft.rfft(x)
+    # time-domain circular correlation with the band-limited template, band written out: bins 10..63
+    q = np.zeros(N, dtype=np.complex128)
+    for m in range(N):
+        for j in range(10, 64):
+            q[m] += u[j] * np.exp(2j * math.pi * ((j * m) % N) / N)
+    ref = np.array([math.sqrt(2.0 / N) * sum(x[m] * np.conj(q[(m - n) % N]) for m in range(N)) for n in range(N)])
+    j_low, _ = orc.band(N, fs, f_low)
+    assert np.abs(orc.snr_series_fft(d, u, 1.0, N, j_low) - ref).max() < 1e-11
+    assert np.abs(orc.snr_series_direct(d, u, 1.0, N, j_low) - ref).max() < 1e-11
+    assert abs(orc.snr_point(d, u, 1.0, N, j_low, 5) - ref[5]) < 1e-11
+    assert np.abs(orc.averaged_series_eq12(d, u, 1.0, N, j_low, 4) - ref.reshape(-1, 4).mean(axis=1)).max() < 1e-11
+    # sensitivity of the pin: the neighbouring readings differ at O(0.1-1)
+    assert np.abs(orc.snr_series_fft(d, u, 1.0, N, 9) - ref).max() > 1e-2
+    # whole path: oracle_filter derives the band from (fs, f_low) itself
+    B = np.zeros((1, N // 2 + 1), dtype=np.complex64)
+    B[0] = (u / np.linalg.norm(u[10:64])).astype(np.complex64)
+    res = orc.oracle_filter(d.astype(np.complex64), B, np.ones((1, 1), dtype=np.complex64), np.ones(1, dtype=np.float32),
+                            N, fs, f_low, 1, 1.0, 1.0)
+    d32 = d.astype(np.complex64).astype(np.complex128)
+    q2 = np.zeros(N, dtype=np.complex128)
+    for m in range(N):
+        for j in range(10, 64):
+            q2[m] += B[0, j].astype(np.complex128) * np.exp(2j * math.pi * ((j * m) % N) / N)
+    x32 = np.fft.irfft(d32, n=N)
+    ref2 = np.array([math.sqrt(2.0 / N) * sum(x32[m] * np.conj(q2[(m - n) % N]) for m in range(N)) for n in range(N)])
+    exp = [n for n in range(N) if abs(ref2[n]) >= 1.0]
+    assert len(exp) > 5 and res["triggers"]["time"].tolist() == exp
+
+
 def test_direct_vs_fft_on_tiny(tiny):
     cfg = tiny["config"]
     h = orc.reconstructed_templates(tiny["coeffs"], tiny["basis"], [3, 40])
