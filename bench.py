@@ -133,8 +133,8 @@ def main():
     ap.add_argument("--config", default="paper")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--w", type=int, default=None, help="override the averaging window")
-    ap.add_argument("--gemm", default="screen", choices=["screen", "bf16x3", "simt"],
-                    help="stage-1 kernel: fp16 screen + fp32 confirm (library default), bf16x3, or the fp32 check kernel")
+    ap.add_argument("--gemm", default="screen", choices=["screen", "bf16x3"],
+                    help="stage-1 kernel: fp16 screen + fp32 confirm (library default) or bf16x3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -183,7 +183,7 @@ def main():
     strain_np, _ = workloads.make_strain(wl, seg)
     stream = torch.cuda.Stream(device=device)
     with torch.cuda.stream(stream):
-        impls = {"screen": rbmf.RBMF_GEMM_SCREEN, "bf16x3": rbmf.RBMF_GEMM_TCGEN05, "simt": rbmf.RBMF_GEMM_SIMT}
+        impls = {"screen": rbmf.RBMF_GEMM_SCREEN, "bf16x3": rbmf.RBMF_GEMM_TCGEN05}
         strain_dev = torch.from_numpy(strain_np).to(device)
         strain_pinned = torch.from_numpy(strain_np).pin_memory()
         capacity = 1 << 22

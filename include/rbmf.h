@@ -64,10 +64,10 @@ typedef enum {
     RBMF_ERR_UNSUPPORTED = -5  /* valid but not implemented for this size / device                     */
 } rbmf_status;
 
-/* Stage-1 reconstruction kernels (rbmf_plan_set_gemm_impl). */
+/* Stage-1 reconstruction kernels (rbmf_plan_set_gemm_impl).  (Value 1 is not a product mode: it selects the
+ * verification kernel of the diagnostics section at the end of this header and is accepted only through it.) */
 typedef enum {
     RBMF_GEMM_TCGEN05 = 0, /* TMA + tcgen05.mma, bf16x3 split precision (fp32-equivalent) + TMEM epilogue          */
-    RBMF_GEMM_SIMT = 1,    /* plain fp32 CUDA-core kernel on the same operands; verification only                  */
     RBMF_GEMM_SCREEN = 2   /* default: the same tensor-core kernel with ONE fp16 product per term and thr_stage1
                               lowered, per (bin, template block), by a rigorous bound of the fp16 error, so its
                               output is a superset of the true candidates; kernel 3 then repeats the stage-1 test at
@@ -76,10 +76,11 @@ typedef enum {
                               fp32 rounding at the threshold, one third of the tensor-core work.               */
 } rbmf_gemm_impl;
 
-/* Create a plan for segments of N samples (power of two, 2^10 <= N <= 2^20) at sampling rate fs [Hz],
+/* Create a plan for segments of N samples (power of two, 2^10 <= N <= 2^24) at sampling rate fs [Hz],
  * lower cutoff f_low [Hz] (0 < f_low < fs/2), k basis vectors (multiple of 16, 16 <= k <= 1024) and T >= 1
  * templates.  Band = bins [ceil(f_low N / fs), N/2).  Host-only; no device work.  Defaults: w = 8,
- * max_candidates = max_triggers = 2^22.  *out is set to NULL on failure. */
+ * max_candidates = max_triggers = 2^22.  *out is set to NULL on failure.  Segments longer than 2^20 samples are a
+ * valid request that this build does not implement (the FFT is two passes of length <= 1024): RBMF_ERR_UNSUPPORTED. */
 rbmf_status rbmf_plan_create(rbmf_plan** out, int64_t N, double fs, double f_low, int32_t k, int32_t T);
 
 /* Stage-1 averaging window w of Eq. 9 (power of two, 1 <= w <= 32, N/w >= 128).  w = 1 is the flat search.
@@ -90,9 +91,7 @@ rbmf_status rbmf_plan_set_window(rbmf_plan* plan, int32_t w);
  * before rbmf_workspace_bytes / rbmf_plan_set_workspace. */
 rbmf_status rbmf_plan_set_capacity(rbmf_plan* plan, int64_t max_candidates, int64_t max_triggers);
 
-/* Select the stage-1 kernel (default RBMF_GEMM_SCREEN).  May be called at any time.
- * (Diagnostics: with the environment variable RBMF_NO_CLUSTER set when rbmf_plan_set_workspace runs, screen mode uses
- * its single-CTA kernel instead of the 2-CTA cluster kernel that multicasts the coefficient tile.) */
+/* Select the stage-1 kernel (RBMF_GEMM_SCREEN, the default, or RBMF_GEMM_TCGEN05).  May be called at any time. */
 rbmf_status rbmf_plan_set_gemm_impl(rbmf_plan* plan, int32_t impl);
 
 /* Bytes of device workspace the plan needs (depends on N, k, T, w, capacities). */
@@ -112,7 +111,8 @@ rbmf_status rbmf_set_basis(rbmf_plan* plan, const void* basis_dev);
 
 /* coeffs_dev: T x k complex64, row-major: c_tk, unconjugated.  sigma_dev: T float32 template
  * norms sigma_t > 0, or NULL => sigma_t = ||c_t||_2.  Copied (conjugated, scaled by 1/sigma_t, split into bf16
- * hi/lo planes) into the workspace. */
+ * hi/lo planes) into the workspace.  A template whose sigma_t is not a positive finite number (or, with NULL, whose
+ * coefficients are all zero) is disabled: it produces no candidates and no triggers. */
 rbmf_status rbmf_set_coeffs(rbmf_plan* plan, const void* coeffs_dev, const float* sigma_dev);
 
 /* Filter one segment.  strain_dev: (N/2+1) complex64, the unnormalised forward DFT of the whitened strain.
@@ -130,9 +130,14 @@ rbmf_status rbmf_filter_host(rbmf_plan* plan, const void* strain_host, float thr
                              rbmf_trigger* out_host, int64_t capacity_out, int64_t* n_out_host);
 
 /* Counts of the last rbmf_filter (synchronises the stream).  RBMF_ERR_OVERFLOW if a capacity was exceeded
- * (in RBMF_GEMM_SCREEN mode the capacity max_candidates applies to the screened superset, while *n_candidates
- * reports the candidates confirmed at fp32 accuracy). */
+ * (in RBMF_GEMM_SCREEN mode the capacity max_candidates applies to the screened superset, see
+ * rbmf_get_screened_count, while *n_candidates reports the candidates confirmed at fp32 accuracy). */
 rbmf_status rbmf_get_counts(rbmf_plan* plan, int64_t* n_candidates, int64_t* n_triggers);
+
+/* Number of entries kernel 2 asked to write to the stage-1 list in the last rbmf_filter (synchronises): the number
+ * max_candidates must hold.  In RBMF_GEMM_SCREEN mode this is the screened superset (>= the confirmed candidates of
+ * rbmf_get_counts); in RBMF_GEMM_TCGEN05 mode it equals *n_candidates. */
+rbmf_status rbmf_get_screened_count(rbmf_plan* plan, int64_t* n_screened);
 
 /* Copy up to `capacity` first-stage candidates of the last rbmf_filter to out_host (synchronises).
  * *n_out = total candidates found. */
@@ -144,6 +149,11 @@ rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64
  *   which = 1 / 2: beta^avg hi / lo plane, bfloat16, [ceil(k/32) K blocks][N/w bins][32 columns][re, im]
  *                  (value = hi + lo; columns >= k of the last block are zero).  In RBMF_GEMM_SCREEN mode plane 1
  *                  holds ONE float16 rounding of beta^avg in the same layout and plane 2 is stale.
+ *   which = 3: the stage-1 list as kernel 2 wrote it (rbmf_candidate records, min(rbmf_get_screened_count,
+ *              max_candidates) valid entries; *bytes = capacity in bytes).  In RBMF_GEMM_SCREEN mode avg_re/avg_im are
+ *              the raw one-product fp16 tensor-core values R_16 the screen tested;
+ *   which = 4: bin_norm, float32[N/w]: the upper bounds of ||beta^avg[i]||_2 the screen's error bound used;
+ *   which = 5: tnorm_blk, float32[ceil(T/128)]: max_t ||c_t||_2 / sigma_t per block of 128 templates.
  * *dev_ptr receives the address, *bytes the size. */
 rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_ptr, size_t* bytes);
 
@@ -161,6 +171,17 @@ rbmf_status rbmf_plan_destroy(rbmf_plan* plan);
 const char* rbmf_status_string(rbmf_status status);
 /* Last cudaError_t / CUresult seen by this plan (0 if none). */
 int32_t rbmf_last_cuda_error(const rbmf_plan* plan);
+
+/* ---- Diagnostics: test-only switches, not product modes -------------------------------------------------------
+ * rbmf_diag_set(plan, option, value), any time after rbmf_plan_create:
+ *   RBMF_DIAG_STAGE1_FP32_CHECK (value 0/1): run steps a4-a5 with a plain fp32 CUDA-core kernel on the bf16 hi + lo
+ *       operands instead of the tensor-core kernel selected by rbmf_plan_set_gemm_impl (cross-check of the two
+ *       tensor-core kernels against ordinary arithmetic; orders of magnitude slower);
+ *   RBMF_DIAG_SINGLE_CTA_SCREEN (value 0/1): RBMF_GEMM_SCREEN uses its single-CTA kernel instead of the 2-CTA
+ *       cluster kernel that multicasts the coefficient tile (the fallback for devices that cannot co-schedule
+ *       clusters of 2); takes effect at the next rbmf_filter. */
+typedef enum { RBMF_DIAG_STAGE1_FP32_CHECK = 1, RBMF_DIAG_SINGLE_CTA_SCREEN = 2 } rbmf_diag_option;
+rbmf_status rbmf_diag_set(rbmf_plan* plan, int32_t option, int32_t value);
 
 #ifdef __cplusplus
 }

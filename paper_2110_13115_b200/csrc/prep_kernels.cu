@@ -131,7 +131,8 @@ __global__ void prep_coeffs_kernel(const float2* __restrict__ coeffs, const floa
             inv_sigma = s > 0.0 ? (float)(1.0 / sqrt(s)) : 0.f;
         }
     } else if (threadIdx.x == 0) {
-        inv_sigma = 1.0f / sigma[t];
+        const float sg = sigma[t];
+        inv_sigma = (sg > 0.f && sg <= 3.0e38f) ? 1.0f / sg : 0.f;   // not a positive finite norm: template disabled
     }
     __syncthreads();
     const float is = inv_sigma;

@@ -35,6 +35,7 @@ struct rbmf_plan {
     int64_t max_cand, max_trig;
     int gemm_impl;
     int last_impl;      // gemm_impl of the last rbmf_filter (decides which candidate list / counter is final)
+    int diag_fp32_check, diag_single_cta;   // rbmf_diag_set
     int timing;
     cudaStream_t stream;
     uint8_t* ws;
@@ -163,10 +164,11 @@ extern "C" {
 rbmf_status rbmf_plan_create(rbmf_plan** out, int64_t N, double fs, double f_low, int32_t k, int32_t T) {
     if (!out) return RBMF_ERR_ARG;
     *out = nullptr;
-    if (N < 1024 || N > (int64_t(1) << 20) || (N & (N - 1)) != 0) return RBMF_ERR_ARG;
+    if (N < 1024 || N > (int64_t(1) << 24) || (N & (N - 1)) != 0) return RBMF_ERR_ARG;
     if (!(fs > 0.0) || !(f_low > 0.0) || !(f_low < fs / 2)) return RBMF_ERR_ARG;
     if (k < 16 || k > 1024 || (k % 16) != 0) return RBMF_ERR_ARG;
     if (T < 1 || T > (1 << 24)) return RBMF_ERR_ARG;
+    if (N > (int64_t(1) << 20)) return RBMF_ERR_UNSUPPORTED;   // valid, but the FFT is two passes of length <= 1024
     rbmf_plan* p = new (std::nothrow) rbmf_plan;
     if (!p) return RBMF_ERR_ARG;
     memset(p, 0, sizeof(*p));
@@ -207,7 +209,7 @@ rbmf_status rbmf_plan_set_capacity(rbmf_plan* plan, int64_t max_candidates, int6
 
 rbmf_status rbmf_plan_set_gemm_impl(rbmf_plan* plan, int32_t impl) {
     if (!plan) return RBMF_ERR_ARG;
-    if (impl != RBMF_GEMM_TCGEN05 && impl != RBMF_GEMM_SIMT && impl != RBMF_GEMM_SCREEN) return RBMF_ERR_ARG;
+    if (impl != RBMF_GEMM_TCGEN05 && impl != RBMF_GEMM_SCREEN) return RBMF_ERR_ARG;
     plan->gemm_impl = impl;
     return RBMF_OK;
 }
@@ -234,10 +236,11 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     CK(cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev));
     if (major != 10) return RBMF_ERR_UNSUPPORTED;   // sm_100a only: tcgen05 / TMEM
     CK(cudaDeviceGetAttribute(&plan->num_sms, cudaDevAttrMultiProcessorCount, dev));
+    // the plan counts as ready only when every step below has succeeded
+    plan->have_ws = plan->have_maps = false;
+    plan->have_basis = plan->have_coeffs = plan->filtered = false;
     plan->ws = (uint8_t*)dev_ptr;
     plan->ws_bytes = bytes;
-    plan->have_ws = true;
-    plan->have_basis = plan->have_coeffs = plan->filtered = false;
     const Layout& L = plan->lay;
     CK(launch_init_tables(at<float2>(plan, L.tw1_a), at<float2>(plan, L.tw1_b), at<float2>(plan, L.twN), plan->logN1,
                           plan->logN2, plan->stream));
@@ -264,12 +267,12 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     if ((s = make_map_rows(plan, &plan->tmB_h16, plan->ws + L.c_h16, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
     if ((s = make_map_rows(plan, &plan->tmB_h16half, plan->ws + L.c_h16, 2 * (uint64_t)plan->Tpad, k2, kGemmTT)) != RBMF_OK) return s;
     CK(gemm_screen_pair_clusters(plan->num_sms, &plan->pair_clusters));
-    if (getenv("RBMF_NO_CLUSTER")) plan->pair_clusters = 0;
-    plan->have_maps = true;
     if (!plan->have_events) {
         for (int i = 0; i < 5; ++i) CK(cudaEventCreate(&plan->ev[i]));
         plan->have_events = true;
     }
+    plan->have_maps = true;
+    plan->have_ws = true;
     return RBMF_OK;
 }
 
@@ -317,7 +320,7 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     a.plane_hi = at<uint16_t>(plan, L.bavg_hi); a.plane_lo = at<uint16_t>(plan, L.bavg_lo);
     a.sched = at<unsigned>(plan, L.sched);
     a.N = plan->N; a.M = (int)plan->M; a.nchunk = plan->k / kFftC; a.w = plan->w; a.inv_w = 1.0f / (float)plan->w;
-    const bool screen = plan->gemm_impl == RBMF_GEMM_SCREEN;
+    const bool screen = plan->gemm_impl == RBMF_GEMM_SCREEN && !plan->diag_fp32_check;
     a.plane_fp16 = screen ? 1 : 0;
     {
         // Pass-1 lookahead: a chunk's pass 2 needs ALL of its pass-1 tiles, so enough pass-1 tiles of later chunks
@@ -348,19 +351,26 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     g.num_ib = (int)(plan->M / kGemmBM);
     g.group = 32;   // template blocks per raster group: 32 coefficient tiles (8 MB fp16) stay L2-resident
     if (screen) {
-        // Rigorous bound of |R_fp16 - R| for the one-product fp16 screen (derivation: gemm_tcgen05.cu header):
-        // operand rounding u = 2^-11 relative (+ eta = 2^-25 sqrt(2) absolute per complex value in the subnormal
-        // range), fp32 accumulation of 2k exact products bounded by (2k + 64) 2^-22 sqrt(2) relative to ||a|| ||b||.
+        // Bound of |R_fp16 - R| for the one-product fp16 screen (derivation: gemm_tcgen05.cu header): operand
+        // rounding u = 2^-11 relative (+ eta = 2^-25 sqrt(2) absolute per complex value in the subnormal range), fp32
+        // accumulation of the 2k exact products in the tensor core taken as (2k + 64) 2^-22 sqrt(2) relative to
+        // ||a|| ||b|| (an assumption about the hardware's accumulator, checked against the oracle on the device by
+        // tests/test_gpu_screen.py).  On top, kappa1 carries the fp32 rounding of the CONFIRM step in kernel 3 -- a
+        // dot product of 2k real terms per component and the mean of w of them, gamma = (2k + w + 8) 2^-24 sqrt(2)
+        // relative to ||a|| times the row norm, for which the bin norm stands in -- so that whatever the confirm
+        // accepts, the screen has passed; `slack` covers the rounding of this threshold arithmetic itself.
         const double u = ldexp(1.0, -11), eta = ldexp(1.0, -25) * 1.4142135623730951;
         const double k = (double)plan->k;
         g.bin_norm = at<float>(plan, L.bin_norm);
         g.tnorm_blk = at<float>(plan, L.tnorm_blk);
         g.thr1 = thr_stage1;
-        g.kappa1 = (float)((2.0 * u + u * u + (2.0 * k + 64.0) * ldexp(1.0, -22) * 1.4142135623730951) * 1.001);
+        const double confirm = (2.0 * k + (double)plan->w + 8.0) * ldexp(1.0, -24) * 1.4142135623730951;
+        g.kappa1 = (float)((2.0 * u + u * u + (2.0 * k + 64.0) * ldexp(1.0, -22) * 1.4142135623730951 + confirm) * 1.001);
         g.kappa2 = (float)(eta * sqrt(k) * 1.001);
-        g.slack = 1e-4f;   // fp32 rounding of the confirm step and of this threshold arithmetic
-        CK(launch_gemm_screen(plan->tmA_hi, plan->tmB_h16, plan->tmB_h16half, plan->pair_clusters, g, plan->num_sms, st));
-    } else if (plan->gemm_impl == RBMF_GEMM_TCGEN05) {
+        g.slack = 1e-4f;
+        CK(launch_gemm_screen(plan->tmA_hi, plan->tmB_h16, plan->tmB_h16half,
+                              plan->diag_single_cta ? 0 : plan->pair_clusters, g, plan->num_sms, st));
+    } else if (!plan->diag_fp32_check) {
         CK(launch_gemm_tcgen05(plan->tmA_hi, plan->tmA_lo, plan->tmB_hi, plan->tmB_lo, g, plan->num_sms, st));
     } else {
         CK(launch_gemm_simt(at<uint16_t>(plan, L.bavg_hi), at<uint16_t>(plan, L.bavg_lo), at<uint16_t>(plan, L.c_hi),
@@ -380,7 +390,7 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     CK(cudaMemcpyAsync(n_out_dev, counters + 1, 8, cudaMemcpyDeviceToDevice, st));
     if (tm) CK(cudaEventRecord(plan->ev[3], st));
     plan->filtered = true;
-    plan->last_impl = plan->gemm_impl;
+    plan->last_impl = screen ? (int)RBMF_GEMM_SCREEN : (int)RBMF_GEMM_TCGEN05;
     return RBMF_OK;
 }
 
@@ -396,6 +406,25 @@ rbmf_status rbmf_get_counts(rbmf_plan* plan, int64_t* n_candidates, int64_t* n_t
     if (n_triggers) *n_triggers = (int64_t)h[1];
     if ((int64_t)h[0] > plan->max_cand || (int64_t)h[1] > plan->max_trig) return RBMF_ERR_OVERFLOW;
     return RBMF_OK;
+}
+
+rbmf_status rbmf_get_screened_count(rbmf_plan* plan, int64_t* n_screened) {
+    if (!plan || !n_screened) return RBMF_ERR_ARG;
+    if (!plan->filtered) return RBMF_ERR_STATE;
+    unsigned long long h = 0;
+    CK(cudaMemcpyAsync(&h, plan->ws + plan->lay.counters, 8, cudaMemcpyDeviceToHost, plan->stream));
+    CK(cudaStreamSynchronize(plan->stream));
+    *n_screened = (int64_t)h;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_diag_set(rbmf_plan* plan, int32_t option, int32_t value) {
+    if (!plan) return RBMF_ERR_ARG;
+    switch (option) {
+        case RBMF_DIAG_STAGE1_FP32_CHECK: plan->diag_fp32_check = value ? 1 : 0; return RBMF_OK;
+        case RBMF_DIAG_SINGLE_CTA_SCREEN: plan->diag_single_cta = value ? 1 : 0; return RBMF_OK;
+        default: return RBMF_ERR_ARG;
+    }
 }
 
 rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64_t capacity, int64_t* n_out) {
@@ -449,6 +478,9 @@ rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_p
         case 0: *dev_ptr = plan->ws + L.beta; *bytes = (size_t)plan->N * plan->k * 8; break;
         case 1: *dev_ptr = plan->ws + L.bavg_hi; *bytes = L.plane_bytes; break;
         case 2: *dev_ptr = plan->ws + L.bavg_lo; *bytes = L.plane_bytes; break;
+        case 3: *dev_ptr = plan->ws + L.cand; *bytes = (size_t)plan->max_cand * sizeof(rbmf_candidate); break;
+        case 4: *dev_ptr = plan->ws + L.bin_norm; *bytes = (size_t)plan->M * 4; break;
+        case 5: *dev_ptr = plan->ws + L.tnorm_blk; *bytes = (size_t)(plan->Tpad / kGemmTT) * 4; break;
         default: return RBMF_ERR_ARG;
     }
     return RBMF_OK;
@@ -474,7 +506,7 @@ rbmf_status rbmf_get_stage_ms(rbmf_plan* plan, float ms[4]) {
 rbmf_status rbmf_launches_per_filter(const rbmf_plan* plan, int32_t* n) {
     if (!plan || !n) return RBMF_ERR_ARG;
     // prep_strain + fused FFT + (screen: bin norms) + GEMM + stage 2
-    *n = plan->gemm_impl == RBMF_GEMM_SCREEN ? 5 : 4;
+    *n = (plan->gemm_impl == RBMF_GEMM_SCREEN && !plan->diag_fp32_check) ? 5 : 4;
     return RBMF_OK;
 }
 

@@ -1,5 +1,5 @@
 // Kernel 3 (step a6): re-score every first-stage candidate at full time resolution and fp32 accuracy
-// (PAPER.md:180, :191, :230, :246), plus the plain fp32 verification version of kernel 2 (RBMF_GEMM_SIMT).
+// (PAPER.md:180, :191, :230, :246), plus the plain fp32 verification version of kernel 2 (RBMF_DIAG_STAGE1_FP32_CHECK).
 #include <cuda_bf16.h>
 
 #include "rbmf_internal.h"
@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(const uint16_t* __restri
     __shared__ float sA[TI][KB + 1];       // beta^avg rows (time bins) x K
     __shared__ float sRe[TT][KB + 1];      // template "re" rows
     __shared__ float sIm[TT][KB + 1];      // template "im" rows
-    const int i0 = blockIdx.x * TI, t0 = blockIdx.y * TT;
+    const int i0 = blockIdx.y * TI, t0 = blockIdx.x * TT;   // templates on grid.x (up to 2^24 of them)
     const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;   // 16 x 16 threads, 4 x 4 outputs each
     float re[4][4] = {}, im[4][4] = {};
     for (int k0 = 0; k0 < g.k2; k0 += KB) {
@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(const uint16_t* __restri
 
 cudaError_t launch_gemm_simt(const uint16_t* a_hi, const uint16_t* a_lo, const uint16_t* c_hi, const uint16_t* c_lo,
                              const GemmArgs& g, cudaStream_t st) {
-    dim3 grid((unsigned)((g.M + 63) / 64), (unsigned)(g.num_tb * kGemmTT / 64));
+    dim3 grid((unsigned)(g.num_tb * kGemmTT / 64), (unsigned)((g.M + 63) / 64));
     gemm_simt_kernel<<<grid, 256, 0, st>>>(a_hi, a_lo, c_hi, c_lo, g);
     return cudaGetLastError();
 }

@@ -23,7 +23,8 @@ if not os.path.exists(LIB_PATH):
 _lib = ctypes.CDLL(LIB_PATH)
 
 RBMF_OK, RBMF_ERR_ARG, RBMF_ERR_STATE, RBMF_ERR_CUDA, RBMF_ERR_OVERFLOW, RBMF_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
-RBMF_GEMM_TCGEN05, RBMF_GEMM_SIMT, RBMF_GEMM_SCREEN = 0, 1, 2
+RBMF_GEMM_TCGEN05, RBMF_GEMM_SCREEN = 0, 2
+RBMF_DIAG_STAGE1_FP32_CHECK, RBMF_DIAG_SINGLE_CTA_SCREEN = 1, 2
 
 TRIGGER_DTYPE = np.dtype([("template", np.int32), ("time", np.int32), ("re", np.float32), ("im", np.float32)])
 CANDIDATE_DTYPE = np.dtype([("template", np.int32), ("bin", np.int32), ("re", np.float32), ("im", np.float32)])
@@ -44,6 +45,7 @@ SIGNATURES = {
     "rbmf_filter": (_i32, [_vp, _vp, _f32, _f32, _vp, _vp]),
     "rbmf_filter_host": (_i32, [_vp, _vp, _f32, _f32, _vp, _i64, _pi64]),
     "rbmf_get_counts": (_i32, [_vp, _pi64, _pi64]),
+    "rbmf_get_screened_count": (_i32, [_vp, _pi64]),
     "rbmf_get_candidates": (_i32, [_vp, _vp, _i64, _pi64]),
     "rbmf_get_internal": (_i32, [_vp, _i32, ctypes.POINTER(_vp), _psz]),
     "rbmf_plan_set_timing": (_i32, [_vp, _i32]),
@@ -52,6 +54,7 @@ SIGNATURES = {
     "rbmf_plan_destroy": (_i32, [_vp]),
     "rbmf_status_string": (ctypes.c_char_p, [_i32]),
     "rbmf_last_cuda_error": (_i32, [_vp]),
+    "rbmf_diag_set": (_i32, [_vp, _i32, _i32]),
 }
 for _name, (_res, _args) in SIGNATURES.items():
     _fn = getattr(_lib, _name)          # AttributeError here = library does not export what rbmf.h declares
@@ -76,7 +79,12 @@ def _ptr(t):
 
 
 class Plan:
-    """Owns an rbmf_plan and its workspace tensor.  All tensors handed in must live on the plan's CUDA device."""
+    """Owns an rbmf_plan and its workspace tensor.  All tensors handed in must live on the plan's CUDA device.
+
+    Stream discipline: the library enqueues on the plan's stream only.  Every copy this wrapper makes (host -> device
+    staging of inputs, device -> host read-back of results) is issued on that same stream, and a tensor the caller
+    produced on another stream is ordered before its first use here (`_order_after_current`), so a `Plan(stream=s)`
+    works whether or not the caller has made `s` torch's current stream."""
 
     def __init__(self, N, fs, f_low, k, T, w=8, max_candidates=1 << 22, max_triggers=1 << 22, device="cuda:0",
                  stream=None):
@@ -86,6 +94,8 @@ class Plan:
         self.max_candidates, self.max_triggers = int(max_candidates), int(max_triggers)
         self.device = torch.device(device)
         self._h = _vp()
+        self.stream = None
+        self._fp32_check = False
         self._check(_lib.rbmf_plan_create(ctypes.byref(self._h), self.N, self.fs, self.f_low, self.k, self.T),
                     "rbmf_plan_create")
         self._check(_lib.rbmf_plan_set_window(self._h, self.w), "rbmf_plan_set_window")
@@ -98,9 +108,11 @@ class Plan:
             self._ws = torch.empty(self.workspace_bytes + 1024, dtype=torch.uint8, device=self.device)
             base = (self._ws.data_ptr() + 1023) // 1024 * 1024
             self.set_stream(stream)
-            self._check(_lib.rbmf_plan_set_workspace(self._h, base, self.workspace_bytes), "rbmf_plan_set_workspace")
-            self._out = torch.empty(self.max_triggers * 4, dtype=torch.int32, device=self.device)
-            self._n_out = torch.zeros(1, dtype=torch.int64, device=self.device)
+            with torch.cuda.stream(self.stream):
+                self._check(_lib.rbmf_plan_set_workspace(self._h, base, self.workspace_bytes),
+                            "rbmf_plan_set_workspace")
+                self._out = torch.empty(self.max_triggers * 4, dtype=torch.int32, device=self.device)
+                self._n_out = torch.zeros(1, dtype=torch.int64, device=self.device)
         self._keep = []
         self.gemm_impl = RBMF_GEMM_SCREEN      # the library's default (include/rbmf.h)
 
@@ -112,23 +124,48 @@ class Plan:
         return status
 
     def set_stream(self, stream=None):
+        """Enqueue on `stream` from now on (default: torch's current stream).  Work already enqueued on the previous
+        stream (table initialisation, set_basis / set_coeffs, an earlier filter) is ordered before the new one."""
         torch = self._torch
         if stream is None:
             stream = torch.cuda.current_stream(self.device)
+        old = self.stream
+        if old is not None and old.cuda_stream != stream.cuda_stream:
+            ev = torch.cuda.Event()
+            ev.record(old)
+            stream.wait_event(ev)
         self.stream = stream
         self._check(_lib.rbmf_set_stream(self._h, _vp(stream.cuda_stream)), "rbmf_set_stream")
 
+    def _order_after_current(self):
+        """Make the plan's stream wait for what torch's current stream has enqueued so far (the producer of a tensor
+        the caller hands in), unless they are the same stream."""
+        cur = self._torch.cuda.current_stream(self.device)
+        if cur.cuda_stream != self.stream.cuda_stream:
+            self.stream.wait_stream(cur)
+
     def _dev(self, x, dtype):
+        """`x` as a contiguous tensor on the plan's device; the copy, if one is needed, runs on the plan's stream."""
         torch = self._torch
         t = torch.as_tensor(x)
         if t.dtype != dtype:
             raise TypeError("expected %s, got %s" % (dtype, t.dtype))
-        return t.to(self.device).contiguous()
+        self._order_after_current()
+        with torch.cuda.stream(self.stream):
+            t = t.to(self.device).contiguous()
+            t.record_stream(self.stream)
+        return t
 
     # -- ABI calls ---------------------------------------------------------------------------
     def set_gemm_impl(self, impl):
         self._check(_lib.rbmf_plan_set_gemm_impl(self._h, int(impl)), "rbmf_plan_set_gemm_impl")
         self.gemm_impl = int(impl)
+
+    def diag_set(self, option, value):
+        """Test-only switches (include/rbmf.h, diagnostics section)."""
+        self._check(_lib.rbmf_diag_set(self._h, int(option), int(value)), "rbmf_diag_set")
+        if int(option) == RBMF_DIAG_STAGE1_FP32_CHECK:
+            self._fp32_check = bool(value)
 
     def set_timing(self, enabled=True):
         self._check(_lib.rbmf_plan_set_timing(self._h, 1 if enabled else 0), "rbmf_plan_set_timing")
@@ -159,6 +196,7 @@ class Plan:
         torch = self._torch
         if strain_dev.dtype != torch.complex64 or strain_dev.numel() != self.N // 2 + 1 or not strain_dev.is_cuda:
             raise ValueError("strain must be a complex64 CUDA tensor with N/2+1 entries")
+        self._order_after_current()
         with torch.cuda.device(self.device):
             self._check(_lib.rbmf_filter(self._h, _ptr(strain_dev), float(thr1), float(thr2), _ptr(self._out),
                                          _ptr(self._n_out)), "rbmf_filter")
@@ -173,7 +211,8 @@ class Plan:
         """Synchronise and return the trigger list of the last filter call, sorted by (template, time)."""
         nc, nt, _ = self.counts(allow_overflow)
         n = min(nt, self.max_triggers)
-        raw = self._out[: 4 * n].cpu().numpy()
+        with self._torch.cuda.stream(self.stream):
+            raw = self._out[: 4 * n].cpu().numpy()
         trig = raw.view(TRIGGER_DTYPE).copy() if n else np.empty(0, dtype=TRIGGER_DTYPE)
         return np.sort(trig, order=("template", "time"))
 
@@ -194,6 +233,11 @@ class Plan:
                                        len(out_host), ctypes.byref(n))
         self._check(st, "rbmf_filter_host", allow=(RBMF_ERR_OVERFLOW,))
         return out_host[: min(n.value, len(out_host))], n.value
+
+    def screened_count(self):
+        n = _i64()
+        self._check(_lib.rbmf_get_screened_count(self._h, ctypes.byref(n)), "rbmf_get_screened_count")
+        return n.value
 
     def candidates(self):
         nc, _, _ = self.counts(allow_overflow=True)
@@ -217,12 +261,23 @@ class Plan:
             return self._ws[off: off + nb.value]
 
         C = 4   # columns per chunk of the library's chunk-blocked layouts (include/rbmf.h, rbmf_get_internal)
+        screen = self.gemm_impl == RBMF_GEMM_SCREEN and not self._fp32_check
+        if which == "screened":      # the stage-1 list as kernel 2 wrote it (raw fp16-product values in screen mode)
+            n = min(self.screened_count(), self.max_candidates)
+            with torch.cuda.stream(self.stream):
+                raw = view(3)[: 16 * n].cpu().numpy()
+            return raw.view(CANDIDATE_DTYPE).copy()
+        if which in ("bin_norm", "tnorm_blk"):
+            with torch.cuda.stream(self.stream):
+                return view(4 if which == "bin_norm" else 5).view(torch.float32).cpu().numpy()
         if which == "beta":
-            v = view(0).view(torch.float32).view(self.k // C, self.N, C, 2)          # [chunk][n][C]
-            return torch.view_as_complex(v.permute(1, 0, 2, 3).reshape(self.N, self.k, 2).contiguous()).cpu().numpy()
+            with torch.cuda.stream(self.stream):
+                v = view(0).view(torch.float32).view(self.k // C, self.N, C, 2)          # [chunk][n][C]
+                return torch.view_as_complex(
+                    v.permute(1, 0, 2, 3).reshape(self.N, self.k, 2).contiguous()).cpu().numpy()
         if which == "beta_avg":
             M, nkb = self.N // self.w, (self.k + 31) // 32
-            if self.gemm_impl == RBMF_GEMM_SCREEN:       # one fp16 plane
+            if screen:                                   # one fp16 plane
                 hi = view(1).view(torch.float16).to(torch.float32)
                 lo = torch.zeros_like(hi)
             else:

@@ -53,7 +53,10 @@ def test_plan_create_validates_arguments(binding):
     st, h = _create(b)
     assert st == b.RBMF_OK and h.value
     assert b.rbmf_plan_destroy(h) == b.RBMF_OK
-    for kw in (dict(N=4095), dict(N=512), dict(N=1 << 21), dict(k=20), dict(k=8), dict(k=2048), dict(T=0),
+    for N in (1 << 21, 1 << 24):      # valid by the contract (up to 2^24), not built: two FFT passes of <= 1024
+        st, h = _create(b, N=N)
+        assert st == b.RBMF_ERR_UNSUPPORTED and not h.value
+    for kw in (dict(N=4095), dict(N=512), dict(N=1 << 25), dict(k=20), dict(k=8), dict(k=2048), dict(T=0),
                dict(f_low=0.0), dict(f_low=600.0), dict(fs=-1.0)):
         st, h = _create(b, **kw)
         assert st == b.RBMF_ERR_ARG and not h.value, kw
@@ -84,9 +87,15 @@ def test_window_capacity_and_workspace_size(binding):
     assert b.rbmf_plan_set_window(h, 1) == b.RBMF_OK
     assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 5
     assert b.rbmf_plan_set_gemm_impl(h, 7) == b.RBMF_ERR_ARG
-    assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_SIMT) == b.RBMF_OK
+    assert b.rbmf_plan_set_gemm_impl(h, 1) == b.RBMF_ERR_ARG     # the fp32 check kernel is not a product mode
+    assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_TCGEN05) == b.RBMF_OK
     assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 4
     assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_SCREEN) == b.RBMF_OK
+    assert b.rbmf_diag_set(h, 99, 1) == b.RBMF_ERR_ARG
+    assert b.rbmf_diag_set(h, b.RBMF_DIAG_STAGE1_FP32_CHECK, 1) == b.RBMF_OK
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 4
+    assert b.rbmf_diag_set(h, b.RBMF_DIAG_STAGE1_FP32_CHECK, 0) == b.RBMF_OK
+    assert b.rbmf_get_screened_count(h, ctypes.byref(ctypes.c_int64())) == b.RBMF_ERR_STATE
     b.rbmf_plan_destroy(h)
 
 

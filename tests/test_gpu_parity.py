@@ -16,7 +16,8 @@ pytestmark = pytest.mark.gpu
 BETA_ATOL = 1e-5
 
 
-X3, SIMT, SCREEN = 0, 1, 2       # rbmf_gemm_impl (include/rbmf.h); SCREEN is the library default
+X3, SCREEN = 0, 2                # rbmf_gemm_impl (include/rbmf.h); SCREEN is the library default
+SIMT = "fp32-check"              # test-only: bf16x3 operands through the plain fp32 CUDA-core kernel (rbmf_diag_set)
 
 
 def beta_avg_close(got, ref, impl=X3):
@@ -45,13 +46,19 @@ def workload(name, **kw):
     return _WL[key]
 
 
+def set_impl(rbmf, plan, impl):
+    if impl is None:
+        return
+    plan.diag_set(rbmf.RBMF_DIAG_STAGE1_FP32_CHECK, 1 if impl == SIMT else 0)
+    plan.set_gemm_impl(X3 if impl == SIMT else impl)
+
+
 def make_plan(rbmf, wl, w=None, impl=None, **kw):
     import torch
     cfg = wl["config"]
     plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w if w is None else w,
                      max_candidates=kw.pop("max_candidates", 1 << 20), max_triggers=kw.pop("max_triggers", 1 << 20))
-    if impl is not None:
-        plan.set_gemm_impl(impl)
+    set_impl(rbmf, plan, impl)
     plan.set_basis(torch.from_numpy(wl["basis"]))
     plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
     return plan
@@ -63,11 +70,12 @@ def oracle(wl, w, thr1, thr2, templates=None):
                              thr1, thr2, templates=templates)
 
 
-def check(rbmf, wl, w, thr1, thr2, impl=SCREEN, expect_triggers=True):
+def check(rbmf, wl, w, thr1, thr2, impl=SCREEN, expect_triggers=True, single_cta=False):
     import torch
     cfg = wl["config"]
-    plan = make_plan(rbmf, wl, w=w)
-    plan.set_gemm_impl(impl)
+    plan = make_plan(rbmf, wl, w=w, impl=impl)
+    if single_cta:
+        plan.diag_set(rbmf.RBMF_DIAG_SINGLE_CTA_SCREEN, 1)
     got = plan.filter(torch.from_numpy(wl["strain"]), thr1, thr2)
     ref = oracle(wl, w, thr1, thr2)
     rep = compare.compare_triggers(got, ref, cfg.N, thr1, thr2)
@@ -91,7 +99,7 @@ def test_beta_matches_oracle_series(rbmf, name):
     plan.filter(torch.from_numpy(wl["strain"]), 50.0, 50.0)
     beta = plan.internal("beta")                       # (N, k)
     bavg = plan.internal("beta_avg")                   # (N/w, k)
-    plan.set_gemm_impl(SCREEN)
+    set_impl(rbmf, plan, SCREEN)
     plan.filter(torch.from_numpy(wl["strain"]), 50.0, 50.0)
     bavg16 = plan.internal("beta_avg")                 # the screen's single fp16 plane
     plan.close()
@@ -160,10 +168,9 @@ def test_mini_largest_window(rbmf):
     check(rbmf, workload("mini"), 32, 0.4, 3.0, impl=SCREEN, expect_triggers=False)
 
 
-def test_screen_single_cta_kernel(rbmf, monkeypatch):
+def test_screen_single_cta_kernel(rbmf):
     """The screen's fallback kernel (no thread-block clusters) gives the same lists as the 2-CTA one."""
-    monkeypatch.setenv("RBMF_NO_CLUSTER", "1")
-    check(rbmf, workload("mini"), 8, 3.5, 5.0, impl=SCREEN)
+    check(rbmf, workload("mini"), 8, 3.5, 5.0, impl=SCREEN, single_cta=True)
 
 
 def test_single_bin_block(rbmf):
@@ -227,7 +234,7 @@ def test_screen_superset_is_tight(rbmf):
     plan = make_plan(rbmf, wl, impl=SCREEN)
     plan.filter(torch.from_numpy(wl["strain"]), cfg.thr1, cfg.thr2)
     n_conf = plan.counts()[0]
-    plan.set_gemm_impl(X3)
+    set_impl(rbmf, plan, X3)
     plan.filter(torch.from_numpy(wl["strain"]), cfg.thr1 - 0.05, cfg.thr2)
     n_loose = plan.counts()[0]
     plan.filter(torch.from_numpy(wl["strain"]), cfg.thr1, cfg.thr2)
@@ -366,6 +373,32 @@ def test_non_default_stream(rbmf):
         plan.close()
     ref = oracle(wl, 4, 3.0, 4.0)
     assert compare.compare_triggers(a, ref, wl["config"].N, 3.0, 4.0)["ok"]
+
+
+def test_explicit_stream_without_entering_it(rbmf):
+    """Plan(stream=s) while torch's current stream is another one: the binding's staging copies and read-backs run on
+    the plan's stream and inputs produced on the current stream are ordered before their use."""
+    import torch
+    wl = workload("mini")
+    cfg = wl["config"]
+    st = torch.cuda.Stream()
+    plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, max_candidates=1 << 20, max_triggers=1 << 20,
+                     stream=st)
+    assert torch.cuda.current_stream().cuda_stream != st.cuda_stream
+    plan.set_basis(torch.from_numpy(wl["basis"]))
+    plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+    # the strain is produced by a kernel on the CURRENT stream right before the call (after a long-running fill)
+    big = torch.empty(1 << 28, dtype=torch.float32, device="cuda").normal_()
+    s = torch.from_numpy(wl["strain"]).cuda() * (1.0 + 0.0 * big[:1].sum())
+    plan.filter_async(s, 3.5, 5.0)
+    a = plan.triggers()
+    st2 = torch.cuda.Stream()
+    plan.set_stream(st2)                                   # ordered after the work on the old stream
+    b = plan.filter(torch.from_numpy(wl["strain"]), 3.5, 5.0)
+    plan.close()
+    ref = oracle(wl, cfg.w, 3.5, 5.0)
+    assert compare.compare_triggers(a, ref, cfg.N, 3.5, 5.0)["ok"]
+    assert np.array_equal(a, b)
 
 
 # ------------------------------------------------------------- full size, bench launch configuration
