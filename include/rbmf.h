@@ -153,7 +153,9 @@ rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64
  *              max_candidates) valid entries; *bytes = capacity in bytes).  In RBMF_GEMM_SCREEN mode avg_re/avg_im are
  *              the raw one-product fp16 tensor-core values R_16 the screen tested;
  *   which = 4: bin_norm, float32[N/w]: the upper bounds of ||beta^avg[i]||_2 the screen's error bound used;
- *   which = 5: tnorm_blk, float32[ceil(T/128)]: max_t ||c_t||_2 / sigma_t per block of 128 templates.
+ *   which = 5: tnorm_blk, float32[ceil(T/128)]: max_t ||c_t||_2 / sigma_t per block of 128 templates;
+ *   which = 6: the final first-stage candidate list of the last rbmf_filter on the device (what rbmf_get_candidates
+ *              copies; min(n_candidates, max_candidates) valid rbmf_candidate records; *bytes = capacity in bytes).
  * *dev_ptr receives the address, *bytes the size. */
 rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_ptr, size_t* bytes);
 

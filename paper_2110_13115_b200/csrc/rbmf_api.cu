@@ -481,6 +481,10 @@ rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_p
         case 3: *dev_ptr = plan->ws + L.cand; *bytes = (size_t)plan->max_cand * sizeof(rbmf_candidate); break;
         case 4: *dev_ptr = plan->ws + L.bin_norm; *bytes = (size_t)plan->M * 4; break;
         case 5: *dev_ptr = plan->ws + L.tnorm_blk; *bytes = (size_t)(plan->Tpad / kGemmTT) * 4; break;
+        case 6:
+            *dev_ptr = plan->ws + (plan->last_impl == RBMF_GEMM_SCREEN ? L.cand2 : L.cand);
+            *bytes = (size_t)plan->max_cand * sizeof(rbmf_candidate);
+            break;
         default: return RBMF_ERR_ARG;
     }
     return RBMF_OK;

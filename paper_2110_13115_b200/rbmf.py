@@ -216,6 +216,23 @@ class Plan:
         trig = raw.view(TRIGGER_DTYPE).copy() if n else np.empty(0, dtype=TRIGGER_DTYPE)
         return np.sort(trig, order=("template", "time"))
 
+    def triggers_device(self, allow_overflow=False):
+        """The trigger list of the last filter call as an (n, 4) int32 CUDA tensor (columns: template, time, and the
+        bit patterns of re, im), unsorted, without a device -> host copy: for callers that select on the device."""
+        nc, nt, _ = self.counts(allow_overflow)
+        n = min(nt, self.max_triggers)
+        return self._out[: 4 * n].view(n, 4)
+
+    def candidates_device(self):
+        """The first-stage candidate list of the last filter call as an (n, 4) int32 CUDA tensor (template, bin, bits
+        of avg_re, avg_im)."""
+        nc, _, _ = self.counts(allow_overflow=True)
+        n = min(nc, self.max_candidates)
+        p, nb = _vp(), ctypes.c_size_t()
+        self._check(_lib.rbmf_get_internal(self._h, 6, ctypes.byref(p), ctypes.byref(nb)), "rbmf_get_internal")
+        off = p.value - self._ws.data_ptr()
+        return self._ws[off: off + 16 * n].view(self._torch.int32).view(n, 4)
+
     def filter(self, strain, thr1, thr2, allow_overflow=False):
         torch = self._torch
         s = self._dev(strain, torch.complex64)

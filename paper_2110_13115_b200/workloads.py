@@ -90,8 +90,19 @@ CONFIGS = {
     "small_narrow": WorkloadConfig("small_narrow", 12, 131072, 2048.0, 25.0, 128, 2000, 8, 1.20, 1.25, 10, 6.0, 15.0),
     "paper": WorkloadConfig("paper", 3, 524288, 2048.0, 20.0, 256, 20000, 8, 1.0, 3.0, 50, 5.0, 20.0),
     "large": WorkloadConfig("large", 4, 262144, 4096.0, 20.0, 256, 100000, 8, 0.5, 5.0, 100, 5.0, 20.0),
-    "sweep_k256_T10000": WorkloadConfig("sweep_k256_T10000", 5, 1 << 20, 4096.0, 20.0, 256, 10000, 8, 1.0, 3.0, 0, 0.0, 0.0),
 }
+
+# BASELINE.json configs[4], the sweep grid: N = 2^20 (256 s at 4096 Hz), f_low not given -> 20 Hz, pure noise,
+# k in {32, 64, 128, 256, 512} x T in {1000, 10000, 100000}, Mc ~ U[1, 3]; w = 8 here, w = 1 (and 2, 4, 16) through
+# `cfg.replace(w=...)` / `bench.py --w`.  One seed per grid point (index 5 is the k = 256, T = 10000 point of round 1).
+SWEEP_K = (32, 64, 128, 256, 512)
+SWEEP_T = (1000, 10000, 100000)
+for _ik, _k in enumerate(SWEEP_K):
+    for _it, _T in enumerate(SWEEP_T):
+        _name = "sweep_k%d_T%d" % (_k, _T)
+        _index = 5 if (_k, _T) == (256, 10000) else 500 + 10 * _ik + _it
+        CONFIGS[_name] = WorkloadConfig(_name, _index, 1 << 20, 4096.0, 20.0, _k, _T, 8, 1.0, 3.0, 0, 0.0, 0.0)
+SWEEP_NAMES = tuple("sweep_k%d_T%d" % (_k, _T) for _k in SWEEP_K for _T in SWEEP_T)
 
 
 def _spa_templates(mc_msun: np.ndarray, cfg: WorkloadConfig, device) -> torch.Tensor:

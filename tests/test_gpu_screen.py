@@ -102,7 +102,7 @@ def check_bound(wl, w, thr1, scr, bn, tn, templates, label):
     return ratio, len(sel)
 
 
-@pytest.mark.parametrize("name,w,thr1,n_templates", [("tiny", 4, 1.2, None), ("mini", 8, 1.5, None),
+@pytest.mark.parametrize("name,w,thr1,n_templates", [("tiny", 4, 1.2, None), ("mini", 8, 1.0, None),
                                                       ("small", 8, 2.5, 320)])
 def test_screened_values_within_the_bound(rbmf, name, w, thr1, n_templates):
     wl = wlm.make_workload(wlm.CONFIGS[name], device="cuda")
