@@ -1,7 +1,12 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the reduced-basis hierarchical matched filter hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config paper|small|large|...] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config paper|small|large|sweep_k512_T100000|...|all]
+                    [--impl ours|reference]
+
+`--config all` prints one JSON line per BASELINE.json config (the sweep as its (k, T) grid); the default run times the
+`paper` config and adds a compact `configs` array (per-stage ms and roofline fractions of small, large and one sweep
+point) measured by the same program.
 
 A "step" is one rbmf_filter call: all of steps a1-a6 (include/rbmf.h) on one strain segment.  `value` is template-
 seconds of strain filtered per second = T * (N / fs) / t_step (the paper's own throughput definition),
@@ -28,10 +33,45 @@ import numpy as np  # noqa: E402
 METRIC = "template_seconds_filtered_per_second"
 UNIT = "template-seconds/s"
 
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the `ncu --set full` captures summarised
-# under profiles/ (r01_launches.md); known only for the configuration that was profiled, else reported as null.
-NCU_TRAFFIC = {("paper", 8, "screen", "gemm"): 359.5e6 + 2.5e6, ("paper", 8, "screen", "fft"): 542.8e6 + 1181.2e6,
-               ("paper", 8, "screen", "stage2"): 186.0e6 + 3.9e6}
+KERNEL_OF = {"fft": "fft_tma_kernel", "gemm": "gemm_", "stage2": "stage2"}
+
+
+def ncu_traffic(config, w, mode):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) per stage, read from the ncu launch list
+    committed as profiles/traffic_<config>_w<w>_<mode>.csv (an `ncu --csv` log of that very configuration; the .md
+    beside it names the command).  Returns ({stage: bytes}, source) -- ({}, reason) when no capture exists."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "traffic_%s_w%d_%s.csv" % (config, w, mode))
+    if not os.path.exists(path):
+        return {}, "no ncu capture committed for (%s, w=%d, %s)" % (config, w, mode)
+    acc = {}
+    with open(path, newline="") as fh:
+        rows = [r for r in csv.reader(fh) if len(r) >= 15 and r[0].isdigit()]
+    for r in rows:
+        name, metric, val = r[4], r[12], float(r[14])
+        if metric not in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            continue
+        for stage, pat in KERNEL_OF.items():
+            if pat in name:
+                acc.setdefault(stage, {}).setdefault(r[0], 0.0)
+                acc[stage][r[0]] += val
+    return {st: sum(v.values()) / len(v) for st, v in acc.items()}, "profiles/" + os.path.basename(path)
+
+
+def cpu_info():
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    try:
+        cores = len(os.sched_getaffinity(0))
+    except AttributeError:
+        cores = os.cpu_count() or 1
+    return cores, model
 
 
 # ------------------------------------------------------------------------------------------------- clocks
@@ -94,9 +134,11 @@ def oracle_throughput(wl, templates_per_step, steps, warmup, time_budget_s):
     cfg = wl["config"]
     try:
         from threadpoolctl import threadpool_info
-        threads = max([int(i.get("num_threads", 1)) for i in threadpool_info()] + [1])
+        blas_threads = max([int(i.get("num_threads", 1)) for i in threadpool_info()] + [1])
     except Exception:
-        threads = 1
+        blas_threads = 1
+    cores, model = cpu_info()
+    threads = cores
     rng = np.random.default_rng(99)
     times = []
     t_begin = time.time()
@@ -113,8 +155,9 @@ def oracle_throughput(wl, templates_per_step, steps, warmup, time_budget_s):
     ms = 1e3 * sum(times) / len(times)
     n_t = min(templates_per_step, cfg.T)
     value = n_t * (cfg.N / cfg.fs) / (ms * 1e-3)
-    sample = ("%d of %d templates per step (seeded random subset), full segment, numpy fp64 oracle_filter "
-              "(FFT single-threaded, BLAS %d threads), %d timed steps" % (n_t, cfg.T, threads, len(times)))
+    sample = ("%d of %d templates per step (seeded random subset), full segment, numpy fp64 oracle_filter as it stands "
+              "(%d cores available by sched_getaffinity on %s; its BLAS leg uses %d threads, its FFT leg one), "
+              "%d timed steps" % (n_t, cfg.T, cores, model, blas_threads, len(times)))
     return value, ms, threads, sample
 
 
@@ -124,17 +167,212 @@ def oracle_templates_per_step(cfg):
     return int(max(4, min(cfg.T, 2.0 / per_template)))
 
 
+# ------------------------------------------------------------------------------------------ one configuration
+def describe(cfg, world):
+    return {"workload": "%s: N=%d fs=%g f_low=%g k=%d T=%d w=%d thr=%g/%g injections=%d" % (
+        cfg.name, cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, cfg.w, cfg.thr1, cfg.thr2, cfg.n_inj),
+        "N": cfg.N, "k": cfg.k, "T": cfg.T, "w": cfg.w, "segment_seconds": cfg.N / cfg.fs,
+        "parallelism": "replicas x%d (one strain segment per GPU, no collective)" % world,
+        "l2": ("working set (basis %.0f MB + beta %.0f MB) exceeds the 126 MB L2; no flush needed" if
+               cfg.N * cfg.k * 12 > 252e6 else
+               "working set (basis %.0f MB + beta %.0f MB) is L2-sized: a 256 MB scrub buffer is written between steps") % (
+            cfg.N / 2 * cfg.k * 8 / 1e6, cfg.N * cfg.k * 8 / 1e6)}
+
+
+def pick_peaks(elapsed_ms, clocks):
+    """(hbm peak, tensor peak of the regime, burst, sustained, regime, source).  The burst figure applies to a short
+    timed region at full clocks, the sustained one to a seconds-long loop or one that ran into the power cap
+    (B200_PROFILING.md)."""
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        peaks = json.load(open(peaks_path))
+        hbm, burst, sust, src = peaks["hbm_gbs"], peaks["bf16_tflops"], peaks["bf16_tflops_sustained"], "measured"
+    else:
+        hbm, burst, sust, src = 6650.0, 1590.0, 1400.0, "fallback"
+    capped = "sw_power_cap" in (clocks.get("reasons") or [])
+    regime = "sustained" if (elapsed_ms >= 1000.0 or capped) else "burst"
+    return hbm, (sust if regime == "sustained" else burst), burst, sust, regime, src
+
+
+def stat(xs):
+    return {"mean": statistics.mean(xs), "median": statistics.median(xs), "best": min(xs)}
+
+
+def measure(cfg, args, rdist, rbmf, workloads, torch, device, stream, rank, world, local_rank, headline):
+    """Times one configuration.  headline = True adds the end-to-end leg, the other tensor-core mode and (N = 1) the
+    CPU baseline; False returns the compact per-stage summary used for the `configs` array."""
+    steps = args.steps if headline else max(3, min(args.steps, args.summary_steps))
+    wl = workloads.make_workload(cfg, device=str(device))
+    seg = rdist.segment_index(rank, 0, world)
+    strain_np, _ = workloads.make_strain(wl, seg)
+    impls = {"screen": rbmf.RBMF_GEMM_SCREEN, "bf16x3": rbmf.RBMF_GEMM_TCGEN05}
+    small_ws = cfg.N * cfg.k * 12 <= 252e6
+    with torch.cuda.stream(stream):
+        strain_dev = torch.from_numpy(strain_np).to(device)
+        scrub = torch.empty(256 << 20, dtype=torch.uint8, device=device) if small_ws else None
+        capacity = 1 << 22
+        while True:
+            # list capacities grow until one warm-up pass fits (SURVEY.md 8(d): dense banks give 1e6-1e9 records)
+            torch.cuda.empty_cache()
+            plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, device=str(device), stream=stream,
+                             max_candidates=capacity, max_triggers=capacity)
+            plan.set_gemm_impl(impls[args.gemm])
+            plan.set_basis(torch.from_numpy(wl["basis"]))
+            plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+            for _ in range(args.warmup):
+                plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
+            stream.synchronize()
+            nc, nt, st = plan.counts(allow_overflow=True)
+            if st != rbmf.RBMF_ERR_OVERFLOW or capacity >= (1 << 30):
+                break
+            plan.close()
+            capacity <<= 2
+        plan.set_timing(True)
+        sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
+                               int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
+        rdist.barrier(device)
+        torch.cuda.synchronize(device)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        stage = {"fft": [], "gemm": [], "stage2": [], "total": []}
+        t_wall0 = time.time()
+        if scrub is None:
+            ev0.record(stream)
+            for _ in range(steps):                    # the timed region: K steps back to back, no host sync inside
+                plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
+            ev1.record(stream)
+            torch.cuda.synchronize(device)
+            elapsed_local = ev0.elapsed_time(ev1)
+        else:
+            # L2-sized working set: scrub L2 between steps, time each step with its own pair of events
+            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+            for a, b in evs:
+                scrub.fill_(1)
+                a.record(stream)
+                plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
+                b.record(stream)
+            torch.cuda.synchronize(device)
+            elapsed_local = sum(a.elapsed_time(b) for a, b in evs)
+        rdist.barrier(device)
+        elapsed_ms = rdist.max_over_ranks(elapsed_local, device)
+        # per-kernel durations: the same K steps again, reading the library's CUDA events after every step (this
+        # costs a host round trip per step, which is why it is not done inside the region `value` comes from)
+        for _ in range(steps):
+            if scrub is not None:
+                scrub.fill_(1)
+            plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
+            ms = plan.stage_ms()                      # waits for this step's last event, reads the stage events
+            for key in stage:
+                stage[key].append(ms[key])
+        t_wall1 = time.time()
+        clocks = sampler.summary(t_wall0, t_wall1)
+        n_screened = plan.screened_count()
+
+        e2e = None
+        other_stage = None
+        if headline:
+            # ---- end-to-end leg: host strain in, host triggers out, every step
+            strain_pinned = torch.from_numpy(strain_np).pin_memory()
+            out_pinned = torch.empty(plan.max_triggers * 4, dtype=torch.int32).pin_memory()
+            out_host = out_pinned.numpy().view(rbmf.TRIGGER_DTYPE)
+            for _ in range(2):
+                plan.filter_host(strain_pinned.numpy(), cfg.thr1, cfg.thr2, out_host)
+            rdist.barrier(device)
+            torch.cuda.synchronize(device)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            n_e2e = 0
+            for _ in range(steps):
+                _, n_e2e = plan.filter_host(strain_pinned.numpy(), cfg.thr1, cfg.thr2, out_host)
+            e1.record(stream)
+            torch.cuda.synchronize(device)
+            e2e_ms = rdist.max_over_ranks(e0.elapsed_time(e1), device)
+            e2e = {"value": world * cfg.T * (cfg.N / cfg.fs) / (e2e_ms / steps * 1e-3), "unit": UNIT,
+                   "h2d_bytes_per_step": (cfg.N // 2 + 1) * 8,
+                   "d2h_bytes_per_step": 16 + int(min(n_e2e, plan.max_triggers)) * 16, "ms_per_step": e2e_ms / steps}
+            del out_pinned, out_host
+        sampler.stop()
+        # ---- the other tensor-core mode, per-stage only (context for `stages`; not part of `value`)
+        other = {"screen": "bf16x3", "bf16x3": "screen"}[args.gemm]
+        plan.set_gemm_impl(impls[other])
+        acc = {"fft": [], "gemm": [], "stage2": [], "total": []}
+        for i in range(3 + min(steps, 20 if headline else 3)):
+            plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
+            ms = plan.stage_ms()
+            if i >= 3:
+                for key in acc:
+                    acc[key].append(ms[key])
+        other_stage = {key + "_ms": statistics.mean(v) for key, v in acc.items()}
+        plan.set_gemm_impl(impls[args.gemm])
+        launches = plan.launches_per_filter()
+        plan.close()
+        del plan, scrub
+        torch.cuda.empty_cache()
+
+    seg_seconds = cfg.N / cfg.fs
+    ms_per_step = elapsed_ms / steps
+    value = world * cfg.T * seg_seconds / (ms_per_step * 1e-3)
+
+    # ---- rooflines (DESIGN.md "Measurement"): dominant kernel = the stage-1 GEMM
+    hbm_peak, tensor_peak, peak_burst, peak_sust, regime, peak_src = pick_peaks(elapsed_ms, clocks)
+    gemm_ms, fft_ms, s2_ms = (statistics.mean(stage[kk]) for kk in ("gemm", "fft", "stage2"))
+    M = cfg.N // cfg.w
+    useful_flops = 8.0 * cfg.T * cfg.k * M
+    products = 1.0 if args.gemm == "screen" else 3.0         # tensor-core products executed per useful one
+    gemm_tflops = products * useful_flops / (gemm_ms * 1e-3) / 1e12
+    band = cfg.N // 2 - cfg.j_low
+    fft_alg_bytes = cfg.k * band * 8 + (cfg.N // 2 + 1) * 8 + cfg.k * cfg.N * 8 + cfg.k * M * 8
+    fft_gbs = fft_alg_bytes / (fft_ms * 1e-3) / 1e9
+    traffic, traffic_src = ncu_traffic(cfg.name, cfg.w, args.gemm)
+    roofline = {"kernel": ("gemm_screen_pair_kernel" if args.gemm == "screen" else "gemm_tcgen05_kernel") + " (a4-a5)",
+                "bound": "tensor", "achieved": gemm_tflops, "peak": tensor_peak, "unit": "TFLOP/s",
+                "frac": gemm_tflops / tensor_peak, "traffic": traffic.get("gemm"), "traffic_source": traffic_src,
+                "regime": regime, "peak_source": "%s bf16 cuBLAS, %s figure (timed region %.0f ms%s)" % (
+                    peak_src, regime, elapsed_ms, ", sw_power_cap active" if "sw_power_cap" in (clocks.get("reasons") or []) else ""),
+                "frac_of_burst_peak": gemm_tflops / peak_burst, "frac_of_sustained_peak": gemm_tflops / peak_sust,
+                "flops_counted": "executed 16-bit MMA flops = %d x 8 T k N/w (%s)" % (
+                    int(products), "one fp16 product: error-bounded screen, fp32 confirm in kernel 3"
+                    if args.gemm == "screen" else "bf16x3 split precision"),
+                "useful_tflops": useful_flops / (gemm_ms * 1e-3) / 1e12, "avg_kernel_ms": gemm_ms}
+    stages = {"fft_ms": fft_ms, "gemm_ms": gemm_ms, "stage2_ms": s2_ms, "total_ms": statistics.mean(stage["total"]),
+              "per_step_ms": {kk: stat(v) for kk, v in stage.items()},
+              "fft": {"bound": "hbm", "algorithmic_GBps": fft_gbs, "peak": hbm_peak, "frac": fft_gbs / hbm_peak,
+                      "algorithmic_bytes": fft_alg_bytes, "traffic": traffic.get("fft")},
+              "stage2": {"candidates_per_s": (nc / (s2_ms * 1e-3)) if s2_ms > 0 else None,
+                         "algorithmic_GBps": n_screened * (cfg.w + 1) * cfg.k * 8 / (s2_ms * 1e-3) / 1e9,
+                         "traffic": traffic.get("stage2")},
+              "n_candidates": nc, "n_screened": n_screened, "n_triggers": nt, "gemm_mode": args.gemm,
+              "list_capacity": capacity, "lists_overflowed": bool(n_screened > capacity or nt > capacity),
+              "other_mode": dict(other_stage, gemm_mode=other)}
+    if not headline:
+        return {"workload": describe(cfg, world)["workload"], "steps": steps, "ms_per_step": ms_per_step, "value": value,
+                "fft_ms": fft_ms, "gemm_ms": gemm_ms, "stage2_ms": s2_ms, "fft_frac_hbm": fft_gbs / hbm_peak,
+                "gemm_frac_tensor": gemm_tflops / tensor_peak, "gemm_tflops": gemm_tflops, "regime": regime,
+                "n_candidates": nc, "n_triggers": nt, "lists_overflowed": stages["lists_overflowed"],
+                "other_mode": stages["other_mode"], "clocks": clocks}, wl
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None,
+            "dtype": ("f16 tensor-core screen with an error bound + f32 confirm/re-score + f32 FFT"
+                      if args.gemm == "screen" else "bf16x3 (fp32-equivalent split bf16 on tensor cores) + f32"),
+            "data": "synthetic", "config": describe(cfg, world), "clocks": clocks, "e2e": e2e,
+            "gpu_launches": launches * steps, "roofline": roofline, "stages": stages}
+    return line, wl
+
+
 # ---------------------------------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="paper")
+    ap.add_argument("--config", default="paper", help="a name in workloads.CONFIGS, or `all`")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--w", type=int, default=None, help="override the averaging window")
     ap.add_argument("--gemm", default="screen", choices=["screen", "bf16x3"],
                     help="stage-1 kernel: fp16 screen + fp32 confirm (library default) or bf16x3")
+    ap.add_argument("--summary-configs", default="small,large,sweep_k256_T10000",
+                    help="configs summarised in the `configs` array of the default line ('' = none)")
+    ap.add_argument("--summary-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -143,27 +381,26 @@ def main():
     from paper_2110_13115_b200 import dist as rdist, workloads
 
     rank, local_rank, world = rdist.env_world()
-    cfg = workloads.CONFIGS[args.config]
-    if args.w is not None:
-        cfg = cfg.replace(w=args.w)
-    config_desc = {"workload": "%s: N=%d fs=%g f_low=%g k=%d T=%d w=%d thr=%g/%g injections=%d" % (
-        cfg.name, cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, cfg.w, cfg.thr1, cfg.thr2, cfg.n_inj),
-        "N": cfg.N, "k": cfg.k, "T": cfg.T, "w": cfg.w, "segment_seconds": cfg.N / cfg.fs,
-        "parallelism": "replicas x%d (one strain segment per GPU, no collective)" % world,
-        "l2": "working set (basis %.0f MB + beta %.0f MB) exceeds the 126 MB L2; no flush needed" % (
-            cfg.N / 2 * cfg.k * 8 / 1e6, cfg.N * cfg.k * 8 / 1e6)}
+    if args.config == "all":
+        names = ["tiny", "small", "paper", "large"] + list(workloads.SWEEP_NAMES)
+    else:
+        names = [args.config]
 
     # ------------------------------------------------------------------ reference arm: the oracle, on host cores
     if args.impl == "reference":
         if rank != 0:
             return 0
+        cfg = workloads.CONFIGS[names[0] if args.config != "all" else "paper"]
+        if args.w is not None:
+            cfg = cfg.replace(w=args.w)
         dev = "cuda" if torch.cuda.is_available() else "cpu"
         wl = workloads.make_workload(cfg, device=dev)
         tps = oracle_templates_per_step(cfg)
         value, ms, threads, sample = oracle_throughput(wl, tps, args.steps, args.warmup, time_budget_s=150.0)
         line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_desc,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": describe(cfg, world),
                 "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
                 "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
                 "gpu_launches": 0}
@@ -177,150 +414,29 @@ def main():
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
     from paper_2110_13115_b200 import rbmf
-
-    wl = workloads.make_workload(cfg, device=str(device))
-    seg = rdist.segment_index(rank, 0, world)
-    strain_np, _ = workloads.make_strain(wl, seg)
     stream = torch.cuda.Stream(device=device)
-    with torch.cuda.stream(stream):
-        impls = {"screen": rbmf.RBMF_GEMM_SCREEN, "bf16x3": rbmf.RBMF_GEMM_TCGEN05}
-        strain_dev = torch.from_numpy(strain_np).to(device)
-        strain_pinned = torch.from_numpy(strain_np).pin_memory()
-        capacity = 1 << 22
-        while True:
-            # list capacities grow until one warm-up pass fits (dense banks give 1e6-1e7 records)
-            plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, device=str(device), stream=stream,
-                             max_candidates=capacity, max_triggers=capacity)
-            plan.set_gemm_impl(impls[args.gemm])
-            plan.set_basis(torch.from_numpy(wl["basis"]))
-            plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
-            torch.cuda.empty_cache()
-            for _ in range(args.warmup):
-                plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
-            stream.synchronize()
-            nc, nt, st = plan.counts(allow_overflow=True)
-            if st != rbmf.RBMF_ERR_OVERFLOW or capacity >= (1 << 26):
-                break
-            plan.close()
-            capacity <<= 2
-        # pinned host array for the trigger list (the end-to-end leg copies into it every step)
-        out_pinned = torch.empty(plan.max_triggers * 4, dtype=torch.int32).pin_memory()
-        out_host = out_pinned.numpy().view(rbmf.TRIGGER_DTYPE)
-        plan.set_timing(True)
-        sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
-                               int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
-        rdist.barrier(device)
-        torch.cuda.synchronize(device)
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        stage = {"fft": [], "gemm": [], "stage2": [], "total": []}
-        t_wall0 = time.time()
-        ev0.record(stream)
-        for _ in range(args.steps):                   # the timed region: K steps back to back, no host sync inside
-            plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
-        ev1.record(stream)
-        torch.cuda.synchronize(device)
-        rdist.barrier(device)
-        elapsed_ms = rdist.max_over_ranks(ev0.elapsed_time(ev1), device)
-        # per-kernel durations: the same K steps again, reading the library's CUDA events after every step (this
-        # costs a host round trip per step, which is why it is not done inside the region `value` comes from)
-        for _ in range(args.steps):
-            plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
-            ms = plan.stage_ms()                      # waits for this step's last event, reads the stage events
-            for key in stage:
-                stage[key].append(ms[key])
-        t_wall1 = time.time()
-        clocks = sampler.summary(t_wall0, t_wall1)
 
-        # ---- end-to-end leg: host strain in, host triggers out, every step
-        for _ in range(2):
-            plan.filter_host(strain_pinned.numpy(), cfg.thr1, cfg.thr2, out_host)
-        rdist.barrier(device)
-        torch.cuda.synchronize(device)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        n_e2e = 0
-        for _ in range(args.steps):
-            _, n_e2e = plan.filter_host(strain_pinned.numpy(), cfg.thr1, cfg.thr2, out_host)
-        e1.record(stream)
-        torch.cuda.synchronize(device)
-        e2e_ms = rdist.max_over_ranks(e0.elapsed_time(e1), device)
-        sampler.stop()
-
-        # ---- the other tensor-core mode, per-stage only (context for `stages`; not part of `value`)
-        other = {"screen": "bf16x3", "bf16x3": "screen"}.get(args.gemm)
-        other_stage = None
-        if other is not None:
-            plan.set_gemm_impl(impls[other])
-            acc = {"fft": [], "gemm": [], "stage2": [], "total": []}
-            for i in range(3 + min(args.steps, 20)):
-                plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
-                ms = plan.stage_ms()
-                if i >= 3:
-                    for key in acc:
-                        acc[key].append(ms[key])
-            other_stage = {key + "_ms": statistics.mean(v) for key, v in acc.items()}
-            plan.set_gemm_impl(impls[args.gemm])
-
-    seg_seconds = cfg.N / cfg.fs
-    ms_per_step = elapsed_ms / args.steps
-    value = world * cfg.T * seg_seconds / (ms_per_step * 1e-3)
-    e2e_value = world * cfg.T * seg_seconds / (e2e_ms / args.steps * 1e-3)
-
-    if rank != 0:
-        rdist.finalize()
-        return 0
-
-    # ---- rooflines: dominant kernel = the stage-1 GEMM
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(peaks_path):
-        peaks = json.load(open(peaks_path))
-        hbm_peak, tensor_peak, peak_src = peaks["hbm_gbs"], peaks["bf16_tflops_sustained"], "measured (sustained bf16)"
-    else:
-        hbm_peak, tensor_peak, peak_src = 6650.0, 1400.0, "fallback"
-    gemm_ms = statistics.mean(stage["gemm"])
-    fft_ms = statistics.mean(stage["fft"])
-    s2_ms = statistics.mean(stage["stage2"])
-    M = cfg.N // cfg.w
-    useful_flops = 8.0 * cfg.T * cfg.k * M
-    products = 1.0 if args.gemm == "screen" else 3.0         # tensor-core products executed per useful one
-    executed_flops = products * useful_flops
-    gemm_tflops = executed_flops / (gemm_ms * 1e-3) / 1e12
-    band = cfg.N // 2 - cfg.j_low
-    fft_alg_bytes = cfg.k * band * 8 + (cfg.N // 2 + 1) * 8 + cfg.k * cfg.N * 8 + cfg.k * M * 8
-    fft_gbs = fft_alg_bytes / (fft_ms * 1e-3) / 1e9
-    roofline = {"kernel": ("gemm_screen_pair_kernel" if args.gemm == "screen" else "gemm_tcgen05_kernel") + " (a4-a5)", "bound": "tensor", "achieved": gemm_tflops,
-                "peak": tensor_peak, "unit": "TFLOP/s", "frac": gemm_tflops / tensor_peak,
-                "traffic": NCU_TRAFFIC.get((args.config, cfg.w, args.gemm, "gemm")),
-                "peak_source": peak_src, "flops_counted": "executed 16-bit MMA flops = %d x 8 T k N/w (%s)" % (
-                    int(products), "one fp16 product: rigorous-bound screen, fp32 confirm in kernel 3"
-                    if args.gemm == "screen" else "bf16x3 split precision"),
-                "useful_tflops": useful_flops / (gemm_ms * 1e-3) / 1e12, "avg_kernel_ms": gemm_ms}
-    stages = {"fft_ms": fft_ms, "gemm_ms": gemm_ms, "stage2_ms": s2_ms, "total_ms": statistics.mean(stage["total"]),
-              "fft": {"bound": "hbm", "algorithmic_GBps": fft_gbs, "peak": hbm_peak, "frac": fft_gbs / hbm_peak,
-                      "algorithmic_bytes": fft_alg_bytes,
-                      "traffic": NCU_TRAFFIC.get((args.config, cfg.w, args.gemm, "fft"))},
-              "n_candidates": nc, "n_triggers": nt, "gemm_mode": args.gemm, "list_capacity": capacity,
-              "lists_overflowed": bool(nc > capacity or nt > capacity)}
-    if other_stage is not None:
-        stages["other_mode"] = dict(other_stage, gemm_mode=other)
-
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": ("f16 tensor-core screen with a rigorous error bound + f32 confirm/re-score + f32 FFT"
-                      if args.gemm == "screen" else "bf16x3 (fp32-equivalent split bf16 on tensor cores) + f32"),
-            "data": "synthetic", "config": config_desc, "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (cfg.N // 2 + 1) * 8,
-                    "d2h_bytes_per_step": 16 + int(min(n_e2e, plan.max_triggers)) * 16,
-                    "ms_per_step": e2e_ms / args.steps},
-            "gpu_launches": plan.launches_per_filter() * args.steps, "roofline": roofline, "stages": stages}
-
-    if world == 1 and not args.no_cpu_baseline:
-        tps = oracle_templates_per_step(cfg)
-        v, ms, threads, sample = oracle_throughput(wl, tps, steps=6, warmup=1, time_budget_s=25.0)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
-                                "ms_per_step": ms}
-    print(json.dumps(line))
-    plan.close()
+    for name in names:
+        cfg = workloads.CONFIGS[name]
+        if args.w is not None:
+            cfg = cfg.replace(w=args.w)
+        line, wl = measure(cfg, args, rdist, rbmf, workloads, torch, device, stream, rank, world, local_rank, True)
+        if world == 1 and not args.no_cpu_baseline:
+            tps = oracle_templates_per_step(cfg)
+            v, ms, threads, sample = oracle_throughput(wl, tps, steps=6, warmup=1,
+                                                       time_budget_s=25.0 if args.config != "all" else 8.0)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                                    "ms_per_step": ms}
+        del wl
+        if args.config != "all" and world == 1 and args.summary_configs:
+            line["configs"] = []
+            for other in [c for c in args.summary_configs.split(",") if c and c != name]:
+                summ, wl2 = measure(workloads.CONFIGS[other], args, rdist, rbmf, workloads, torch, device, stream, rank,
+                                    world, local_rank, False)
+                del wl2
+                line["configs"].append(summ)
+        if rank == 0:
+            print(json.dumps(line), flush=True)
     rdist.finalize()
     return 0
 
