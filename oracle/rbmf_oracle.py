@@ -33,6 +33,8 @@ Pins (tests/test_oracle_pins.py, all `-m "not gpu"`):
   averaging                    Eq. 12 alias-fold route (`averaged_series_eq12`) == binned mean; w=1 => flat
   thresholds / sets            independent pure-Python enumeration on tiny inputs
   cost model                   Eq. 13-14 reproduce the paper's quoted ~6x / ~10x (tests/golden/paper_values.txt)
+  forward transform, whitening literal O(N^2) sum at small N, a cosine's closed form (N/2 at its bin), Parseval; batches:
+                               segment b of `oracle_filter_batch` against the time-domain brute force on strain b alone
 Parity status: every function below is pinned by at least one of these; nothing is "parity unpinned".
 """
 from __future__ import annotations
@@ -229,6 +231,41 @@ def oracle_filter(strain, basis, coeffs, sigma, N, fs, f_low, w, thr1, thr2, tem
     cat = lambda parts, dt: np.concatenate(parts) if parts else np.empty(0, dtype=dt)
     return {"triggers": cat(trig_parts, trig_dt), "candidates": cat(cand_parts, cand_dt),
             "near": cat(near_parts, trig_dt), "cand_near": cat(cnear_parts, cand_dt), "n_flat": n_flat}
+
+
+# ------------------------------------------------- the step before the path, and batches of segments
+def strain_from_time_series(x, inv_asd=None):
+    """Step 1 of the paper's scheme (PAPER.md:175 "FFT of the data", :177 "divided by sqrt(S_n)"):
+    d[j] = inv_asd[j] * sum_n x[n] e^{-2 pi i j n / N}, j = 0..N/2 -- the unnormalised forward DFT of the real series
+    (SURVEY.md App. A), times the caller's whitening array 1/sqrt(S_n(f_j)) (omitted = already white).
+    x: (N,) or (B, N) real.  Returns complex128 (N/2+1,) or (B, N/2+1)."""
+    x = np.asarray(x, dtype=np.float64)
+    d = np.fft.rfft(x, axis=-1)
+    if inv_asd is not None:
+        d = d * np.asarray(inv_asd, dtype=np.float64)
+    return d
+
+
+def oracle_filter_batch(strains, basis, coeffs, sigma, N, fs, f_low, w, thr1, thr2, templates=None, chunk=64):
+    """A batch of segments filtered against the same resident basis and coefficients ("filtering each
+    segment in parallel"): segment b is the whole hot path on strains[b], independent of the others; its records are
+    reported with time = b N + n and bin = b N/w + i.  Same fields as `oracle_filter`."""
+    strains = np.asarray(strains)
+    out = None
+    for b in range(strains.shape[0]):
+        r = oracle_filter(strains[b], basis, coeffs, sigma, N, fs, f_low, w, thr1, thr2, templates=templates,
+                          chunk=chunk)
+        for key in ("triggers", "near"):
+            r[key]["time"] += b * N
+        for key in ("candidates", "cand_near"):
+            r[key]["bin"] += b * (N // w)
+        if out is None:
+            out = r
+        else:
+            for key in ("triggers", "near", "candidates", "cand_near"):
+                out[key] = np.concatenate([out[key], r[key]])
+            out["n_flat"] += r["n_flat"]
+    return out
 
 
 def evaluate_points(strain, basis, coeffs, sigma, N, fs, f_low, w, template, times):

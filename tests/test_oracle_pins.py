@@ -317,3 +317,69 @@ def test_paper_throughput_and_cost_model_values():
     # memory arithmetic, PAPER.md:136-140 (8 B per entry)
     assert abs(N ** 2 * 8 / 1e9 / g["covariance_full_gb"] - 1) < 0.01
     assert abs(g["nonuniform_Nt"] ** 2 * 8 / 1e9 / g["covariance_nonuniform_gb"] - 1) < 0.10
+
+
+# ---------------------------------------------------------------- step 1 of the scheme and batches
+def test_forward_transform_against_literal_sum_closed_form_and_parseval():
+    """PAPER.md:175 (FFT of the data), :177 (division by sqrt(S_n)): literal O(N^2) DFT, a cosine's closed form,
+    Parseval, and the whitening array as a plain per-bin factor."""
+    N = 64
+    rng = np.random.default_rng(11)
+    x = rng.standard_normal(N)
+    d = orc.strain_from_time_series(x)
+    assert d.shape == (N // 2 + 1,)
+    for j in (0, 1, 7, N // 2):
+        lit = sum(x[n] * complex(math.cos(2 * math.pi * j * n / N), -math.sin(2 * math.pi * j * n / N)) for n in range(N))
+        assert abs(d[j] - lit) < 1e-12
+    # Parseval for a real series: sum x^2 = (|d0|^2 + |d_{N/2}|^2 + 2 sum_{0<j<N/2} |d_j|^2) / N
+    assert abs((x ** 2).sum() - (abs(d[0]) ** 2 + abs(d[-1]) ** 2 + 2 * (np.abs(d[1:-1]) ** 2).sum()) / N) < 1e-11
+    j0, amp, ph = 5, 1.7, 0.3
+    c = amp * np.cos(2 * math.pi * j0 * np.arange(N) / N + ph)
+    dc = orc.strain_from_time_series(c)
+    assert abs(dc[j0] - amp * N / 2 * complex(math.cos(ph), math.sin(ph))) < 1e-11
+    assert np.abs(np.delete(dc, j0)).max() < 1e-11
+    inv_asd = rng.uniform(0.5, 2.0, N // 2 + 1)
+    dw = orc.strain_from_time_series(np.stack([x, c]), inv_asd)
+    assert dw.shape == (2, N // 2 + 1)
+    assert np.abs(dw[0] - d * inv_asd).max() < 1e-12 and abs(dw[1][j0] - dc[j0] * inv_asd[j0]) < 1e-11
+
+
+def test_whitened_time_series_feeds_the_time_domain_bruteforce():
+    """Front end + path together: with a flat whitening array the SNR series of the transformed time series equals
+    the brute-force time-domain circular correlation of that very series (same pin as the FFT sign/scale)."""
+    N, fs, f_low = 128, 128.0, 9.0
+    rng = np.random.default_rng(8)
+    x = rng.standard_normal(N)
+    j_low, _ = orc.band(N, fs, f_low)
+    u = np.zeros(N // 2 + 1, dtype=np.complex128)
+    u[j_low:N // 2] = rng.standard_normal(N // 2 - j_low) + 1j * rng.standard_normal(N // 2 - j_low)
+    u /= np.linalg.norm(u)
+    d = orc.strain_from_time_series(x, np.ones(N // 2 + 1))
+    assert np.abs(orc.snr_series_fft(d, u, 1.0, N, j_low) - _time_domain_bruteforce(x, u, N, j_low)).max() < 1e-11
+
+
+def test_batch_segments_are_independent_and_offset(micro):
+    """each segment of a batch is filtered on its own.  Segment 1's records of `oracle_filter_batch`
+    against a pure-Python enumeration that only ever sees strain 1; offsets time = b N + n, bin = b N/w + i."""
+    cfg = micro["config"]
+    N, w = cfg.N, cfg.w
+    s1, _ = wlm.make_strain(micro, 1)
+    strains = np.stack([micro["strain"], s1])
+    res = orc.oracle_filter_batch(strains, micro["basis"], micro["coeffs"], micro["sigma"], N, cfg.fs, cfg.f_low, w,
+                                  cfg.thr1, cfg.thr2)
+    hp = orc.reconstructed_templates(micro["coeffs"], micro["basis"])
+    exp_trig, exp_cand = [], []
+    for t in range(cfg.T):
+        rho = orc.snr_series_direct(s1, hp[t], micro["sigma"][t], N, cfg.j_low)
+        for i in range(N // w):
+            if abs(sum(rho[i * w + r] for r in range(w)) / w) >= cfg.thr1:
+                exp_cand.append((t, N // w + i))
+                exp_trig += [(t, N + i * w + r) for r in range(w) if abs(rho[i * w + r]) >= cfg.thr2]
+    got_trig = [(int(a), int(b)) for a, b in zip(res["triggers"]["template"], res["triggers"]["time"]) if b >= N]
+    got_cand = [(int(a), int(b)) for a, b in zip(res["candidates"]["template"], res["candidates"]["bin"]) if b >= N // w]
+    assert len(exp_trig) > 3 and got_trig == exp_trig and got_cand == exp_cand
+    seg0 = orc.oracle_filter(micro["strain"], micro["basis"], micro["coeffs"], micro["sigma"], N, cfg.fs, cfg.f_low, w,
+                             cfg.thr1, cfg.thr2)
+    n0 = len(seg0["triggers"])
+    assert n0 > 0 and np.array_equal(res["triggers"][:n0], seg0["triggers"]) and (res["triggers"]["time"][:n0] < N).all()
+    assert len(res["near"]) >= len(res["triggers"]) and res["n_flat"] >= len(res["triggers"])
