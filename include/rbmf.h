@@ -91,6 +91,12 @@ rbmf_status rbmf_plan_set_window(rbmf_plan* plan, int32_t w);
  * before rbmf_workspace_bytes / rbmf_plan_set_workspace. */
 rbmf_status rbmf_plan_set_capacity(rbmf_plan* plan, int64_t max_candidates, int64_t max_triggers);
 
+/* Largest number of strain segments one rbmf_filter_batch call may take (default 1).  The paper filters a batch of
+ * segments in parallel against the resident basis and coefficients; the workspace holds beta and the
+ * beta^avg planes of max_batch segments.  max_batch * N must stay below 2^31 (a trigger's time_index counts samples
+ * over the whole batch).  Must be called before rbmf_workspace_bytes / rbmf_plan_set_workspace. */
+rbmf_status rbmf_plan_set_batch(rbmf_plan* plan, int32_t max_batch);
+
 /* Select the stage-1 kernel (RBMF_GEMM_SCREEN, the default, or RBMF_GEMM_TCGEN05).  May be called at any time. */
 rbmf_status rbmf_plan_set_gemm_impl(rbmf_plan* plan, int32_t impl);
 
@@ -123,11 +129,38 @@ rbmf_status rbmf_set_coeffs(rbmf_plan* plan, const void* coeffs_dev, const float
 rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage1, float thr_stage2,
                         rbmf_trigger* out_dev, int64_t* n_out_dev);
 
+/* The step in front of the path (PAPER.md:175 "FFT of the data", :177 division by sqrt(S_n)): forward real-to-complex
+ * DFT of n_segments (<= max_batch) time series and whitening,
+ *     strain_out[b][j] = inv_asd[j] * sum_n x[b][n] exp(-2 pi i j n / N),   j = 0 .. N/2,
+ * i.e. exactly the array rbmf_filter / rbmf_filter_batch take.  x_dev: n_segments x N float32 (8-byte aligned);
+ * inv_asd_dev: N/2+1 float32 = 1/sqrt(S_n(f_j)) in the caller's normalisation (such that the whitened series has unit
+ * variance per sample), or NULL for data that is already white; strain_out_dev: n_segments x (N/2+1) complex64, must
+ * not alias x_dev.  Enqueues three small kernels on the plan's stream (a four-step radix-2 FFT of the series packed
+ * as N/2 complex values, then the real-input split); needs the workspace, not the basis or the coefficients. */
+rbmf_status rbmf_prepare_strain(rbmf_plan* plan, const float* x_dev, const float* inv_asd_dev, int32_t n_segments,
+                                void* strain_out_dev);
+
+/* Filter n_segments (1 <= n_segments <= max_batch) segments at once ("filtering each segment in
+ * parallel", basis and coefficients loaded once).  strain_dev: n_segments x (N/2+1) complex64, row-major, each row as
+ * in rbmf_filter.  Steps a1-a3 run once per (segment, basis column) in ONE launch that reads every block of the
+ * basis from HBM once and takes it from L2 for the other segments; steps a4-a5 run as ONE contraction over the
+ * n_segments * N/w bins of the batch (each coefficient tile is loaded once per batch); step a6 over all candidates.
+ * Triggers carry the segment in the time index: time_index = segment * N + n, n in [0, N)  (rbmf_candidate:
+ * bin_index = segment * N/w + i).  The result equals n_segments calls of rbmf_filter, segment by segment.
+ * Other arguments, asynchrony and overflow behaviour as in rbmf_filter. */
+rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n_segments, float thr_stage1,
+                              float thr_stage2, rbmf_trigger* out_dev, int64_t* n_out_dev);
+
 /* End-to-end convenience with HOST buffers: copies the strain to the device, filters, waits, and copies
  * the triggers back.  strain_host: (N/2+1) complex64.  out_host: capacity_out entries (<= max_triggers).
  * *n_out_host = total found.  Synchronous.  Returns RBMF_ERR_OVERFLOW if either list overflowed. */
 rbmf_status rbmf_filter_host(rbmf_plan* plan, const void* strain_host, float thr_stage1, float thr_stage2,
                              rbmf_trigger* out_host, int64_t capacity_out, int64_t* n_out_host);
+
+/* rbmf_filter_host for a batch: strain_host is n_segments x (N/2+1) complex64; triggers as in rbmf_filter_batch. */
+rbmf_status rbmf_filter_batch_host(rbmf_plan* plan, const void* strain_host, int32_t n_segments, float thr_stage1,
+                                   float thr_stage2, rbmf_trigger* out_host, int64_t capacity_out,
+                                   int64_t* n_out_host);
 
 /* Counts of the last rbmf_filter (synchronises the stream).  RBMF_ERR_OVERFLOW if a capacity was exceeded
  * (in RBMF_GEMM_SCREEN mode the capacity max_candidates applies to the screened superset, see
@@ -145,14 +178,15 @@ rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64
 
 /* Read-only device views of internal arrays for diagnostics and parity tests (valid after rbmf_filter on the
  * plan's stream, until the next call), in the library's blocked layouts:
- *   which = 0: beta, complex64, [k/4 chunks][N samples][4 columns]: beta_c[n] at ((c/4) N + n) 4 + c%4;
- *   which = 1 / 2: beta^avg hi / lo plane, bfloat16, [ceil(k/32) K blocks][N/w bins][32 columns][re, im]
+ *   which = 0: beta, complex64, [segment][k/4 chunks][N samples][4 columns]: beta_c[n] of segment b at
+ *              ((b k/4 + c/4) N + n) 4 + c%4  (max_batch segments; a single-segment plan has b = 0 only);
+ *   which = 1 / 2: beta^avg hi / lo plane, bfloat16, [ceil(k/32) K blocks][max_batch N/w bins][32 columns][re, im]
  *                  (value = hi + lo; columns >= k of the last block are zero).  In RBMF_GEMM_SCREEN mode plane 1
  *                  holds ONE float16 rounding of beta^avg in the same layout and plane 2 is stale.
  *   which = 3: the stage-1 list as kernel 2 wrote it (rbmf_candidate records, min(rbmf_get_screened_count,
  *              max_candidates) valid entries; *bytes = capacity in bytes).  In RBMF_GEMM_SCREEN mode avg_re/avg_im are
  *              the raw one-product fp16 tensor-core values R_16 the screen tested;
- *   which = 4: bin_norm, float32[N/w]: the upper bounds of ||beta^avg[i]||_2 the screen's error bound used;
+ *   which = 4: bin_norm, float32[max_batch N/w]: the upper bounds of ||beta^avg[i]||_2 the screen's error bound used;
  *   which = 5: tnorm_blk, float32[ceil(T/128)]: max_t ||c_t||_2 / sigma_t per block of 128 templates;
  *   which = 6: the final first-stage candidate list of the last rbmf_filter on the device (what rbmf_get_candidates
  *              copies; min(n_candidates, max_candidates) valid rbmf_candidate records; *bytes = capacity in bytes).
@@ -181,8 +215,15 @@ int32_t rbmf_last_cuda_error(const rbmf_plan* plan);
  *       tensor-core kernels against ordinary arithmetic; orders of magnitude slower);
  *   RBMF_DIAG_SINGLE_CTA_SCREEN (value 0/1): RBMF_GEMM_SCREEN uses its single-CTA kernel instead of the 2-CTA
  *       cluster kernel that multicasts the coefficient tile (the fallback for devices that cannot co-schedule
- *       clusters of 2); takes effect at the next rbmf_filter. */
-typedef enum { RBMF_DIAG_STAGE1_FP32_CHECK = 1, RBMF_DIAG_SINGLE_CTA_SCREEN = 2 } rbmf_diag_option;
+ *       clusters of 2); takes effect at the next rbmf_filter;
+ *   RBMF_DIAG_STAGE2_PER_CANDIDATE (value 0/1): step a6 with the one-warp-per-candidate kernel (the fallback for
+ *       w = 32 with k > 608, where one bin's block of beta does not fit in shared memory) instead of the kernel that
+ *       regroups the candidates by bin. */
+typedef enum {
+    RBMF_DIAG_STAGE1_FP32_CHECK = 1,
+    RBMF_DIAG_SINGLE_CTA_SCREEN = 2,
+    RBMF_DIAG_STAGE2_PER_CANDIDATE = 3
+} rbmf_diag_option;
 rbmf_status rbmf_diag_set(rbmf_plan* plan, int32_t option, int32_t value);
 
 #ifdef __cplusplus

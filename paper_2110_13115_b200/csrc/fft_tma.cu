@@ -293,7 +293,9 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chu
     group_sync(g);
 
     // ---- stage 1 + inter-pass twiddle + store of Y (in place in the beta array) -------------------------------
-    float2* yrow = a.beta + ((size_t)chunk * (size_t)a.N + (size_t)j2 * L1) * C + col;
+    // virtual chunk = c * nb + b: basis chunk c against segment b's strain; beta arrays are [segment][chunk]
+    const int bc = chunk / a.nb, bs = chunk - bc * a.nb;
+    float2* yrow = a.beta + ((size_t)(bs * a.nchunk + bc) * (size_t)a.N + (size_t)j2 * L1) * C + col;
     const float2* e2 = e2s + line * (R1 + 2);
 #pragma unroll
     for (int bb = 0; bb < NB; ++bb) {
@@ -348,7 +350,10 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, const CUtensorMap* tm
     const int col = gt % C, line = (gt / C) % SUB, wk = gt / (C * SUB);
     const int slot = line * C + col;
     const int w = a.w;
-    const int gcol = chunk * C + col;
+    const int bc = chunk / a.nb, bs = chunk - bc * a.nb;   // virtual chunk = c * nb + b (see p1_tile)
+    const int zc = bs * a.nchunk + bc;                     // the chunk's block of the beta array
+    const int gcol = bc * C + col;
+    const int bin0 = bs * a.Mseg;                          // the segment's first row of the planes
 
     float2 u[R0];
 #pragma unroll
@@ -384,7 +389,7 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, const CUtensorMap* tm
     if (gt == 0) {
         constexpr int BR = L2 < 256 ? L2 : 256;
         const int x = (n1_0 + rd * SUB) * C * 2;
-        for (int p = 0; p < L2 / BR; ++p) tma_store_3d(tmY, smem_u32(B + (size_t)p * BR * RB), x, p * BR, chunk);
+        for (int p = 0; p < L2 / BR; ++p) tma_store_3d(tmY, smem_u32(B + (size_t)p * BR * RB), x, p * BR, zc);
         bulk_commit();
     }
     if (rd == 0) {
@@ -409,7 +414,7 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, const CUtensorMap* tm
         }
         if (rd == rounds - 1) {
             // bins n1_0 / w + (L1 / w) n2, n2 = gt / C + it GT / C: a constant element stride between iterations
-            const size_t e0 = ((size_t)(gcol / 32) * a.M + n1_0 / w + (size_t)(L1 / w) * (gt / C)) * 64 + (gcol % 32) * 2;
+            const size_t e0 = ((size_t)(gcol / 32) * a.M + bin0 + n1_0 / w + (size_t)(L1 / w) * (gt / C)) * 64 + (gcol % 32) * 2;
             const size_t es = (size_t)(L1 / w) * (GT / C) * 64;
             const float iw = a.inv_w;
             if (a.plane_fp16) {
@@ -435,7 +440,7 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, const CUtensorMap* tm
             float2 sum = row[(rb * w) * C];
 #pragma unroll 1
             for (int rr = 1; rr < w; ++rr) sum = cadd(sum, row[(rb * w + rr) * C]);
-            store_planes(a, (n1_0 + rd * SUB + rb * w) / w + (L1 / w) * n2, gcol,
+            store_planes(a, bin0 + (n1_0 + rd * SUB + rb * w) / w + (L1 / w) * n2, gcol,
                          make_float2(sum.x * a.inv_w, sum.y * a.inv_w));
         }
     }
@@ -472,7 +477,8 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
     const int rounds = span / K2::SUB;
     const int n2t = L1 / span;                                     // pass-2 items per chunk
     const int per = n1t + n2t;
-    const int total = a.nchunk * per;
+    const int nvc = a.nchunk * a.nb;                               // virtual chunks (basis chunk, segment)
+    const int total = nvc * per;
 
     for (int i = threadIdx.x; i < L1; i += NT) tw_a[i] = a.tw1_a[i];
     for (int i = threadIdx.x; i < L2; i += NT) tw_b[i] = a.tw1_b[i];
@@ -512,7 +518,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                     // queue order, pass 1 running LA chunks ahead of pass 2:
                     //   P1(0) .. P1(LA-1) | P1(LA) P2(0) | P1(LA+1) P2(1) | ... | P2(n-LA) | ... | P2(n-1)
                     const int LA = a.lookahead;
-                    const int la = a.nchunk < LA ? a.nchunk : LA, nfull = a.nchunk - la;
+                    const int la = nvc < LA ? nvc : LA, nfull = nvc - la;
                     bool first = true;
                     if (t < la * n1t) {
                         chunk = t / n1t; idx = t - chunk * n1t;
@@ -531,7 +537,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                         type = TILE_P1;
                     } else {
                         type = TILE_P2; idx *= span; rd = 0;
-                        wait_counter(a.sched + 16 + chunk, (unsigned)n1t);   // all of the chunk's Y is in L2
+                        wait_counter(a.sched + kSchedBase + chunk, (unsigned)n1t);   // all of the chunk's Y is in L2
                     }
                 } else if (!it_open[g ^ 1]) {
                     type = TILE_STOP;
@@ -549,18 +555,22 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                 constexpr uint32_t basis_bytes = (uint32_t)H * K1::RB * 8, strain_bytes = (uint32_t)K1::SUB * H * 8;
                 if (lane == 0) mbar_expect_tx(full_bar(buf, g), basis_bytes + strain_bytes);
                 __syncwarp();
-                const float2* src = a.basisP + ((size_t)chunk * n1t + idx) * (size_t)(H * K1::RB);
+                const int bc = chunk / a.nb, bs = chunk - bc * a.nb;
+                // a basis chunk is streamed from HBM once per call: later segments of a batch find it in L2
+                const unsigned long long pol_basis = bs == a.nb - 1 ? pol_first : pol_last;
+                const float2* src = a.basisP + ((size_t)bc * n1t + idx) * (size_t)(H * K1::RB);
                 if (K1::PAD) {
                     for (int p = lane; p < H / 32; p += 32)
                         bulk_g2s(dst + (uint32_t)(33 * p) * K1::RB * 8, src + (size_t)p * 32 * K1::RB, 32 * K1::RB * 8,
-                                 full_bar(buf, g), pol_first);
+                                 full_bar(buf, g), pol_basis);
                 } else if (lane == 0) {
-                    bulk_g2s(dst, src, basis_bytes, full_bar(buf, g), pol_first);
+                    bulk_g2s(dst, src, basis_bytes, full_bar(buf, g), pol_basis);
                 }
                 if (lane >= 32 - K1::SUB) {   // one copy per line (padded rows, see Cfg::SPAD)
                     const int l = 31 - lane;
                     bulk_g2s(dst + (uint32_t)(K1::idx(H) * K1::RB + l * (H + K1::SPAD)) * 8,
-                             a.dsT + ((size_t)idx * K1::SUB + l) * H, (uint32_t)H * 8, full_bar(buf, g), pol_last);
+                             a.dsT + (size_t)bs * ((size_t)H * L2) + ((size_t)idx * K1::SUB + l) * H, (uint32_t)H * 8,
+                             full_bar(buf, g), pol_last);
                 }
             } else if (type == TILE_P2) {
                 constexpr int BR = L2 < 256 ? L2 : 256;   // rows per tensor copy
@@ -568,7 +578,8 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                 __syncwarp();
                 const int x = (idx + rd * K2::SUB) * C * 2;   // floats along the (n1, col) axis
                 for (int p = lane; p < L2 / BR; p += 32)
-                    tma_load_3d(dst + (uint32_t)K2::idx(p * BR) * K2::RB * 8, &tmY, full_bar(buf, g), x, p * BR, chunk);
+                    tma_load_3d(dst + (uint32_t)K2::idx(p * BR) * K2::RB * 8, &tmY, full_bar(buf, g), x, p * BR,
+                                (chunk % a.nb) * a.nchunk + chunk / a.nb);
                 if (rd + 1 < rounds) { it_open[g] = true; it_chunk[g] = chunk; it_n1[g] = idx; it_rd[g] = rd + 1; }
                 else it_open[g] = false;
             } else {
@@ -600,7 +611,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                     // release: the group's Y stores happen before this fence through the barrier above (bar.sync
                     // orders them at CTA scope, the gpu-scope fence is cumulative), then the counter is bumped
                     __threadfence();
-                    atomicAdd(a.sched + 16 + chunk, 1u);
+                    atomicAdd(a.sched + kSchedBase + chunk, 1u);
                 }
             }
         }

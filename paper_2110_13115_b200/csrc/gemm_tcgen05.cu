@@ -215,6 +215,11 @@ __device__ __forceinline__ void epilogue_tile(const GemmArgs& g, uint32_t taddr,
     if (lane == 0) base = atomicAdd(g.counters, (unsigned long long)total);
     base = __shfl_sync(0xffffffffu, base, 0);
     unsigned long long idx = base + (unsigned long long)(incl - cnt);
+    if (cnt > 0 && idx < g.cand_cap) {
+        // histogram of the entries actually written, per bin: stage 2 regroups the list by bin (stage2_bybin.cu)
+        const unsigned long long room = g.cand_cap - idx;
+        atomicAdd(g.bin_count + bin, (unsigned)(room < (unsigned long long)cnt ? room : (unsigned long long)cnt));
+    }
 #pragma unroll 1
     for (int ch = 0; ch < NCH; ++ch) {
         const uint32_t m = mask[ch];

@@ -181,7 +181,7 @@ cudaError_t launch_prep_coeffs(const float2* coeffs, const float* sigma, float2*
 // within 2^-11 relative (+ 2^-25 absolute in the subnormal range) of the fp32 ones, hence the inflation.
 // Eight lanes share a bin (16 bytes each of its 128-byte K-block row); consecutive lanes read consecutive bytes.
 __global__ void __launch_bounds__(256) bin_norm_kernel(const uint16_t* __restrict__ plane, float* __restrict__ bin_norm,
-                                                       int M, int nkb) {
+                                                       int M, int Mplane, int nkb) {
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long bin = gid >> 3;
     const int piece = (int)(gid & 7);
@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(256) bin_norm_kernel(const uint16_t* __restric
     if (bin < M) {
         const uint4* p = reinterpret_cast<const uint4*>(plane) + bin * 8 + piece;
         for (int kb = 0; kb < nkb; ++kb) {
-            const uint4 v = __ldg(p + (size_t)kb * M * 8);
+            const uint4 v = __ldg(p + (size_t)kb * Mplane * 8);
             const unsigned wds[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
@@ -205,28 +205,29 @@ __global__ void __launch_bounds__(256) bin_norm_kernel(const uint16_t* __restric
     if (bin < M && piece == 0) bin_norm[bin] = sqrtf(acc) * (1.0f + 0x1p-9f) + 1e-5f;
 }
 
-cudaError_t launch_bin_norm(const uint16_t* plane_h16, float* bin_norm, int M, int nkb, cudaStream_t st) {
+// M = bins to process (all segments of the batch), Mplane = rows of the plane (its K-block stride)
+cudaError_t launch_bin_norm(const uint16_t* plane_h16, float* bin_norm, int M, int Mplane, int nkb, cudaStream_t st) {
     const long long threads = (long long)M * 8;
-    bin_norm_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(plane_h16, bin_norm, M, nkb);
+    bin_norm_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(plane_h16, bin_norm, M, Mplane, nkb);
     return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------ strain prep
-// dsT[j2][j1] = s d[j1 L2 + j2], j1 < L1/2 (s = sqrt(2/N)): the strain in the order pass 1
-// of the FFT reads it.
+// dsT[b][j2][j1] = s d_b[j1 L2 + j2], j1 < L1/2 (s = sqrt(2/N)): the strain of segment b (blockIdx.y;
+// N/2 + 1 bins per segment on input) in the order pass 1 of the FFT reads it.
 __global__ void prep_strain_kernel(const float2* __restrict__ strain, float2* __restrict__ dsT, int logL1,
                                    int logL2, float scale) {
     const int L2 = 1 << logL2, H = (1 << logL1) / 2;
     const int j = blockIdx.x * blockDim.x + threadIdx.x;   // j = j1 L2 + j2 < N/2
     if (j >= H * L2) return;
-    const float2 d = strain[j];
-    dsT[(size_t)(j % L2) * H + j / L2] = make_float2(d.x * scale, d.y * scale);
+    const float2 d = strain[(size_t)blockIdx.y * ((size_t)H * L2 + 1) + j];
+    dsT[(size_t)blockIdx.y * ((size_t)H * L2) + (size_t)(j % L2) * H + j / L2] = make_float2(d.x * scale, d.y * scale);
 }
 
-cudaError_t launch_prep_strain(const float2* strain, float2* dsT, int logL1, int logL2, float scale,
+cudaError_t launch_prep_strain(const float2* strain, float2* dsT, int logL1, int logL2, float scale, int nb,
                                cudaStream_t st) {
     const int n_half = 1 << (logL1 + logL2 - 1);
-    prep_strain_kernel<<<(n_half + 255) / 256, 256, 0, st>>>(strain, dsT, logL1, logL2, scale);
+    prep_strain_kernel<<<dim3((n_half + 255) / 256, nb), 256, 0, st>>>(strain, dsT, logL1, logL2, scale);
     return cudaGetLastError();
 }
 

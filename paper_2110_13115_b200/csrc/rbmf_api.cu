@@ -17,7 +17,8 @@ inline int ilog2(int64_t x) { int l = 0; while ((int64_t(1) << l) < x) ++l; retu
 
 struct Layout {
     size_t basisP, beta, bavg_hi, bavg_lo, c_hi, c_lo, c_h16, tnorm_blk, bin_norm, cs, tw1_a, tw1_b, twN, dsT,
-        cand, cand2, counters, sched, strain_stage, trig_stage, total;
+        cand, cand2, cand3, bin_count, bin_start, items, counters, sched, strain_stage, trig_stage, twF, r2c_s, r2c_z, total;
+    size_t sched_bytes;
     size_t plane_bytes;
 };
 
@@ -33,9 +34,11 @@ struct rbmf_plan {
     int logN1, logN2;   // FFT: N = 2^logN1 * 2^logN2 (pass 1 length, pass 2 length)
     int fft_grid;       // persistent CTAs of the fused FFT kernel
     int64_t max_cand, max_trig;
+    int max_batch;      // segments rbmf_filter_batch may take at once (rbmf_plan_set_batch; default 1)
+    int last_nb;        // segments of the last rbmf_filter / rbmf_filter_batch
     int gemm_impl;
     int last_impl;      // gemm_impl of the last rbmf_filter (decides which candidate list / counter is final)
-    int diag_fp32_check, diag_single_cta;   // rbmf_diag_set
+    int diag_fp32_check, diag_single_cta, diag_stage2_per_cand;   // rbmf_diag_set
     int timing;
     cudaStream_t stream;
     uint8_t* ws;
@@ -57,11 +60,12 @@ Layout make_layout(const rbmf_plan* p) {
     Layout L;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
-    const size_t k = (size_t)p->k, N = (size_t)p->N, M = (size_t)p->M;
+    const size_t k = (size_t)p->k, N = (size_t)p->N, B = (size_t)p->max_batch;
+    const size_t M = (size_t)p->M * B;   // rows of the planes: all segments of a batch, segment-major
     const size_t nkb = (k + 31) / 32;
     L.plane_bytes = nkb * M * 64 * 2;
     L.basisP = take((size_t)p->n_half * k * 8);
-    L.beta = take(N * k * 8);
+    L.beta = take(B * N * k * 8);
     L.bavg_hi = take(L.plane_bytes);
     L.bavg_lo = take(L.plane_bytes);
     L.c_hi = take((size_t)p->Tpad * 2 * 2 * k * 2);
@@ -73,13 +77,22 @@ Layout make_layout(const rbmf_plan* p) {
     L.tw1_a = take(((size_t)1 << p->logN1) * 8);
     L.tw1_b = take(((size_t)1 << p->logN2) * 8);
     L.twN = take(((size_t)1 << p->logN2) * (size_t)(fft_r0(p->logN1) + fft_r1(p->logN1)) * 8);   // two factor tables
-    L.dsT = take((size_t)p->n_half * 8);
+    L.dsT = take(B * (size_t)p->n_half * 8);
     L.cand = take((size_t)p->max_cand * sizeof(rbmf_candidate));
     L.cand2 = take((size_t)p->max_cand * sizeof(rbmf_candidate));
-    L.counters = take(64 + (size_t)kSchedWords * 4);   // counters, then the FFT scheduler words: one memset
-    L.sched = L.counters + 64;
-    L.strain_stage = take((size_t)(p->n_half + 1) * 8);
+    L.cand3 = take((size_t)p->max_cand * sizeof(rbmf_candidate));
+    L.bin_start = take(M * 4);
+    L.items = take(((size_t)p->max_cand / kStage2Chunk + M + 1) * sizeof(int4));
+    // counters, the FFT scheduler words and the per-bin histogram are contiguous: one memset per call
+    L.sched_bytes = ((size_t)kSchedBase + (size_t)kMaxChunks * B) * 4;
+    L.counters = take(kCounterBytes + L.sched_bytes + M * 4);
+    L.sched = L.counters + kCounterBytes;
+    L.bin_count = L.sched + L.sched_bytes;
+    L.strain_stage = take(B * (size_t)(p->n_half + 1) * 8);
     L.trig_stage = take((size_t)p->max_trig * sizeof(rbmf_trigger));
+    L.twF = take((size_t)p->n_half * 8);                 // front end: e^{-2 pi i m / N}, m < N/2
+    L.r2c_s = take(B * (size_t)p->n_half * 8);
+    L.r2c_z = take(B * (size_t)p->n_half * 8);
     L.total = off;
     return L;
 }
@@ -148,7 +161,7 @@ rbmf_status make_map_planes(rbmf_plan* plan, CUtensorMap* map, void* base, uint6
 // of beta[n1 + L1 j2]); box = sub2 lines x C columns (re, im) wide, up to 256 rows j2, unswizzled.
 rbmf_status make_map_y(rbmf_plan* plan, CUtensorMap* map, void* base) {
     const uint64_t L1 = 1ull << plan->logN1, L2 = 1ull << plan->logN2;
-    const cuuint64_t dims[3] = {2 * kFftC * L1, L2, (cuuint64_t)(plan->k / kFftC)};
+    const cuuint64_t dims[3] = {2 * kFftC * L1, L2, (cuuint64_t)(plan->k / kFftC) * (cuuint64_t)plan->max_batch};
     const cuuint64_t strides[2] = {L1 * kFftC * 8, (cuuint64_t)plan->N * kFftC * 8};
     const cuuint32_t box[3] = {(cuuint32_t)(2 * kFftC * fft_sub(plan->logN2)), (cuuint32_t)(L2 < 256 ? L2 : 256), 1};
     return encode_map(plan, map, base, 3, dims, strides, box, CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
@@ -179,6 +192,7 @@ rbmf_status rbmf_plan_create(rbmf_plan** out, int64_t N, double fs, double f_low
     if (p->j_low >= p->n_half) { delete p; return RBMF_ERR_ARG; }
     p->max_cand = int64_t(1) << 22;
     p->max_trig = int64_t(1) << 22;
+    p->max_batch = 1;
     p->gemm_impl = RBMF_GEMM_SCREEN;
     refresh(p);
     *out = p;
@@ -203,6 +217,16 @@ rbmf_status rbmf_plan_set_capacity(rbmf_plan* plan, int64_t max_candidates, int6
         return RBMF_ERR_ARG;
     plan->max_cand = max_candidates;
     plan->max_trig = max_triggers;
+    refresh(plan);
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_plan_set_batch(rbmf_plan* plan, int32_t max_batch) {
+    if (!plan) return RBMF_ERR_ARG;
+    if (plan->have_ws) return RBMF_ERR_STATE;
+    // time_index = segment * N + n is an int32
+    if (max_batch < 1 || (int64_t)max_batch * plan->N > (int64_t(1) << 31) - 1) return RBMF_ERR_ARG;
+    plan->max_batch = max_batch;
     refresh(plan);
     return RBMF_OK;
 }
@@ -244,11 +268,14 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     const Layout& L = plan->lay;
     CK(launch_init_tables(at<float2>(plan, L.tw1_a), at<float2>(plan, L.tw1_b), at<float2>(plan, L.twN), plan->logN1,
                           plan->logN2, plan->stream));
-    CK(cudaMemsetAsync(plan->ws + L.counters, 0, 64 + (size_t)kSchedWords * 4, plan->stream));
+    CK(cudaMemsetAsync(plan->ws + L.counters, 0, kCounterBytes + L.sched_bytes + (size_t)plan->M * plan->max_batch * 4,
+                       plan->stream));
     // columns of the last K block beyond k are never written by the FFT: they must be finite (they meet zeros)
     CK(cudaMemsetAsync(plan->ws + L.bavg_hi, 0, L.plane_bytes, plan->stream));
     CK(cudaMemsetAsync(plan->ws + L.bavg_lo, 0, L.plane_bytes, plan->stream));
     CK(gemm_tcgen05_configure());
+    CK(r2c_configure());
+    CK(launch_r2c_table(at<float2>(plan, L.twF), plan->N, plan->stream));
     {
         size_t smem = 0;
         CK(fft_tma_configure(plan->logN1, plan->logN2, &smem));
@@ -259,8 +286,9 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     const uint64_t k2 = 2 * (uint64_t)plan->k;
     const uint64_t nkb = (uint64_t)((plan->k + 31) / 32);
     if ((s = make_map_y(plan, &plan->tmY, plan->ws + L.beta)) != RBMF_OK) return s;
-    if ((s = make_map_planes(plan, &plan->tmA_hi, plan->ws + L.bavg_hi, (uint64_t)plan->M, nkb)) != RBMF_OK) return s;
-    if ((s = make_map_planes(plan, &plan->tmA_lo, plan->ws + L.bavg_lo, (uint64_t)plan->M, nkb)) != RBMF_OK) return s;
+    const uint64_t Mplane = (uint64_t)plan->M * (uint64_t)plan->max_batch;
+    if ((s = make_map_planes(plan, &plan->tmA_hi, plan->ws + L.bavg_hi, Mplane, nkb)) != RBMF_OK) return s;
+    if ((s = make_map_planes(plan, &plan->tmA_lo, plan->ws + L.bavg_lo, Mplane, nkb)) != RBMF_OK) return s;
     if ((s = make_map_rows(plan, &plan->tmB_hi, plan->ws + L.c_hi, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
     if ((s = make_map_rows(plan, &plan->tmB_lo, plan->ws + L.c_lo, 2 * (uint64_t)plan->Tpad, k2, 2 * kGemmTT)) != RBMF_OK) return s;
     // fp16 data through a 16-bit tensor map: TMA only moves bytes, the element type is irrelevant without OOB fill
@@ -296,22 +324,44 @@ rbmf_status rbmf_set_coeffs(rbmf_plan* plan, const void* coeffs_dev, const float
     return RBMF_OK;
 }
 
+rbmf_status rbmf_prepare_strain(rbmf_plan* plan, const float* x_dev, const float* inv_asd_dev, int32_t n_segments,
+                                void* strain_out_dev) {
+    if (!plan || !x_dev || !strain_out_dev) return RBMF_ERR_ARG;
+    if (!plan->have_ws) return RBMF_ERR_STATE;
+    if (n_segments < 1 || n_segments > plan->max_batch) return RBMF_ERR_ARG;
+    if (((uintptr_t)x_dev % 8) != 0 || ((uintptr_t)strain_out_dev % 8) != 0) return RBMF_ERR_ARG;
+    const Layout& L = plan->lay;
+    CK(launch_r2c(x_dev, inv_asd_dev, at<float2>(plan, L.r2c_s), at<float2>(plan, L.r2c_z), (float2*)strain_out_dev,
+                  at<float2>(plan, L.twF), plan->logN1 + plan->logN2, n_segments, plan->stream));
+    return RBMF_OK;
+}
+
 rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage1, float thr_stage2,
                         rbmf_trigger* out_dev, int64_t* n_out_dev) {
+    return rbmf_filter_batch(plan, strain_dev, 1, thr_stage1, thr_stage2, out_dev, n_out_dev);
+}
+
+rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n_segments, float thr_stage1,
+                              float thr_stage2, rbmf_trigger* out_dev, int64_t* n_out_dev) {
     if (!plan || !strain_dev || !out_dev || !n_out_dev) return RBMF_ERR_ARG;
     if (!(thr_stage1 > 0.f) || !(thr_stage2 > 0.f)) return RBMF_ERR_ARG;
     if (!plan->have_ws || !plan->have_basis || !plan->have_coeffs) return RBMF_ERR_STATE;
+    if (n_segments < 1 || n_segments > plan->max_batch) return RBMF_ERR_ARG;
     const Layout& L = plan->lay;
     cudaStream_t st = plan->stream;
     const bool tm = plan->timing != 0;
+    const int nb = n_segments;
+    const int64_t Mtot = plan->M * nb;                       // bins of the whole batch
+    const int64_t Mplane = plan->M * plan->max_batch;        // rows of the planes
     unsigned long long* counters = at<unsigned long long>(plan, L.counters);
 
     if (tm) CK(cudaEventRecord(plan->ev[0], st));
-    CK(cudaMemsetAsync(counters, 0, 64 + (size_t)kSchedWords * 4, st));   // counters + FFT scheduler words
+    // counters + FFT scheduler words + per-bin histogram
+    CK(cudaMemsetAsync(counters, 0, kCounterBytes + L.sched_bytes + (size_t)Mtot * 4, st));
     CK(launch_prep_strain((const float2*)strain_dev, at<float2>(plan, L.dsT), plan->logN1, plan->logN2,
-                          (float)sqrt(2.0 / (double)plan->N), st));
+                          (float)sqrt(2.0 / (double)plan->N), nb, st));
 
-    // ---- kernel 1: a1-a3, one persistent launch ------------------------------------------------
+    // ---- kernel 1: a1-a3, one persistent launch over all (basis chunk, segment) pairs ----------------
     FftArgs a;
     memset(&a, 0, sizeof(a));
     a.basisP = at<float2>(plan, L.basisP); a.dsT = at<float2>(plan, L.dsT);
@@ -319,7 +369,8 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     a.beta = at<float2>(plan, L.beta);
     a.plane_hi = at<uint16_t>(plan, L.bavg_hi); a.plane_lo = at<uint16_t>(plan, L.bavg_lo);
     a.sched = at<unsigned>(plan, L.sched);
-    a.N = plan->N; a.M = (int)plan->M; a.nchunk = plan->k / kFftC; a.w = plan->w; a.inv_w = 1.0f / (float)plan->w;
+    a.N = plan->N; a.M = (int)Mplane; a.Mseg = (int)plan->M; a.nb = nb;
+    a.nchunk = plan->k / kFftC; a.w = plan->w; a.inv_w = 1.0f / (float)plan->w;
     const bool screen = plan->gemm_impl == RBMF_GEMM_SCREEN && !plan->diag_fp32_check;
     a.plane_fp16 = screen ? 1 : 0;
     {
@@ -335,20 +386,21 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     }
     CK(launch_fft_tma(plan->tmY, a, plan->logN1, plan->logN2, plan->fft_grid, st));
     if (screen)
-        CK(launch_bin_norm(at<uint16_t>(plan, L.bavg_hi), at<float>(plan, L.bin_norm), (int)plan->M,
+        CK(launch_bin_norm(at<uint16_t>(plan, L.bavg_hi), at<float>(plan, L.bin_norm), (int)Mtot, (int)Mplane,
                            (plan->k + 31) / 32, st));
     if (tm) CK(cudaEventRecord(plan->ev[1], st));
 
-    // ---- kernel 2: a4-a5 -----------------------------------------------------------------------
+    // ---- kernel 2: a4-a5 over the bins of all segments ------------------------------------------
     GemmArgs g;
     memset(&g, 0, sizeof(g));
     g.cand = at<rbmf_candidate>(plan, L.cand);
+    g.bin_count = at<unsigned>(plan, L.bin_count);
     g.counters = counters;
     g.cand_cap = (unsigned long long)plan->max_cand;
     g.thr1_sq = thr_stage1 * thr_stage1;
-    g.T = plan->T; g.M = (int)plan->M; g.k2 = 2 * plan->k;
+    g.T = plan->T; g.M = (int)Mtot; g.k2 = 2 * plan->k;
     g.num_tb = plan->Tpad / kGemmTT;
-    g.num_ib = (int)(plan->M / kGemmBM);
+    g.num_ib = (int)(Mtot / kGemmBM);
     g.group = 32;   // template blocks per raster group: 32 coefficient tiles (8 MB fp16) stay L2-resident
     if (screen) {
         // Bound of |R_fp16 - R| for the one-product fp16 screen (derivation: gemm_tcgen05.cu header): operand
@@ -374,11 +426,11 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
         CK(launch_gemm_tcgen05(plan->tmA_hi, plan->tmA_lo, plan->tmB_hi, plan->tmB_lo, g, plan->num_sms, st));
     } else {
         CK(launch_gemm_simt(at<uint16_t>(plan, L.bavg_hi), at<uint16_t>(plan, L.bavg_lo), at<uint16_t>(plan, L.c_hi),
-                            at<uint16_t>(plan, L.c_lo), g, st));
+                            at<uint16_t>(plan, L.c_lo), g, (int)Mplane, st));
     }
     if (tm) CK(cudaEventRecord(plan->ev[2], st));
 
-    // ---- kernel 3: a6 --------------------------------------------------------------------------
+    // ---- kernel 3: a6 (candidates regrouped by bin; one warp per candidate where a bin's block is too large) ----
     Stage2Args s2;
     memset(&s2, 0, sizeof(s2));
     s2.cand = g.cand; s2.cs = at<float2>(plan, L.cs); s2.beta = at<float2>(plan, L.beta);
@@ -386,10 +438,16 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
     s2.confirmed = at<rbmf_candidate>(plan, L.cand2); s2.thr1_sq = g.thr1_sq; s2.screen = screen ? 1 : 0;
     s2.cand_cap = (unsigned long long)plan->max_cand; s2.trig_cap = (unsigned long long)plan->max_trig;
     s2.thr2_sq = thr_stage2 * thr_stage2; s2.k = plan->k; s2.w = plan->w; s2.N = plan->N;
-    CK(launch_stage2(s2, plan->num_sms, st));
+    s2.bin_count = g.bin_count; s2.bin_start = at<unsigned>(plan, L.bin_start); s2.items = at<int4>(plan, L.items);
+    s2.sorted = at<rbmf_candidate>(plan, L.cand3);
+    s2.Mseg = (int)plan->M; s2.Mtot = (int)Mtot; s2.seg_stride = (size_t)plan->N * plan->k;
+    s2.smem_bytes = stage2_bybin_smem(plan->w, plan->k);
+    if (s2.smem_bytes > 0 && !plan->diag_stage2_per_cand) CK(launch_stage2_bybin(s2, plan->num_sms, st));
+    else CK(launch_stage2(s2, plan->num_sms, st));
     CK(cudaMemcpyAsync(n_out_dev, counters + 1, 8, cudaMemcpyDeviceToDevice, st));
     if (tm) CK(cudaEventRecord(plan->ev[3], st));
     plan->filtered = true;
+    plan->last_nb = nb;
     plan->last_impl = screen ? (int)RBMF_GEMM_SCREEN : (int)RBMF_GEMM_TCGEN05;
     return RBMF_OK;
 }
@@ -423,6 +481,7 @@ rbmf_status rbmf_diag_set(rbmf_plan* plan, int32_t option, int32_t value) {
     switch (option) {
         case RBMF_DIAG_STAGE1_FP32_CHECK: plan->diag_fp32_check = value ? 1 : 0; return RBMF_OK;
         case RBMF_DIAG_SINGLE_CTA_SCREEN: plan->diag_single_cta = value ? 1 : 0; return RBMF_OK;
+        case RBMF_DIAG_STAGE2_PER_CANDIDATE: plan->diag_stage2_per_cand = value ? 1 : 0; return RBMF_OK;
         default: return RBMF_ERR_ARG;
     }
 }
@@ -446,16 +505,23 @@ rbmf_status rbmf_get_candidates(rbmf_plan* plan, rbmf_candidate* out_host, int64
 
 rbmf_status rbmf_filter_host(rbmf_plan* plan, const void* strain_host, float thr_stage1, float thr_stage2,
                              rbmf_trigger* out_host, int64_t capacity_out, int64_t* n_out_host) {
+    return rbmf_filter_batch_host(plan, strain_host, 1, thr_stage1, thr_stage2, out_host, capacity_out, n_out_host);
+}
+
+rbmf_status rbmf_filter_batch_host(rbmf_plan* plan, const void* strain_host, int32_t n_segments, float thr_stage1,
+                                   float thr_stage2, rbmf_trigger* out_host, int64_t capacity_out,
+                                   int64_t* n_out_host) {
     if (!plan || !strain_host || !out_host || !n_out_host || capacity_out < 1) return RBMF_ERR_ARG;
     if (!plan->have_ws || !plan->have_basis || !plan->have_coeffs) return RBMF_ERR_STATE;
+    if (n_segments < 1 || n_segments > plan->max_batch) return RBMF_ERR_ARG;
     if (capacity_out > plan->max_trig) capacity_out = plan->max_trig;
     const Layout& L = plan->lay;
-    const size_t strain_bytes = (size_t)(plan->N / 2 + 1) * 8;
+    const size_t strain_bytes = (size_t)n_segments * (size_t)(plan->N / 2 + 1) * 8;
     uint8_t* strain_dev = plan->ws + L.strain_stage;
     rbmf_trigger* trig_dev = (rbmf_trigger*)(plan->ws + L.trig_stage);
-    int64_t* n_dev = (int64_t*)(plan->ws + L.counters + 32);
+    int64_t* n_dev = (int64_t*)(plan->ws + L.counters + 64);   // counter word 8
     CK(cudaMemcpyAsync(strain_dev, strain_host, strain_bytes, cudaMemcpyHostToDevice, plan->stream));
-    rbmf_status s = rbmf_filter(plan, strain_dev, thr_stage1, thr_stage2, trig_dev, n_dev);
+    rbmf_status s = rbmf_filter_batch(plan, strain_dev, n_segments, thr_stage1, thr_stage2, trig_dev, n_dev);
     if (s != RBMF_OK) return s;
     int64_t nc = 0, nt = 0;
     s = rbmf_get_counts(plan, &nc, &nt);
@@ -475,11 +541,11 @@ rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_p
     if (!plan->have_ws) return RBMF_ERR_STATE;
     const Layout& L = plan->lay;
     switch (which) {
-        case 0: *dev_ptr = plan->ws + L.beta; *bytes = (size_t)plan->N * plan->k * 8; break;
+        case 0: *dev_ptr = plan->ws + L.beta; *bytes = (size_t)plan->max_batch * plan->N * plan->k * 8; break;
         case 1: *dev_ptr = plan->ws + L.bavg_hi; *bytes = L.plane_bytes; break;
         case 2: *dev_ptr = plan->ws + L.bavg_lo; *bytes = L.plane_bytes; break;
         case 3: *dev_ptr = plan->ws + L.cand; *bytes = (size_t)plan->max_cand * sizeof(rbmf_candidate); break;
-        case 4: *dev_ptr = plan->ws + L.bin_norm; *bytes = (size_t)plan->M * 4; break;
+        case 4: *dev_ptr = plan->ws + L.bin_norm; *bytes = (size_t)plan->M * plan->max_batch * 4; break;
         case 5: *dev_ptr = plan->ws + L.tnorm_blk; *bytes = (size_t)(plan->Tpad / kGemmTT) * 4; break;
         case 6:
             *dev_ptr = plan->ws + (plan->last_impl == RBMF_GEMM_SCREEN ? L.cand2 : L.cand);
@@ -509,8 +575,9 @@ rbmf_status rbmf_get_stage_ms(rbmf_plan* plan, float ms[4]) {
 
 rbmf_status rbmf_launches_per_filter(const rbmf_plan* plan, int32_t* n) {
     if (!plan || !n) return RBMF_ERR_ARG;
-    // prep_strain + fused FFT + (screen: bin norms) + GEMM + stage 2
-    *n = (plan->gemm_impl == RBMF_GEMM_SCREEN && !plan->diag_fp32_check) ? 5 : 4;
+    // prep_strain + fused FFT + (screen: bin norms) + GEMM + stage 2 (by bin: alloc, scatter, score)
+    const int s2 = (stage2_bybin_smem(plan->w, plan->k) > 0 && !plan->diag_stage2_per_cand) ? 3 : 1;
+    *n = ((plan->gemm_impl == RBMF_GEMM_SCREEN && !plan->diag_fp32_check) ? 4 : 3) + s2;
     return RBMF_OK;
 }
 

@@ -23,8 +23,14 @@ __host__ __device__ constexpr int fft_r1(int logL) { return (1 << logL) / fft_r0
 // lines (independent transforms) a 256-thread consumer group works on in lockstep = lines per tile
 __host__ __device__ constexpr int fft_sub(int logL) { return kFftThreads / (fft_r1(logL) * kFftC); }
 
-// Scheduler words (uint32) in the workspace: [0] ticket, [16 + c] pass-1 tiles done of chunk c.
-constexpr int kSchedWords = 16 + kMaxChunks;
+// Scheduler words (uint32) in the workspace: [0] ticket, [16 + v] pass-1 tiles done of virtual chunk v = c * nb + b
+// (c = chunk of 4 basis columns, b = segment of the batch): 16 + kMaxChunks * max_batch words.
+constexpr int kSchedBase = 16;
+// Counter block (uint64 words) at the head of the scheduler area, zeroed by every rbmf_filter:
+//   [0] stage-1 list entries requested by kernel 2, [1] triggers, [2] confirmed candidates (screen mode),
+//   [3] cursor of the by-bin candidate array, [4] stage-2 work items, [5] stage-2 ticket, [8] rbmf_filter_host's count.
+constexpr int kCounterBytes = 128;
+constexpr int kStage2Chunk = 128;   // candidates per stage-2 work item (one CTA of 4 warps)
 
 // Device views handed to the fused FFT kernel.
 struct FftArgs {
@@ -36,13 +42,15 @@ struct FftArgs {
     float2* beta;            // [chunk][n < N][C]; between the passes it holds Y[n1][j2] at index n1 + L1 j2
     uint16_t* plane_hi;      // [kb = col / 32][bin < M][64]: bf16 (re, im) of column col % 32
     uint16_t* plane_lo;
-    unsigned* sched;         // kSchedWords
+    unsigned* sched;         // kSchedBase + nchunk * nb words
     long long N;
-    int M;                   // N / w
+    int M;                   // rows of the planes = max_batch * N / w
     int nchunk;              // k / C
     int w;
     float inv_w;
-    int lookahead;           // chunks pass 1 runs ahead of pass 2 in the work queue (their Y must fit in L2)
+    int lookahead;           // (virtual) chunks pass 1 runs ahead of pass 2 in the work queue (their Y must fit in L2)
+    int nb;                  // segments of the batch: virtual chunk v = c * nb + b reads basis chunk c, strain b
+    int Mseg;                // bins per segment (N / w); segment b's bins are [b Mseg, (b + 1) Mseg) of the planes
     int plane_fp16;          // 1: write ONE fp16 plane (screen mode) into plane_hi; 0: bf16 hi + lo planes
 };
 
@@ -53,11 +61,12 @@ struct GemmArgs {
     float thr1;
     float kappa1, kappa2, slack;
     rbmf_candidate* cand;
+    unsigned* bin_count;            // per (segment, bin): entries written to `cand` (histogram for stage 2's grouping)
     unsigned long long* counters;   // [0] = candidates, [1] = triggers
     unsigned long long cand_cap;
     float thr1_sq;
     int T;                    // real templates (rows >= T are padding)
-    int M;                    // time bins N/w
+    int M;                    // time bins of the whole batch, nb * N / w
     int k2;                   // 2k (reals along K)
     int num_tb;               // template blocks  = Tpad / 128
     int num_ib;               // time-bin blocks  = M / 128
@@ -66,6 +75,15 @@ struct GemmArgs {
 
 struct Stage2Args {
     const rbmf_candidate* cand;
+    // by-bin path: candidates regrouped by bin (bin_count from kernel 2; alloc -> bin_start + items; scatter -> sorted)
+    unsigned* bin_count;
+    unsigned* bin_start;
+    int4* items;                 // {bin, first entry in `sorted`, entries (<= kStage2Chunk), 0}
+    rbmf_candidate* sorted;
+    int Mseg;                    // bins per segment (N / w); bin / Mseg = segment of the batch
+    int Mtot;                    // nb * Mseg
+    size_t seg_stride;           // float2 entries between the beta arrays of consecutive segments
+    int smem_bytes;              // dynamic shared memory of the score kernel (beta block of one bin)
     const float2* cs;         // T x k: conj(c_tk) / sigma_t
     const float2* beta;       // [chunk][n][C]
     rbmf_trigger* out;
@@ -88,15 +106,15 @@ cudaError_t launch_layout_basis(const float2* basis, float2* basisP, int k, int6
 cudaError_t launch_prep_coeffs(const float2* coeffs, const float* sigma, float2* cs, uint16_t* c_hi,
                                uint16_t* c_lo, uint16_t* c_h16, float* tnorm_blk, int T, int Tpad, int k,
                                cudaStream_t st);
-cudaError_t launch_bin_norm(const uint16_t* plane_h16, float* bin_norm, int M, int nkb, cudaStream_t st);
-cudaError_t launch_prep_strain(const float2* strain, float2* dsT, int logL1, int logL2, float scale,
+cudaError_t launch_bin_norm(const uint16_t* plane_h16, float* bin_norm, int M, int Mplane, int nkb, cudaStream_t st);
+cudaError_t launch_prep_strain(const float2* strain, float2* dsT, int logL1, int logL2, float scale, int nb,
                                cudaStream_t st);
 // Fused FFT (a1-a3): configure once per (logL1, logL2); then launch with one CTA per SM.  tmY: 3-D fp32 tensor map
 // over the beta array, dims {2 C L1, L2, k/C}, box {2 C sub2, min(L2, 256), 1} (the Y rows of a pass-2 tile).
 cudaError_t fft_tma_configure(int logL1, int logL2, size_t* smem_bytes);
 cudaError_t launch_fft_tma(const CUtensorMap& tmY, const FftArgs& a, int logL1, int logL2, int grid, cudaStream_t st);
 cudaError_t launch_gemm_simt(const uint16_t* a_hi, const uint16_t* a_lo, const uint16_t* c_hi,
-                             const uint16_t* c_lo, const GemmArgs& g, cudaStream_t st);
+                             const uint16_t* c_lo, const GemmArgs& g, int Mplane, cudaStream_t st);
 cudaError_t launch_gemm_tcgen05(const CUtensorMap& tmA_hi, const CUtensorMap& tmA_lo, const CUtensorMap& tmB_hi,
                                 const CUtensorMap& tmB_lo, const GemmArgs& g, int num_sms, cudaStream_t st);
 // screen mode: one fp16 product; tmA = beta^avg fp16 plane, tmB = coefficient fp16 plane
@@ -106,6 +124,13 @@ cudaError_t launch_gemm_screen(const CUtensorMap& tmA, const CUtensorMap& tmB, c
                                int pair_clusters, const GemmArgs& g, int num_sms, cudaStream_t st);
 cudaError_t gemm_screen_pair_clusters(int num_sms, int* clusters);
 cudaError_t gemm_tcgen05_configure();   // sets the dynamic shared memory attribute once
-cudaError_t launch_stage2(const Stage2Args& a, int num_sms, cudaStream_t st);
+cudaError_t launch_stage2(const Stage2Args& a, int num_sms, cudaStream_t st);          // one warp per candidate
+cudaError_t launch_stage2_bybin(const Stage2Args& a, int num_sms, cudaStream_t st);    // regrouped by bin (default)
+int stage2_bybin_smem(int w, int k);
+// front end (fft_r2c.cu): forward real-to-complex FFT of nb series of N = 2^logN samples + whitening
+cudaError_t r2c_configure();
+cudaError_t launch_r2c_table(float2* twF, long long N, cudaStream_t st);
+cudaError_t launch_r2c(const float* x, const float* inv_asd, float2* S, float2* Z, float2* out, const float2* twF,
+                       int logN, int nb, cudaStream_t st);   // shared memory of the by-bin score kernel; 0 = does not fit
 
 }  // namespace rbmf

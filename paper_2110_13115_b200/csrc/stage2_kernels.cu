@@ -1,5 +1,7 @@
 // Kernel 3 (step a6): re-score every first-stage candidate at full time resolution and fp32 accuracy
-// (PAPER.md:180, :191, :230, :246), plus the plain fp32 verification version of kernel 2 (RBMF_DIAG_STAGE1_FP32_CHECK).
+// with one warp per candidate -- the fallback of the by-bin kernel (stage2_bybin.cu)
+// for the (w, k) whose beta block does not fit in shared memory (w = 32 with k > 608), also selectable for tests with
+// RBMF_DIAG_STAGE2_PER_CANDIDATE --, plus the plain fp32 verification version of kernel 2 (RBMF_DIAG_STAGE1_FP32_CHECK).
 #include <cuda_bf16.h>
 
 #include "rbmf_internal.h"
@@ -49,7 +51,8 @@ __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
     for (unsigned long long ci = warp0; ci < n_cand; ci += nwarps) {
         const rbmf_candidate cd = a.cand[ci];
         const float2* __restrict__ crow = a.cs + (size_t)cd.template_id * k;
-        const float2* __restrict__ brow = a.beta + (size_t)cd.bin_index * w * kFftC;
+        const int seg = cd.bin_index / a.Mseg;   // batches: bin = segment * Mseg + i, beta arrays seg_stride apart
+        const float2* __restrict__ brow = a.beta + (size_t)seg * a.seg_stride + (size_t)(cd.bin_index - seg * a.Mseg) * w * kFftC;
         float re0 = 0.f, im0 = 0.f, re1 = 0.f, im1 = 0.f;
         // per_chunk = 2w is a power of two: shifts instead of divisions; four items per lane in flight (the loop is
         // bound by the latency of its two loads, not by their bandwidth)
@@ -160,7 +163,8 @@ __device__ __forceinline__ float plane_val(const uint16_t* hi, const uint16_t* l
 __global__ void __launch_bounds__(256) gemm_simt_kernel(const uint16_t* __restrict__ a_hi,
                                                         const uint16_t* __restrict__ a_lo,
                                                         const uint16_t* __restrict__ c_hi,
-                                                        const uint16_t* __restrict__ c_lo, const GemmArgs g) {
+                                                        const uint16_t* __restrict__ c_lo, const GemmArgs g,
+                                                        const int Mplane) {
     constexpr int TI = 64, TT = 64, KB = 32;
     __shared__ float sA[TI][KB + 1];       // beta^avg rows (time bins) x K
     __shared__ float sRe[TT][KB + 1];      // template "re" rows
@@ -172,7 +176,7 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(const uint16_t* __restri
         for (int e = threadIdx.x; e < TI * KB; e += 256) {
             const int r = e / KB, kk = e % KB;
             const int i = i0 + r;
-            sA[r][kk] = i < g.M ? plane_val(a_hi, a_lo, ((size_t)((k0 + kk) / 64) * g.M + i) * 64 + (k0 + kk) % 64) : 0.f;
+            sA[r][kk] = i < g.M ? plane_val(a_hi, a_lo, ((size_t)((k0 + kk) / 64) * Mplane + i) * 64 + (k0 + kk) % 64) : 0.f;
             const int t = t0 + r;   // t < Tpad always (grid covers padded templates)
             const size_t row_re = (size_t)(t / kGemmTT) * 2 * kGemmTT + (t % kGemmTT);
             sRe[r][kk] = plane_val(c_hi, c_lo, row_re * g.k2 + k0 + kk);
@@ -202,15 +206,16 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(const uint16_t* __restri
                     rbmf_candidate cd;
                     cd.template_id = t; cd.bin_index = i; cd.avg_re = re[u][v]; cd.avg_im = im[u][v];
                     g.cand[idx] = cd;
+                    atomicAdd(g.bin_count + i, 1u);
                 }
             }
         }
 }
 
 cudaError_t launch_gemm_simt(const uint16_t* a_hi, const uint16_t* a_lo, const uint16_t* c_hi, const uint16_t* c_lo,
-                             const GemmArgs& g, cudaStream_t st) {
+                             const GemmArgs& g, int Mplane, cudaStream_t st) {
     dim3 grid((unsigned)(g.num_tb * kGemmTT / 64), (unsigned)((g.M + 63) / 64));
-    gemm_simt_kernel<<<grid, 256, 0, st>>>(a_hi, a_lo, c_hi, c_lo, g);
+    gemm_simt_kernel<<<grid, 256, 0, st>>>(a_hi, a_lo, c_hi, c_lo, g, Mplane);
     return cudaGetLastError();
 }
 

@@ -24,7 +24,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 
 RBMF_OK, RBMF_ERR_ARG, RBMF_ERR_STATE, RBMF_ERR_CUDA, RBMF_ERR_OVERFLOW, RBMF_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 RBMF_GEMM_TCGEN05, RBMF_GEMM_SCREEN = 0, 2
-RBMF_DIAG_STAGE1_FP32_CHECK, RBMF_DIAG_SINGLE_CTA_SCREEN = 1, 2
+RBMF_DIAG_STAGE1_FP32_CHECK, RBMF_DIAG_SINGLE_CTA_SCREEN, RBMF_DIAG_STAGE2_PER_CANDIDATE = 1, 2, 3
 
 TRIGGER_DTYPE = np.dtype([("template", np.int32), ("time", np.int32), ("re", np.float32), ("im", np.float32)])
 CANDIDATE_DTYPE = np.dtype([("template", np.int32), ("bin", np.int32), ("re", np.float32), ("im", np.float32)])
@@ -36,6 +36,7 @@ SIGNATURES = {
     "rbmf_plan_create": (_i32, [ctypes.POINTER(_vp), _i64, _f64, _f64, _i32, _i32]),
     "rbmf_plan_set_window": (_i32, [_vp, _i32]),
     "rbmf_plan_set_capacity": (_i32, [_vp, _i64, _i64]),
+    "rbmf_plan_set_batch": (_i32, [_vp, _i32]),
     "rbmf_plan_set_gemm_impl": (_i32, [_vp, _i32]),
     "rbmf_workspace_bytes": (_i32, [_vp, _psz]),
     "rbmf_plan_set_workspace": (_i32, [_vp, _vp, ctypes.c_size_t]),
@@ -43,7 +44,10 @@ SIGNATURES = {
     "rbmf_set_basis": (_i32, [_vp, _vp]),
     "rbmf_set_coeffs": (_i32, [_vp, _vp, _vp]),
     "rbmf_filter": (_i32, [_vp, _vp, _f32, _f32, _vp, _vp]),
+    "rbmf_prepare_strain": (_i32, [_vp, _vp, _vp, _i32, _vp]),
+    "rbmf_filter_batch": (_i32, [_vp, _vp, _i32, _f32, _f32, _vp, _vp]),
     "rbmf_filter_host": (_i32, [_vp, _vp, _f32, _f32, _vp, _i64, _pi64]),
+    "rbmf_filter_batch_host": (_i32, [_vp, _vp, _i32, _f32, _f32, _vp, _i64, _pi64]),
     "rbmf_get_counts": (_i32, [_vp, _pi64, _pi64]),
     "rbmf_get_screened_count": (_i32, [_vp, _pi64]),
     "rbmf_get_candidates": (_i32, [_vp, _vp, _i64, _pi64]),
@@ -87,11 +91,12 @@ class Plan:
     works whether or not the caller has made `s` torch's current stream."""
 
     def __init__(self, N, fs, f_low, k, T, w=8, max_candidates=1 << 22, max_triggers=1 << 22, device="cuda:0",
-                 stream=None):
+                 stream=None, max_batch=1):
         import torch
         self._torch = torch
         self.N, self.fs, self.f_low, self.k, self.T, self.w = int(N), float(fs), float(f_low), int(k), int(T), int(w)
         self.max_candidates, self.max_triggers = int(max_candidates), int(max_triggers)
+        self.max_batch = int(max_batch)
         self.device = torch.device(device)
         self._h = _vp()
         self.stream = None
@@ -101,6 +106,7 @@ class Plan:
         self._check(_lib.rbmf_plan_set_window(self._h, self.w), "rbmf_plan_set_window")
         self._check(_lib.rbmf_plan_set_capacity(self._h, self.max_candidates, self.max_triggers),
                     "rbmf_plan_set_capacity")
+        self._check(_lib.rbmf_plan_set_batch(self._h, self.max_batch), "rbmf_plan_set_batch")
         nbytes = ctypes.c_size_t()
         self._check(_lib.rbmf_workspace_bytes(self._h, ctypes.byref(nbytes)), "rbmf_workspace_bytes")
         self.workspace_bytes = nbytes.value
@@ -201,6 +207,52 @@ class Plan:
             self._check(_lib.rbmf_filter(self._h, _ptr(strain_dev), float(thr1), float(thr2), _ptr(self._out),
                                          _ptr(self._n_out)), "rbmf_filter")
 
+    def prepare_strain(self, x_dev, inv_asd_dev=None):
+        """rbmf_prepare_strain: (n_segments, N) float32 CUDA time series [+ (N/2+1,) float32 whitening array] ->
+        (n_segments, N/2+1) complex64 CUDA tensor, the input of filter_batch_async."""
+        torch = self._torch
+        if x_dev.dtype != torch.float32 or x_dev.dim() != 2 or x_dev.shape[1] != self.N or not x_dev.is_cuda \
+                or not x_dev.is_contiguous():
+            raise ValueError("x must be a contiguous float32 CUDA tensor of shape (n_segments, N)")
+        if inv_asd_dev is not None and (inv_asd_dev.dtype != torch.float32 or inv_asd_dev.numel() != self.N // 2 + 1
+                                        or not inv_asd_dev.is_cuda or not inv_asd_dev.is_contiguous()):
+            raise ValueError("inv_asd must be a contiguous float32 CUDA tensor with N/2+1 entries")
+        self._order_after_current()
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            out = torch.empty((x_dev.shape[0], self.N // 2 + 1), dtype=torch.complex64, device=self.device)
+            self._check(_lib.rbmf_prepare_strain(self._h, _ptr(x_dev), _ptr(inv_asd_dev), int(x_dev.shape[0]),
+                                                 _ptr(out)), "rbmf_prepare_strain")
+        return out
+
+    def filter_batch_async(self, strain_dev, thr1, thr2):
+        """Enqueue rbmf_filter_batch; strain_dev is a complex64 CUDA tensor of shape (n_segments, N/2+1)."""
+        torch = self._torch
+        if (strain_dev.dtype != torch.complex64 or strain_dev.dim() != 2 or strain_dev.shape[1] != self.N // 2 + 1
+                or not strain_dev.is_cuda or not strain_dev.is_contiguous()):
+            raise ValueError("strain must be a contiguous complex64 CUDA tensor of shape (n_segments, N/2+1)")
+        self._order_after_current()
+        with torch.cuda.device(self.device):
+            self._check(_lib.rbmf_filter_batch(self._h, _ptr(strain_dev), int(strain_dev.shape[0]), float(thr1),
+                                               float(thr2), _ptr(self._out), _ptr(self._n_out)), "rbmf_filter_batch")
+
+    def filter_batch(self, strains, thr1, thr2, allow_overflow=False):
+        """Filter a batch; returns the triggers sorted by (template, time) with time = segment * N + n."""
+        s = self._dev(strains, self._torch.complex64)
+        self.filter_batch_async(s, thr1, thr2)
+        return self.triggers(allow_overflow)
+
+    def filter_batch_host(self, strains_host, thr1, thr2, out_host=None):
+        """rbmf_filter_batch_host: host strains (n_segments, N/2+1) in, host triggers out (unsorted)."""
+        torch = self._torch
+        if out_host is None:
+            out_host = np.empty(self.max_triggers, dtype=TRIGGER_DTYPE)
+        n = _i64()
+        with torch.cuda.device(self.device):
+            st = _lib.rbmf_filter_batch_host(self._h, _ptr(strains_host), int(strains_host.shape[0]), float(thr1),
+                                             float(thr2), _ptr(out_host), len(out_host), ctypes.byref(n))
+        self._check(st, "rbmf_filter_batch_host", allow=(RBMF_ERR_OVERFLOW,))
+        return out_host[: min(n.value, len(out_host))], n.value
+
     def counts(self, allow_overflow=False):
         nc, nt = _i64(), _i64()
         st = self._check(_lib.rbmf_get_counts(self._h, ctypes.byref(nc), ctypes.byref(nt)), "rbmf_get_counts",
@@ -265,9 +317,9 @@ class Plan:
                     allow=(RBMF_ERR_OVERFLOW,))
         return np.sort(out[:n], order=("template", "bin"))
 
-    def internal(self, which):
+    def internal(self, which, segment=0):
         """Copy of an internal array: 'beta' -> (N, k) complex64; 'beta_avg' -> (N/w, k) complex64 (bf16 hi + lo, or
-        the single fp16 plane in RBMF_GEMM_SCREEN mode)."""
+        the single fp16 plane in RBMF_GEMM_SCREEN mode), of segment `segment` of the last batch."""
         torch = self._torch
         self.stream.synchronize()
 
@@ -289,18 +341,19 @@ class Plan:
                 return view(4 if which == "bin_norm" else 5).view(torch.float32).cpu().numpy()
         if which == "beta":
             with torch.cuda.stream(self.stream):
-                v = view(0).view(torch.float32).view(self.k // C, self.N, C, 2)          # [chunk][n][C]
+                v = view(0).view(torch.float32).view(self.max_batch, self.k // C, self.N, C, 2)[segment]   # [chunk][n][C]
                 return torch.view_as_complex(
                     v.permute(1, 0, 2, 3).reshape(self.N, self.k, 2).contiguous()).cpu().numpy()
         if which == "beta_avg":
-            M, nkb = self.N // self.w, (self.k + 31) // 32
+            M, nkb, Mp = self.N // self.w, (self.k + 31) // 32, self.max_batch * (self.N // self.w)
             if screen:                                   # one fp16 plane
                 hi = view(1).view(torch.float16).to(torch.float32)
                 lo = torch.zeros_like(hi)
             else:
                 hi = view(1).view(torch.bfloat16).to(torch.float32)
                 lo = view(2).view(torch.bfloat16).to(torch.float32)
-            v = (hi + lo).view(nkb, M, 32, 2).permute(1, 0, 2, 3).reshape(M, nkb * 32, 2)[:, : self.k]   # [kb][bin][32]
+            v = (hi + lo).view(nkb, Mp, 32, 2)[:, segment * M:(segment + 1) * M]                        # [kb][bin][32]
+            v = v.permute(1, 0, 2, 3).reshape(M, nkb * 32, 2)[:, : self.k]
             return torch.view_as_complex(v.contiguous()).cpu().numpy()
         raise KeyError(which)
 

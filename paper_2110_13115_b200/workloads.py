@@ -260,3 +260,17 @@ def bank_templates(wl: dict, idx, device: Optional[str] = None) -> np.ndarray:
     cfg = wl["config"]
     idx = np.atleast_1d(np.asarray(idx))
     return _spa_templates(wl["mc"][idx], cfg, device or "cpu").cpu().numpy()
+
+
+def make_time_series(wl: dict, segment: int = 0) -> tuple:
+    """Time-domain input for the step in front of the path: a COLOURED real series whose
+    whitened spectrum is the strain of `make_strain(wl, segment)`, and the whitening array that undoes the colouring.
+    asd(f) = sqrt(1 + (f0/max(f, f_low))^4 + (f/f1)^2) with f0 = 2 f_low, f1 = fs/4 (a smooth seismic-wall + shot-noise
+    shape, flat below the band so that float32 keeps the in-band content; a stand-in for the aLIGO PSD);
+    x = irfft(strain * asd).  Returns (x float32 (N,), inv_asd float32 (N/2+1,))."""
+    cfg = wl["config"]
+    d, _ = make_strain(wl, segment)
+    f = np.arange(cfg.bins, dtype=np.float64) * (cfg.fs / cfg.N)
+    asd = np.sqrt(1.0 + (2.0 * cfg.f_low / np.maximum(f, cfg.f_low)) ** 4 + (f / (cfg.fs / 4.0)) ** 2)
+    x = np.fft.irfft(d.astype(np.complex128) * asd, n=cfg.N)
+    return x.astype(np.float32), (1.0 / asd).astype(np.float32)

@@ -83,17 +83,26 @@ def test_window_capacity_and_workspace_size(binding):
     assert b.rbmf_workspace_bytes(h, ctypes.byref(nbytes)) == b.RBMF_OK
     assert nbytes.value < default_bytes          # smaller lists
     n = ctypes.c_int32()
-    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 5   # screen mode (default)
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 7   # screen mode (default): prep, FFT, bin norms, GEMM, stage 2 = alloc + scatter + score
     assert b.rbmf_plan_set_window(h, 1) == b.RBMF_OK
-    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 5
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 7
     assert b.rbmf_plan_set_gemm_impl(h, 7) == b.RBMF_ERR_ARG
     assert b.rbmf_plan_set_gemm_impl(h, 1) == b.RBMF_ERR_ARG     # the fp32 check kernel is not a product mode
     assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_TCGEN05) == b.RBMF_OK
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 6
+    assert b.rbmf_diag_set(h, b.RBMF_DIAG_STAGE2_PER_CANDIDATE, 1) == b.RBMF_OK
     assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 4
+    assert b.rbmf_diag_set(h, b.RBMF_DIAG_STAGE2_PER_CANDIDATE, 0) == b.RBMF_OK
+    assert b.rbmf_plan_set_batch(h, 0) == b.RBMF_ERR_ARG
+    assert b.rbmf_plan_set_batch(h, 1 << 20) == b.RBMF_ERR_ARG     # batch * N must fit a 31-bit sample index
+    before = ctypes.c_size_t()
+    assert b.rbmf_workspace_bytes(h, ctypes.byref(before)) == b.RBMF_OK
+    assert b.rbmf_plan_set_batch(h, 4) == b.RBMF_OK
+    assert b.rbmf_workspace_bytes(h, ctypes.byref(nbytes)) == b.RBMF_OK and nbytes.value > before.value
     assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_SCREEN) == b.RBMF_OK
     assert b.rbmf_diag_set(h, 99, 1) == b.RBMF_ERR_ARG
     assert b.rbmf_diag_set(h, b.RBMF_DIAG_STAGE1_FP32_CHECK, 1) == b.RBMF_OK
-    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 4
+    assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 6
     assert b.rbmf_diag_set(h, b.RBMF_DIAG_STAGE1_FP32_CHECK, 0) == b.RBMF_OK
     assert b.rbmf_get_screened_count(h, ctypes.byref(ctypes.c_int64())) == b.RBMF_ERR_STATE
     b.rbmf_plan_destroy(h)

@@ -1,0 +1,272 @@
+"""Batched segments and the by-bin stage 2 against the fp64 oracle, plus guard-zone
+and repeatability checks that stand in for compute-sanitizer (closed on this pool, profiles/r02_sanitizer.md)."""
+import numpy as np
+import pytest
+
+from oracle import compare
+from oracle import rbmf_oracle as orc
+from paper_2110_13115_b200 import workloads as wlm
+
+pytestmark = pytest.mark.gpu
+
+X3, SCREEN = 0, 2
+
+
+@pytest.fixture(scope="module")
+def rbmf(built_library):
+    from paper_2110_13115_b200 import rbmf as mod
+    return mod
+
+
+_WL = {}
+
+
+def workload(name, **kw):
+    key = (name, tuple(sorted(kw.items())))
+    if key not in _WL:
+        cfg = wlm.CONFIGS[name]
+        if kw:
+            cfg = cfg.replace(**kw)
+        _WL[key] = wlm.make_workload(cfg, device="cuda")
+    return _WL[key]
+
+
+def strains_of(wl, n):
+    return np.stack([wlm.make_strain(wl, s)[0] for s in range(n)])
+
+
+def make_plan(rbmf, wl, w=None, impl=SCREEN, max_batch=1, cap=1 << 20):
+    import torch
+    cfg = wl["config"]
+    plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w if w is None else w, max_candidates=cap,
+                     max_triggers=cap, max_batch=max_batch)
+    plan.set_gemm_impl(impl)
+    plan.set_basis(torch.from_numpy(wl["basis"]))
+    plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+    return plan
+
+
+def batch_oracle(wl, strains, w, thr1, thr2):
+    cfg = wl["config"]
+    return orc.oracle_filter_batch(strains, wl["basis"], wl["coeffs"], wl["sigma"], cfg.N, cfg.fs, cfg.f_low, w,
+                                   thr1, thr2)
+
+
+@pytest.mark.parametrize("impl", [SCREEN, X3])
+@pytest.mark.parametrize("name,nb,max_batch,w,thr", [("tiny", 3, 3, 4, (3.0, 4.0)), ("mini", 3, 4, 8, (3.0, 4.0)),
+                                                      ("mini", 2, 2, 1, (4.0, 4.5)), ("mini", 5, 5, 32, (0.5, 3.5))])
+def test_batch_against_oracle(rbmf, name, nb, max_batch, w, thr, impl):
+    import torch
+    wl = workload(name)
+    cfg = wl["config"]
+    strains = strains_of(wl, nb)
+    plan = make_plan(rbmf, wl, w=w, impl=impl, max_batch=max_batch)
+    got = plan.filter_batch(torch.from_numpy(strains), *thr)
+    cand = plan.candidates()
+    ref = batch_oracle(wl, strains, w, *thr)
+    rep = compare.compare_triggers(got, ref, nb * cfg.N, *thr)
+    crep = compare.compare_candidates(cand, ref, nb * cfg.N // w, thr[0])
+    assert rep["ok"] and rep["n_mandatory"] > 0, rep
+    assert crep["ok"], crep
+    assert len(np.unique(got["time"] // cfg.N)) >= min(nb, 2)   # more than one segment produced triggers
+    # beta / beta^avg of the last segment against the oracle's series of that strain alone
+    beta = plan.internal("beta", segment=nb - 1)
+    ref_beta = orc.basis_series(strains[nb - 1], wl["basis"], cfg.N, cfg.j_low).T
+    assert np.abs(beta - ref_beta).max() <= 1e-5
+    # a single-segment call on the same plan afterwards reproduces segment 0 of the batch
+    one = plan.filter(torch.from_numpy(strains[0]), *thr)
+    seg0 = got[got["time"] < cfg.N]
+    assert np.array_equal(np.sort(one, order=("template", "time"))[["template", "time"]], seg0[["template", "time"]])
+    plan.close()
+
+
+def test_batch_small_config_two_segments(rbmf):
+    import torch
+    wl = workload("small")
+    cfg = wl["config"]
+    strains = strains_of(wl, 2)
+    plan = make_plan(rbmf, wl, max_batch=2)
+    got = plan.filter_batch(torch.from_numpy(strains), cfg.thr1, cfg.thr2)
+    ref = batch_oracle(wl, strains, cfg.w, cfg.thr1, cfg.thr2)
+    rep = compare.compare_triggers(got, ref, 2 * cfg.N, cfg.thr1, cfg.thr2)
+    crep = compare.compare_candidates(plan.candidates(), ref, 2 * cfg.N // cfg.w, cfg.thr1)
+    host, n_host = plan.filter_batch_host(strains, cfg.thr1, cfg.thr2)
+    plan.close()
+    assert rep["ok"] and rep["n_mandatory"] > 100, rep
+    assert crep["ok"], crep
+    assert n_host == len(got)
+    assert np.array_equal(np.sort(host, order=("template", "time")), got)
+
+
+@pytest.mark.parametrize("w", [1, 2, 4, 8, 16, 32])
+def test_stage2_by_bin_and_per_candidate_kernels_agree(rbmf, w):
+    """Both stage-2 kernels pass the oracle comparison on the same call and report the same sets."""
+    import torch
+    wl = workload("mini")
+    cfg = wl["config"]
+    thr = ({16: 1.5, 32: 0.5}.get(w, 2.5), 3.5)     # wide windows attenuate the averaged SNR
+    ref = orc.oracle_filter(wl["strain"], wl["basis"], wl["coeffs"], wl["sigma"], cfg.N, cfg.fs, cfg.f_low, w, *thr)
+    res = []
+    for per_cand in (0, 1):
+        plan = make_plan(rbmf, wl, w=w)
+        plan.diag_set(rbmf.RBMF_DIAG_STAGE2_PER_CANDIDATE, per_cand)
+        got = plan.filter(torch.from_numpy(wl["strain"]), *thr)
+        rep = compare.compare_triggers(got, ref, cfg.N, *thr)
+        crep = compare.compare_candidates(plan.candidates(), ref, cfg.N // w, thr[0])
+        assert rep["ok"] and rep["n_mandatory"] > 500, rep
+        assert crep["ok"], crep
+        res.append(got)
+        plan.close()
+    a, b = res
+    ka, kb = a["template"].astype(np.int64) * cfg.N + a["time"], b["template"].astype(np.int64) * cfg.N + b["time"]
+    assert len(np.setxor1d(ka, kb)) <= max(2, rep["tie_band"])      # they may differ only inside the tie band
+    common = np.intersect1d(ka, kb, return_indices=True)
+    assert np.abs(a["re"][common[1]] - b["re"][common[2]]).max() < 1e-5
+
+
+def test_dense_bin_with_more_candidates_than_one_work_item(rbmf):
+    """thr1 so low that every (template, bin) is a candidate: bins hold T = 300 > 128 candidates (several work items
+    per bin, a ragged last one), and the list is exactly T * N/w long."""
+    import torch
+    wl = workload("mini")
+    cfg = wl["config"]
+    w, thr = 32, (1e-6, 4.0)
+    plan = make_plan(rbmf, wl, w=w, cap=1 << 19)
+    got = plan.filter(torch.from_numpy(wl["strain"]), *thr)
+    nc, nt, _ = plan.counts()
+    assert nc == cfg.T * (cfg.N // w)
+    ref = orc.oracle_filter(wl["strain"], wl["basis"], wl["coeffs"], wl["sigma"], cfg.N, cfg.fs, cfg.f_low, w, *thr)
+    rep = compare.compare_triggers(got, ref, cfg.N, *thr)
+    plan.close()
+    assert rep["ok"] and rep["n_got"] == nt and rep["n_mandatory"] > 50, rep
+
+
+# ------------------------------------------------------------------------------------- guard zones, repeatability
+GUARD = 1 << 20
+
+
+def _guarded_plan(rbmf, wl, **kw):
+    """A Plan whose workspace, trigger array and count sit between guard zones of a known pattern."""
+    import ctypes
+    import torch
+    cfg = wl["config"]
+    plan = make_plan(rbmf, wl, **kw)
+    torch.cuda.synchronize()
+    nbytes = plan.workspace_bytes
+    big = torch.full((nbytes + 2 * GUARD + 2048,), 0xA5, dtype=torch.uint8, device="cuda")
+    base = (big.data_ptr() + GUARD + 1023) // 1024 * 1024
+    off = base - big.data_ptr()
+    # re-point the plan at the guarded block (invalidates basis / coefficients: set them again)
+    st = rbmf.rbmf_plan_set_workspace(plan._h, ctypes.c_void_p(base), nbytes)
+    assert st == rbmf.RBMF_OK
+    plan._ws = big
+    plan.set_basis(torch.from_numpy(wl["basis"]))
+    plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+    out = torch.full((plan.max_triggers * 4 + 2 * GUARD // 4,), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+    plan._out = out[GUARD // 4: GUARD // 4 + plan.max_triggers * 4]
+    plan._out_guarded = out
+    cnt = torch.full((1 + 2 * 1024,), 0x0123456789ABCDEF, dtype=torch.int64, device="cuda")
+    plan._n_out = cnt[1024:1025]
+    plan._cnt_guarded = cnt
+    return plan, big, off, nbytes
+
+
+def _guards_intact(plan, big, off, nbytes):
+    import torch
+    torch.cuda.synchronize()
+    assert bool((big[:off] == 0xA5).all()) and bool((big[off + nbytes:] == 0xA5).all()), "workspace guard overwritten"
+    out = plan._out_guarded
+    assert bool((out[: GUARD // 4] == 0x5A5A5A5A).all()) and bool((out[GUARD // 4 + plan.max_triggers * 4:] == 0x5A5A5A5A).all())
+    cnt = plan._cnt_guarded
+    assert bool((cnt[:1024] == 0x0123456789ABCDEF).all()) and bool((cnt[1025:] == 0x0123456789ABCDEF).all())
+
+
+@pytest.mark.parametrize("name,w,impl,nb,thr,cap", [
+    ("tiny", 4, SCREEN, 1, (3.0, 4.0), 1 << 16), ("tiny", 4, X3, 1, (3.0, 4.0), 1 << 16),
+    ("mini", 8, SCREEN, 3, (3.0, 4.0), 1 << 18), ("mini", 1, X3, 2, (4.0, 4.5), 1 << 18),
+    ("mini", 32, SCREEN, 1, (0.5, 3.5), 1 << 18),
+    ("mini", 8, SCREEN, 2, (1.0, 2.0), 1000),          # both lists overflow: writes must stop at the capacity
+])
+def test_guard_zones_stay_intact(rbmf, name, w, impl, nb, thr, cap):
+    import torch
+    wl = workload(name)
+    plan, big, off, nbytes = _guarded_plan(rbmf, wl, w=w, impl=impl, max_batch=nb, cap=cap)
+    strains = torch.from_numpy(strains_of(wl, nb)).cuda()
+    for single_cta in (0, 1):
+        plan.diag_set(rbmf.RBMF_DIAG_SINGLE_CTA_SCREEN, single_cta)
+        for per_cand in (0, 1):
+            plan.diag_set(rbmf.RBMF_DIAG_STAGE2_PER_CANDIDATE, per_cand)
+            plan.filter_batch_async(strains, *thr)
+            nc, nt, st = plan.counts(allow_overflow=True)
+            assert nt > 0 and (st == rbmf.RBMF_ERR_OVERFLOW) == (cap == 1000)
+            _guards_intact(plan, big, off, nbytes)
+    plan.close()
+
+
+def test_guarded_calls_repeat_bit_exact(rbmf):
+    """20 calls: identical beta bytes and identical sorted lists every time (a race between the FFT's producer, its
+    consumer groups and the TMA stores, or in the GEMM's multicast pipeline, would show as run-to-run differences)."""
+    import torch
+    wl = workload("mini")
+    plan, big, off, nbytes = _guarded_plan(rbmf, wl, w=8, max_batch=2, cap=1 << 18)
+    strains = torch.from_numpy(strains_of(wl, 2)).cuda()
+    first = None
+    for _ in range(20):
+        plan.filter_batch_async(strains, 3.0, 4.0)
+        trig = plan.triggers()
+        cand = plan.candidates()
+        beta = plan.internal("beta", segment=1)
+        cur = (trig.tobytes(), cand.tobytes(), beta.tobytes())
+        if first is None:
+            first = cur
+            assert len(trig) > 100
+        assert cur == first
+    _guards_intact(plan, big, off, nbytes)
+    plan.close()
+
+
+# ------------------------------------------------------------------------------------- the step before the path
+@pytest.mark.parametrize("N", [1024, 2048, 16384, 131072, 1 << 20])
+def test_prepare_strain_against_oracle(rbmf, N):
+    """rbmf_prepare_strain vs the oracle's fp64 forward DFT + whitening, all lengths' splits
+    (odd and even log2 N), two segments, with and without a whitening array.  Bar: fp32 radix-2 FFT with exact
+    twiddles, error <= 4e-6 of the output rms sqrt(N) per bin (log2 N <= 20 stages of 2^-24 relative rounding)."""
+    import torch
+    rng = np.random.default_rng(N)
+    x = rng.standard_normal((2, N)).astype(np.float32)
+    x[1] += (3.0 * np.cos(2 * np.pi * 37 * np.arange(N) / N + 0.4)).astype(np.float32)
+    inv_asd = rng.uniform(0.5, 2.0, N // 2 + 1).astype(np.float32)
+    plan = rbmf.Plan(N, 1024.0, 30.0, 16, 8, w=1, max_candidates=1024, max_triggers=1024, max_batch=2)
+    for wht in (None, inv_asd):
+        got = plan.prepare_strain(torch.from_numpy(x).cuda(), None if wht is None else torch.from_numpy(wht).cuda())
+        plan.stream.synchronize()
+        ref = orc.strain_from_time_series(x, wht)
+        err = np.abs(got.cpu().numpy() - ref)
+        # per bin: relative to that bin's own magnitude (the cosine's line is 1.5 N high) plus the noise floor's rms
+        bar = 1e-6 * np.abs(ref) + 4e-6 * np.sqrt(N) * (2.0 if wht is not None else 1.0)
+        assert (err <= bar).all(), (N, float((err / bar).max()))
+    one = plan.prepare_strain(torch.from_numpy(x[1:2]).cuda(), torch.from_numpy(inv_asd).cuda())
+    assert np.array_equal(one.cpu().numpy()[0], got.cpu().numpy()[1])
+    plan.close()
+
+
+def test_time_series_to_triggers(rbmf):
+    """Front end + path: coloured time series -> rbmf_prepare_strain -> rbmf_filter_batch, against the oracle fed
+    with its own fp64 transform of the same float32 series."""
+    import torch
+    wl = workload("mini")
+    cfg = wl["config"]
+    nb, thr = 3, (3.0, 4.0)
+    xs, inv_asd = zip(*[wlm.make_time_series(wl, s) for s in range(nb)])
+    x = np.stack(xs)
+    plan = make_plan(rbmf, wl, max_batch=nb)
+    strain = plan.prepare_strain(torch.from_numpy(x).cuda(), torch.from_numpy(inv_asd[0]).cuda())
+    plan.filter_batch_async(strain, *thr)
+    got = plan.triggers()
+    ref_strain = orc.strain_from_time_series(x, inv_asd[0])
+    # the whitened spectrum is the frequency-domain workload itself, up to the float32 rounding of x
+    assert np.abs(ref_strain[0, cfg.j_low:cfg.N // 2] - wl["strain"][cfg.j_low:cfg.N // 2]).max() < 2e-3
+    ref = batch_oracle(wl, ref_strain.astype(np.complex64), cfg.w, *thr)
+    rep = compare.compare_triggers(got, ref, nb * cfg.N, *thr)
+    plan.close()
+    assert rep["ok"] and rep["n_mandatory"] > 100, rep
