@@ -33,6 +33,9 @@ Pins (tests/test_oracle_pins.py, all `-m "not gpu"`):
   averaging                    Eq. 12 alias-fold route (`averaged_series_eq12`) == binned mean; w=1 => flat
   thresholds / sets            independent pure-Python enumeration on tiny inputs
   cost model                   Eq. 13-14 reproduce the paper's quoted ~6x / ~10x (tests/golden/paper_values.txt)
+  template routes              flat method: pure-Python enumeration of `snr_series_direct` on the BANK templates, and its
+                               count == oracle_filter's n_flat on reconstructed templates; fast first stage: candidates ==
+                               oracle_filter's (Eq. 12 route == binned mean, already pinned) incl. the values
   forward transform, whitening literal O(N^2) sum at small N, a cosine's closed form (N/2 at its bin), Parseval; batches:
                                segment b of `oracle_filter_batch` against the time-domain brute force on strain b alone
 Parity status: every function below is pinned by at least one of these; nothing is "parity unpinned".
@@ -266,6 +269,52 @@ def oracle_filter_batch(strains, basis, coeffs, sigma, N, fs, f_low, w, thr1, th
                 out[key] = np.concatenate([out[key], r[key]])
             out["n_flat"] += r["n_flat"]
     return out
+
+
+# ------------------------------------------------- the paper's template routes
+def template_method_triggers(strain, templates, sigma, N, fs, f_low, thr, chunk=64):
+    """The flat template method (PAPER.md:61-68; cost Eq. 13, :238; the paper's cuFFT baseline, :338): for every
+    template h_t the full SNR series of Eq. 4 by one inverse FFT, and a trigger for every sample with |rho| >= thr.
+    templates: (T, bins) filters h_t; sigma: (T,) or None (=> 1).  Returns a dict shaped like `oracle_filter`'s:
+    'triggers' and 'near' (|rho| >= thr (1 - 2e-3)) with avg_abs = +inf (there is no first stage), 'n_flat'."""
+    j_low, _ = band(N, fs, f_low)
+    templates = np.asarray(templates)
+    T = templates.shape[0]
+    sg = np.ones(T) if sigma is None else np.asarray(sigma, dtype=np.float64)
+    dt = np.dtype([("template", np.int64), ("time", np.int64), ("re", np.float64), ("im", np.float64),
+                   ("avg_abs", np.float64)])
+    parts, near = [], []
+    for a in range(0, T, chunk):
+        rho = snr_series_fft(strain, templates[a:a + chunk], sg[a:a + chunk], N, j_low)
+        mod = np.abs(rho)
+        for lst, level in ((parts, thr), (near, thr * (1.0 - 2e-3))):
+            m, n = np.nonzero(mod >= level)
+            r = np.empty(len(m), dtype=dt)
+            r["template"], r["time"] = a + m, n
+            r["re"], r["im"], r["avg_abs"] = rho[m, n].real, rho[m, n].imag, np.inf
+            lst.append(r)
+    trig = np.concatenate(parts) if parts else np.empty(0, dtype=dt)
+    return {"triggers": trig, "near": np.concatenate(near) if near else np.empty(0, dtype=dt), "n_flat": len(trig)}
+
+
+def first_stage_by_templates(strain, templates, sigma, N, fs, f_low, w, thr1):
+    """The paper's fast first stage by templates: rho_bar_t from the alias-folded spectrum and an
+    inverse FFT of length N/w (`averaged_series_eq12`), thresholded at thr1.  Returns 'candidates' and 'cand_near'
+    (|rho_bar| >= thr1 (1 - 2e-3)) as in `oracle_filter`."""
+    j_low, _ = band(N, fs, f_low)
+    templates = np.asarray(templates)
+    T = templates.shape[0]
+    sg = np.ones(T) if sigma is None else np.asarray(sigma, dtype=np.float64)
+    dt = np.dtype([("template", np.int64), ("bin", np.int64), ("re", np.float64), ("im", np.float64)])
+    cand, near = [], []
+    for t in range(T):
+        rb = averaged_series_eq12(strain, templates[t], sg[t], N, j_low, w)
+        for lst, level in ((cand, thr1), (near, thr1 * (1.0 - 2e-3))):
+            i = np.nonzero(np.abs(rb) >= level)[0]
+            c = np.empty(len(i), dtype=dt)
+            c["template"], c["bin"], c["re"], c["im"] = t, i, rb[i].real, rb[i].imag
+            lst.append(c)
+    return {"candidates": np.concatenate(cand), "cand_near": np.concatenate(near)}
 
 
 def evaluate_points(strain, basis, coeffs, sigma, N, fs, f_low, w, template, times):

@@ -383,3 +383,40 @@ def test_batch_segments_are_independent_and_offset(micro):
     n0 = len(seg0["triggers"])
     assert n0 > 0 and np.array_equal(res["triggers"][:n0], seg0["triggers"]) and (res["triggers"]["time"][:n0] < N).all()
     assert len(res["near"]) >= len(res["triggers"]) and res["n_flat"] >= len(res["triggers"])
+
+
+# ---------------------------------------------------------------- the paper's template routes
+def test_flat_template_method_against_enumeration_and_nflat(micro):
+    cfg = micro["config"]
+    N = cfg.N
+    bank = wlm.bank_templates(micro, np.arange(cfg.T))
+    res = orc.template_method_triggers(micro["strain"], bank, None, N, cfg.fs, cfg.f_low, 2.5, chunk=3)
+    exp = []
+    for t in range(cfg.T):
+        rho = orc.snr_series_direct(micro["strain"], bank[t], 1.0, N, cfg.j_low)
+        exp += [(t, n) for n in range(N) if abs(rho[n]) >= 2.5]
+    got = sorted((int(a), int(b)) for a, b in zip(res["triggers"]["template"], res["triggers"]["time"]))
+    assert len(exp) > 10 and got == exp and len(res["near"]) >= len(exp)
+    # with the reconstructed templates and their sigma it is oracle_filter's flat set
+    hp = orc.reconstructed_templates(micro["coeffs"], micro["basis"])
+    res2 = orc.template_method_triggers(micro["strain"], hp, micro["sigma"], N, cfg.fs, cfg.f_low, cfg.thr2)
+    ref = orc.oracle_filter(micro["strain"], micro["basis"], micro["coeffs"], micro["sigma"], N, cfg.fs, cfg.f_low,
+                            1, cfg.thr2, cfg.thr2)
+    assert res2["n_flat"] == ref["n_flat"] == len(ref["triggers"]) > 0
+    assert np.array_equal(np.sort(res2["triggers"], order=("template", "time"))["time"], ref["triggers"]["time"])
+
+
+@pytest.mark.parametrize("w", [2, 4, 8])
+def test_fast_first_stage_by_templates_gives_the_same_candidates(micro, w):
+    """either route may produce the first stage; with h_t = sum_k c_tk b_k they coincide."""
+    cfg = micro["config"]
+    hp = orc.reconstructed_templates(micro["coeffs"], micro["basis"])
+    thr1 = {2: 1.5, 4: 1.5, 8: 0.5}[w]           # w = 8 averages a 256-sample segment's SNR away
+    res = orc.first_stage_by_templates(micro["strain"], hp, micro["sigma"], cfg.N, cfg.fs, cfg.f_low, w, thr1)
+    ref = orc.oracle_filter(micro["strain"], micro["basis"], micro["coeffs"], micro["sigma"], cfg.N, cfg.fs, cfg.f_low,
+                            w, thr1, 2.5)
+    assert len(ref["candidates"]) > 5
+    for key in ("candidates", "cand_near"):
+        a, b = np.sort(res[key], order=("template", "bin")), ref[key]
+        assert np.array_equal(a["template"], b["template"]) and np.array_equal(a["bin"], b["bin"])
+        assert np.abs(a["re"] - b["re"]).max() < 1e-12 and np.abs(a["im"] - b["im"]).max() < 1e-12
