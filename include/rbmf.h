@@ -162,6 +162,29 @@ rbmf_status rbmf_filter_batch_host(rbmf_plan* plan, const void* strain_host, int
                                    float thr_stage2, rbmf_trigger* out_host, int64_t capacity_out,
                                    int64_t* n_out_host);
 
+/* ---- The paper's template routes, as on-GPU comparators of the basis route ------
+ * rbmf_plan_enable_template_routes(plan, slab): reserve workspace for them; slab = templates transformed per pass
+ * (multiple of 4, <= 1024; 0 disables).  Before rbmf_workspace_bytes / rbmf_plan_set_workspace and after
+ * rbmf_plan_set_window; needs w >= 2 and 2 N / w >= 1024 (RBMF_ERR_UNSUPPORTED otherwise).
+ * rbmf_set_templates(plan, templates_dev, sigma_dev): templates_dev = T x (N/2+1) complex64, row-major, the filters
+ * h_t[j] themselves (bank templates, or reconstructed ones sum_k c_tk b_k); values outside the band are ignored.  The
+ * POINTER IS RETAINED (42 GB at T = 20000, N = 2^19: too large to copy): the array must stay valid and unchanged while
+ * the template routes are used.  sigma_dev: T float32 norms (copied), or NULL => sigma_t = 1.
+ * rbmf_filter_flat: the flat template method (PAPER.md:61-68; Eq. 13; the paper's cuFFT baseline, :338): one
+ * full-length inverse FFT per template, rho_t[n] = (s / sigma_t) sum_j d[j] conj(h_t[j]) exp(2 pi i j n / N), and a
+ * trigger for EVERY sample with |rho_t[n]| >= thr.  Needs no basis and no coefficients.  Outputs as in rbmf_filter.
+ * rbmf_plan_set_stage1_route(plan, RBMF_STAGE1_TEMPLATES): rbmf_filter takes its first-stage candidates from the
+ * paper's fast first stage by templates (Eq. 10-12: alias-folded spectrum + an inverse FFT of length N / w per
+ * template) instead of the GEMM on the basis series; the second stage is unchanged (it re-scores from beta, so basis
+ * and coefficients are still needed).  With h_t = sum_k c_tk b_k both routes define the same candidates (linearity,
+ * PAPER.md:191, :218).  Single segments only (rbmf_filter_batch with n_segments > 1: RBMF_ERR_UNSUPPORTED). */
+typedef enum { RBMF_STAGE1_BASIS = 0, RBMF_STAGE1_TEMPLATES = 1 } rbmf_stage1_route;
+rbmf_status rbmf_plan_enable_template_routes(rbmf_plan* plan, int32_t slab);
+rbmf_status rbmf_set_templates(rbmf_plan* plan, const void* templates_dev, const float* sigma_dev);
+rbmf_status rbmf_plan_set_stage1_route(rbmf_plan* plan, int32_t route);
+rbmf_status rbmf_filter_flat(rbmf_plan* plan, const void* strain_dev, float thr, rbmf_trigger* out_dev,
+                             int64_t* n_out_dev);
+
 /* Counts of the last rbmf_filter (synchronises the stream).  RBMF_ERR_OVERFLOW if a capacity was exceeded
  * (in RBMF_GEMM_SCREEN mode the capacity max_candidates applies to the screened superset, see
  * rbmf_get_screened_count, while *n_candidates reports the candidates confirmed at fp32 accuracy). */

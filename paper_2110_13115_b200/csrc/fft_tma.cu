@@ -396,7 +396,9 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, const CUtensorMap* tm
 #pragma unroll
         for (int it = 0; it < NIT; ++it) acc[it] = make_float2(0.f, 0.f);
     }
-    if (w >= SUB) {
+    if (a.no_planes) {
+        // template routes (template_route.cu): the caller reads beta itself; no operand planes for kernel 2
+    } else if (w >= SUB) {
         // all SUB lines of this round fall into one bin per n2; a bin spans `rounds` rounds.  Each thread starts at
         // a different line (rot) so that the 16 lanes of a shared-memory wavefront hit 16 distinct 8-byte banks.
         const int rot = (gt >> (RB * 8 == 64 ? 3 : 2)) & (SUB - 1);

@@ -43,8 +43,9 @@ cudaError_t launch_init_tables(float2* tw1_a, float2* tw1_b, float2* twN, int lo
 // basis: k x bins (row-major, caller's layout)  ->  basisP[chunk][tile][j1 < L1/2][line < sub][C] with
 // j = j1 L2 + j2, j2 = tile * sub + line, zero outside the band: the block a pass-1 tile (sub lines) reads is
 // contiguous and already in the [position][line][column] order of the FFT kernel's tile buffer.
+// Rows >= rows_valid (the padding of the last slab of a template bank, template_route.cu) are written as zeros.
 __global__ void layout_basis_kernel(const float2* __restrict__ basis, float2* __restrict__ basisP, long long bins,
-                                    int j_low, int logL1, int logL2, int sub) {
+                                    int j_low, int logL1, int logL2, int sub, int rows_valid) {
     __shared__ float2 tile[kFftC][32][33];
     const int L2 = 1 << logL2, H = (1 << logL1) / 2;
     const int chunk = blockIdx.z;
@@ -56,7 +57,7 @@ __global__ void layout_basis_kernel(const float2* __restrict__ basis, float2* __
             float2 v = make_float2(0.f, 0.f);
             if (j1 < H && j2 < L2) {
                 const long long j = (long long)j1 * L2 + j2;
-                if (j >= j_low) v = basis[(long long)(chunk * kFftC + c) * bins + j];
+                if (j >= j_low && chunk * kFftC + c < rows_valid) v = basis[(long long)(chunk * kFftC + c) * bins + j];
             }
             tile[c][r][tx] = v;
         }
@@ -75,10 +76,10 @@ __global__ void layout_basis_kernel(const float2* __restrict__ basis, float2* __
 }
 
 cudaError_t launch_layout_basis(const float2* basis, float2* basisP, int k, int64_t bins, int j_low, int logL1,
-                                int logL2, int sub, cudaStream_t st) {
+                                int logL2, int sub, int rows_valid, cudaStream_t st) {
     const int L2 = 1 << logL2, H = (1 << logL1) / 2;
     dim3 grid((unsigned)((L2 + 31) / 32), (unsigned)((H + 31) / 32), (unsigned)(k / kFftC));
-    layout_basis_kernel<<<grid, 256, 0, st>>>(basis, basisP, bins, j_low, logL1, logL2, sub);
+    layout_basis_kernel<<<grid, 256, 0, st>>>(basis, basisP, bins, j_low, logL1, logL2, sub, rows_valid);
     return cudaGetLastError();
 }
 

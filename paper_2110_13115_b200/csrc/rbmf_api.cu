@@ -15,9 +15,18 @@ constexpr size_t kAlign = 1024;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 inline int ilog2(int64_t x) { int l = 0; while ((int64_t(1) << l) < x) ++l; return l; }
 
+// One instance of kernel 1 working on `ncols` columns of length-N series (the template routes run two besides the
+// plan's own: full length for the flat method, length 2 N / w for the fast first stage).
+struct TmUnit {
+    int64_t N;
+    int logN1, logN2, ncols;
+    size_t basisP, beta, tw1_a, tw1_b, twN, dsT, sched;   // workspace offsets
+    CUtensorMap tmY;
+};
+
 struct Layout {
     size_t basisP, beta, bavg_hi, bavg_lo, c_hi, c_lo, c_h16, tnorm_blk, bin_norm, cs, tw1_a, tw1_b, twN, dsT,
-        cand, cand2, cand3, bin_count, bin_start, items, counters, sched, strain_stage, trig_stage, twF, r2c_s, r2c_z, total;
+        cand, cand2, cand3, bin_count, bin_start, items, counters, sched, strain_stage, trig_stage, twF, r2c_s, r2c_z, tm_S, tm_isg, total;
     size_t sched_bytes;
     size_t plane_bytes;
 };
@@ -49,6 +58,11 @@ struct rbmf_plan {
     int last_cuda;
     CUtensorMap tmA_hi, tmA_lo, tmB_hi, tmB_lo, tmB_h16, tmB_h16half, tmY;
     int pair_clusters;   // 2-CTA clusters of the screen GEMM the device holds (0: single-CTA kernel)
+    // template routes (rbmf_plan_enable_template_routes): slab = templates per pass (0 = disabled)
+    int tm_slab, stage1_route;
+    TmUnit tmF, tmS;     // flat method: length N; fast first stage: length 2 N / w
+    const void* tm_templates;   // caller's T x (N/2+1) bank (retained pointer)
+    bool have_templates;
     bool have_maps;
     cudaEvent_t ev[5];
     bool have_events;
@@ -93,6 +107,24 @@ Layout make_layout(const rbmf_plan* p) {
     L.twF = take((size_t)p->n_half * 8);                 // front end: e^{-2 pi i m / N}, m < N/2
     L.r2c_s = take(B * (size_t)p->n_half * 8);
     L.r2c_z = take(B * (size_t)p->n_half * 8);
+    if (p->tm_slab > 0) {
+        L.tm_S = take((size_t)p->n_half * 8);
+        L.tm_isg = take((size_t)p->T * 4);
+        TmUnit* units[2] = {const_cast<TmUnit*>(&p->tmF), const_cast<TmUnit*>(&p->tmS)};
+        for (int u = 0; u < 2; ++u) {
+            TmUnit& U = *units[u];
+            U.N = u == 0 ? p->N : 2 * p->N / p->w;
+            const int n = ilog2(U.N);
+            U.logN1 = (n + 1) / 2; U.logN2 = n / 2; U.ncols = p->tm_slab;
+            U.basisP = take((size_t)(U.N / 2) * U.ncols * 8);
+            U.beta = take((size_t)U.N * U.ncols * 8);
+            U.tw1_a = take(((size_t)1 << U.logN1) * 8);
+            U.tw1_b = take(((size_t)1 << U.logN2) * 8);
+            U.twN = take(((size_t)1 << U.logN2) * (size_t)(fft_r0(U.logN1) + fft_r1(U.logN1)) * 8);
+            U.dsT = take((size_t)(U.N / 2) * 8);
+            U.sched = take(((size_t)kSchedBase + kMaxChunks) * 4);
+        }
+    }
     L.total = off;
     return L;
 }
@@ -159,16 +191,63 @@ rbmf_status make_map_planes(rbmf_plan* plan, CUtensorMap* map, void* base, uint6
 
 // Y rows of a pass-2 FFT tile: the beta array viewed as fp32 [chunk][j2 < L2][2 C L1] (Y[n1][j2] sits at the address
 // of beta[n1 + L1 j2]); box = sub2 lines x C columns (re, im) wide, up to 256 rows j2, unswizzled.
-rbmf_status make_map_y(rbmf_plan* plan, CUtensorMap* map, void* base) {
-    const uint64_t L1 = 1ull << plan->logN1, L2 = 1ull << plan->logN2;
-    const cuuint64_t dims[3] = {2 * kFftC * L1, L2, (cuuint64_t)(plan->k / kFftC) * (cuuint64_t)plan->max_batch};
-    const cuuint64_t strides[2] = {L1 * kFftC * 8, (cuuint64_t)plan->N * kFftC * 8};
-    const cuuint32_t box[3] = {(cuuint32_t)(2 * kFftC * fft_sub(plan->logN2)), (cuuint32_t)(L2 < 256 ? L2 : 256), 1};
+rbmf_status make_map_y(rbmf_plan* plan, CUtensorMap* map, void* base, int logN1, int logN2, uint64_t nblocks) {
+    const uint64_t L1 = 1ull << logN1, L2 = 1ull << logN2;
+    const cuuint64_t dims[3] = {2 * kFftC * L1, L2, (cuuint64_t)nblocks};
+    const cuuint64_t strides[2] = {L1 * kFftC * 8, (cuuint64_t)(L1 * L2) * kFftC * 8};
+    const cuuint32_t box[3] = {(cuuint32_t)(2 * kFftC * fft_sub(logN2)), (cuuint32_t)(L2 < 256 ? L2 : 256), 1};
     return encode_map(plan, map, base, 3, dims, strides, box, CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
                       CU_TENSOR_MAP_SWIZZLE_NONE);
 }
 
 template <typename T> T* at(rbmf_plan* p, size_t off) { return reinterpret_cast<T*>(p->ws + off); }
+
+}  // namespace
+
+// ---- template routes ------------------------------------------------------------------------
+namespace {
+
+// One launch of kernel 1 on a template-route unit: ncols columns, one segment, no operand planes.
+rbmf_status run_tm_unit(rbmf_plan* plan, const TmUnit& U) {
+    cudaStream_t st = plan->stream;
+    CK(cudaMemsetAsync(plan->ws + U.sched, 0, ((size_t)kSchedBase + kMaxChunks) * 4, st));
+    FftArgs a;
+    memset(&a, 0, sizeof(a));
+    a.basisP = at<float2>(plan, U.basisP); a.dsT = at<float2>(plan, U.dsT);
+    a.tw1_a = at<float2>(plan, U.tw1_a); a.tw1_b = at<float2>(plan, U.tw1_b); a.twN = at<float2>(plan, U.twN);
+    a.beta = at<float2>(plan, U.beta);
+    a.sched = at<unsigned>(plan, U.sched);
+    a.N = U.N; a.M = (int)U.N; a.Mseg = (int)U.N; a.nb = 1; a.nchunk = U.ncols / kFftC; a.w = 1; a.inv_w = 1.f;
+    a.no_planes = 1;
+    const long long n1t = (1ll << U.logN2) / fft_sub(U.logN1);
+    long long la = (4ll * plan->fft_grid + n1t - 1) / n1t;
+    const long long cap = (48ll << 20) / ((long long)U.N * kFftC * 8) - 1;
+    if (la > cap) la = cap;
+    if (la < 1) la = 1;
+    a.lookahead = (int)la;
+    CK(launch_fft_tma(U.tmY, a, U.logN1, U.logN2, plan->fft_grid, st));
+    return RBMF_OK;
+}
+
+// Fast first stage by templates (Eq. 10-12): fold -> short transform -> threshold scan, slab by slab; fills the
+// stage-1 list, counters[0] and the per-bin histogram exactly like kernel 2 does.
+rbmf_status stage1_by_templates(rbmf_plan* plan, const float2* strain_dev, float thr1) {
+    const Layout& L = plan->lay;
+    const TmUnit& U = plan->tmS;
+    unsigned long long* counters = at<unsigned long long>(plan, L.counters);
+    const float scale = (float)sqrt(2.0 / (double)plan->N);
+    for (int t0 = 0; t0 < plan->T; t0 += U.ncols) {
+        CK(launch_tm_fold((const float2*)plan->tm_templates, strain_dev, at<float2>(plan, L.tm_S),
+                          at<float2>(plan, U.basisP), plan->N / 2 + 1, plan->j_low, plan->n_half, plan->w, scale, t0,
+                          plan->T, U.ncols, U.logN1, U.logN2, fft_sub(U.logN1), plan->stream));
+        rbmf_status s = run_tm_unit(plan, U);
+        if (s != RBMF_OK) return s;
+        CK(launch_tm_scan(at<float2>(plan, U.beta), U.N, 2, (int)plan->M, at<float>(plan, L.tm_isg), t0, plan->T,
+                          U.ncols, thr1 * thr1, (rbmf_trigger*)at<rbmf_candidate>(plan, L.cand), counters,
+                          (unsigned long long)plan->max_cand, at<unsigned>(plan, L.bin_count), plan->stream));
+    }
+    return RBMF_OK;
+}
 
 }  // namespace
 
@@ -285,7 +364,24 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     rbmf_status s;
     const uint64_t k2 = 2 * (uint64_t)plan->k;
     const uint64_t nkb = (uint64_t)((plan->k + 31) / 32);
-    if ((s = make_map_y(plan, &plan->tmY, plan->ws + L.beta)) != RBMF_OK) return s;
+    if ((s = make_map_y(plan, &plan->tmY, plan->ws + L.beta, plan->logN1, plan->logN2,
+                        (uint64_t)(plan->k / kFftC) * (uint64_t)plan->max_batch)) != RBMF_OK) return s;
+    if (plan->tm_slab > 0) {
+        TmUnit* units[2] = {&plan->tmF, &plan->tmS};
+        for (int u = 0; u < 2; ++u) {
+            TmUnit& U = *units[u];
+            size_t smem = 0;
+            CK(fft_tma_configure(U.logN1, U.logN2, &smem));
+            CK(launch_init_tables(at<float2>(plan, U.tw1_a), at<float2>(plan, U.tw1_b), at<float2>(plan, U.twN),
+                                  U.logN1, U.logN2, plan->stream));
+            if ((s = make_map_y(plan, &U.tmY, plan->ws + U.beta, U.logN1, U.logN2, (uint64_t)(U.ncols / kFftC))) != RBMF_OK)
+                return s;
+        }
+        // S(f) of Eq. 11; the fast first stage feeds its folded spectrum to kernel 1 with a unit "strain"
+        CK(launch_tm_tables(at<float2>(plan, L.tm_S), at<float2>(plan, plan->tmS.dsT), plan->N, plan->w,
+                            plan->tmS.N / 2, plan->stream));
+    }
+    plan->have_templates = false;
     const uint64_t Mplane = (uint64_t)plan->M * (uint64_t)plan->max_batch;
     if ((s = make_map_planes(plan, &plan->tmA_hi, plan->ws + L.bavg_hi, Mplane, nkb)) != RBMF_OK) return s;
     if ((s = make_map_planes(plan, &plan->tmA_lo, plan->ws + L.bavg_lo, Mplane, nkb)) != RBMF_OK) return s;
@@ -308,7 +404,7 @@ rbmf_status rbmf_set_basis(rbmf_plan* plan, const void* basis_dev) {
     if (!plan || !basis_dev) return RBMF_ERR_ARG;
     if (!plan->have_ws) return RBMF_ERR_STATE;
     CK(launch_layout_basis((const float2*)basis_dev, at<float2>(plan, plan->lay.basisP), plan->k, plan->N / 2 + 1,
-                           plan->j_low, plan->logN1, plan->logN2, fft_sub(plan->logN1), plan->stream));
+                           plan->j_low, plan->logN1, plan->logN2, fft_sub(plan->logN1), plan->k, plan->stream));
     plan->have_basis = true;
     return RBMF_OK;
 }
@@ -385,7 +481,9 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
         a.lookahead = (int)la;
     }
     CK(launch_fft_tma(plan->tmY, a, plan->logN1, plan->logN2, plan->fft_grid, st));
-    if (screen)
+    const bool by_templates = plan->stage1_route == RBMF_STAGE1_TEMPLATES;
+    if (by_templates && (nb != 1 || !plan->have_templates)) return nb != 1 ? RBMF_ERR_UNSUPPORTED : RBMF_ERR_STATE;
+    if (screen && !by_templates)
         CK(launch_bin_norm(at<uint16_t>(plan, L.bavg_hi), at<float>(plan, L.bin_norm), (int)Mtot, (int)Mplane,
                            (plan->k + 31) / 32, st));
     if (tm) CK(cudaEventRecord(plan->ev[1], st));
@@ -402,7 +500,11 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     g.num_tb = plan->Tpad / kGemmTT;
     g.num_ib = (int)(Mtot / kGemmBM);
     g.group = 32;   // template blocks per raster group: 32 coefficient tiles (8 MB fp16) stay L2-resident
-    if (screen) {
+    if (by_templates) {
+        // the paper's fast first stage by templates (Eq. 10-12) in the place of the GEMM; exact fp32 candidates
+        rbmf_status s1 = stage1_by_templates(plan, (const float2*)strain_dev, thr_stage1);
+        if (s1 != RBMF_OK) return s1;
+    } else if (screen) {
         // Bound of |R_fp16 - R| for the one-product fp16 screen (derivation: gemm_tcgen05.cu header): operand
         // rounding u = 2^-11 relative (+ eta = 2^-25 sqrt(2) absolute per complex value in the subnormal range), fp32
         // accumulation of the 2k exact products in the tensor core taken as (2k + 64) 2^-22 sqrt(2) relative to
@@ -435,7 +537,8 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     memset(&s2, 0, sizeof(s2));
     s2.cand = g.cand; s2.cs = at<float2>(plan, L.cs); s2.beta = at<float2>(plan, L.beta);
     s2.out = out_dev; s2.counters = counters;
-    s2.confirmed = at<rbmf_candidate>(plan, L.cand2); s2.thr1_sq = g.thr1_sq; s2.screen = screen ? 1 : 0;
+    const bool confirm = screen && !by_templates;   // the list is the fp16 screen's superset: confirm in fp32
+    s2.confirmed = at<rbmf_candidate>(plan, L.cand2); s2.thr1_sq = g.thr1_sq; s2.screen = confirm ? 1 : 0;
     s2.cand_cap = (unsigned long long)plan->max_cand; s2.trig_cap = (unsigned long long)plan->max_trig;
     s2.thr2_sq = thr_stage2 * thr_stage2; s2.k = plan->k; s2.w = plan->w; s2.N = plan->N;
     s2.bin_count = g.bin_count; s2.bin_start = at<unsigned>(plan, L.bin_start); s2.items = at<int4>(plan, L.items);
@@ -448,7 +551,65 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     if (tm) CK(cudaEventRecord(plan->ev[3], st));
     plan->filtered = true;
     plan->last_nb = nb;
-    plan->last_impl = screen ? (int)RBMF_GEMM_SCREEN : (int)RBMF_GEMM_TCGEN05;
+    plan->last_impl = confirm ? (int)RBMF_GEMM_SCREEN : (int)RBMF_GEMM_TCGEN05;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_plan_enable_template_routes(rbmf_plan* plan, int32_t slab) {
+    if (!plan) return RBMF_ERR_ARG;
+    if (plan->have_ws) return RBMF_ERR_STATE;
+    if (slab < 0 || slab > 4 * kMaxChunks || (slab % kFftC) != 0) return RBMF_ERR_ARG;
+    if (slab > 0 && (plan->w < 2 || 2 * plan->N / plan->w < 1024)) return RBMF_ERR_UNSUPPORTED;
+    plan->tm_slab = slab;
+    refresh(plan);
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_plan_set_stage1_route(rbmf_plan* plan, int32_t route) {
+    if (!plan) return RBMF_ERR_ARG;
+    if (route != RBMF_STAGE1_BASIS && route != RBMF_STAGE1_TEMPLATES) return RBMF_ERR_ARG;
+    if (route == RBMF_STAGE1_TEMPLATES && plan->tm_slab == 0) return RBMF_ERR_STATE;
+    plan->stage1_route = route;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_set_templates(rbmf_plan* plan, const void* templates_dev, const float* sigma_dev) {
+    if (!plan || !templates_dev) return RBMF_ERR_ARG;
+    if (!plan->have_ws || plan->tm_slab == 0) return RBMF_ERR_STATE;
+    CK(launch_tm_inv_sigma(sigma_dev, at<float>(plan, plan->lay.tm_isg), plan->T, plan->stream));
+    plan->tm_templates = templates_dev;
+    plan->have_templates = true;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_filter_flat(rbmf_plan* plan, const void* strain_dev, float thr, rbmf_trigger* out_dev,
+                             int64_t* n_out_dev) {
+    if (!plan || !strain_dev || !out_dev || !n_out_dev || !(thr > 0.f)) return RBMF_ERR_ARG;
+    if (!plan->have_ws || plan->tm_slab == 0 || !plan->have_templates) return RBMF_ERR_STATE;
+    const Layout& L = plan->lay;
+    const TmUnit& U = plan->tmF;
+    cudaStream_t st = plan->stream;
+    unsigned long long* counters = at<unsigned long long>(plan, L.counters);
+    const bool tm = plan->timing != 0;
+    if (tm) CK(cudaEventRecord(plan->ev[0], st));
+    CK(cudaMemsetAsync(counters, 0, kCounterBytes, st));
+    CK(launch_prep_strain((const float2*)strain_dev, at<float2>(plan, U.dsT), U.logN1, U.logN2,
+                          (float)sqrt(2.0 / (double)plan->N), 1, st));
+    if (tm) { CK(cudaEventRecord(plan->ev[1], st)); CK(cudaEventRecord(plan->ev[2], st)); }
+    for (int t0 = 0; t0 < plan->T; t0 += U.ncols) {
+        CK(launch_layout_basis((const float2*)plan->tm_templates + (size_t)t0 * (size_t)(plan->N / 2 + 1),
+                               at<float2>(plan, U.basisP), U.ncols, plan->N / 2 + 1, plan->j_low, U.logN1, U.logN2,
+                               fft_sub(U.logN1), plan->T - t0, st));
+        rbmf_status s = run_tm_unit(plan, U);
+        if (s != RBMF_OK) return s;
+        CK(launch_tm_scan(at<float2>(plan, U.beta), U.N, 1, (int)plan->N, at<float>(plan, L.tm_isg), t0, plan->T,
+                          U.ncols, thr * thr, out_dev, counters + 1, (unsigned long long)plan->max_trig, nullptr, st));
+    }
+    CK(cudaMemcpyAsync(n_out_dev, counters + 1, 8, cudaMemcpyDeviceToDevice, st));
+    if (tm) CK(cudaEventRecord(plan->ev[3], st));
+    plan->filtered = true;
+    plan->last_nb = 1;
+    plan->last_impl = RBMF_GEMM_TCGEN05;   // counters[0] (unused here: 0 candidates) is the final candidate count
     return RBMF_OK;
 }
 

@@ -52,6 +52,7 @@ struct FftArgs {
     int nb;                  // segments of the batch: virtual chunk v = c * nb + b reads basis chunk c, strain b
     int Mseg;                // bins per segment (N / w); segment b's bins are [b Mseg, (b + 1) Mseg) of the planes
     int plane_fp16;          // 1: write ONE fp16 plane (screen mode) into plane_hi; 0: bf16 hi + lo planes
+    int no_planes;           // 1: skip step a3's plane output altogether (template routes read beta directly)
 };
 
 struct GemmArgs {
@@ -102,7 +103,16 @@ struct Stage2Args {
 // ---- launchers (each returns the cudaError_t of the launch) -------------------------------------
 cudaError_t launch_init_tables(float2* tw1_a, float2* tw1_b, float2* twN, int logL1, int logL2, cudaStream_t st);
 cudaError_t launch_layout_basis(const float2* basis, float2* basisP, int k, int64_t bins, int j_low, int logL1,
-                                int logL2, int sub, cudaStream_t st);
+                                int logL2, int sub, int rows_valid, cudaStream_t st);
+// template routes (template_route.cu)
+cudaError_t launch_tm_tables(float2* S, float2* ones, long long N, int w, long long n_ones, cudaStream_t st);
+cudaError_t launch_tm_inv_sigma(const float* sigma, float* inv_sigma, int T, cudaStream_t st);
+cudaError_t launch_tm_fold(const float2* templates, const float2* strain, const float2* S, float2* out, long long bins,
+                           int j_low, long long n_half, int w, float scale, int t0, int T, int ncols, int logL1,
+                           int logL2, int sub, cudaStream_t st);
+cudaError_t launch_tm_scan(const float2* beta, long long Nrows, int step, int nout, const float* inv_sigma, int t0,
+                           int T, int ncols, float thr_sq, rbmf_trigger* out, unsigned long long* counter,
+                           unsigned long long cap, unsigned* bin_count, cudaStream_t st);
 cudaError_t launch_prep_coeffs(const float2* coeffs, const float* sigma, float2* cs, uint16_t* c_hi,
                                uint16_t* c_lo, uint16_t* c_h16, float* tnorm_blk, int T, int Tpad, int k,
                                cudaStream_t st);

@@ -24,6 +24,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 
 RBMF_OK, RBMF_ERR_ARG, RBMF_ERR_STATE, RBMF_ERR_CUDA, RBMF_ERR_OVERFLOW, RBMF_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 RBMF_GEMM_TCGEN05, RBMF_GEMM_SCREEN = 0, 2
+RBMF_STAGE1_BASIS, RBMF_STAGE1_TEMPLATES = 0, 1
 RBMF_DIAG_STAGE1_FP32_CHECK, RBMF_DIAG_SINGLE_CTA_SCREEN, RBMF_DIAG_STAGE2_PER_CANDIDATE = 1, 2, 3
 
 TRIGGER_DTYPE = np.dtype([("template", np.int32), ("time", np.int32), ("re", np.float32), ("im", np.float32)])
@@ -45,6 +46,10 @@ SIGNATURES = {
     "rbmf_set_coeffs": (_i32, [_vp, _vp, _vp]),
     "rbmf_filter": (_i32, [_vp, _vp, _f32, _f32, _vp, _vp]),
     "rbmf_prepare_strain": (_i32, [_vp, _vp, _vp, _i32, _vp]),
+    "rbmf_plan_enable_template_routes": (_i32, [_vp, _i32]),
+    "rbmf_set_templates": (_i32, [_vp, _vp, _vp]),
+    "rbmf_plan_set_stage1_route": (_i32, [_vp, _i32]),
+    "rbmf_filter_flat": (_i32, [_vp, _vp, _f32, _vp, _vp]),
     "rbmf_filter_batch": (_i32, [_vp, _vp, _i32, _f32, _f32, _vp, _vp]),
     "rbmf_filter_host": (_i32, [_vp, _vp, _f32, _f32, _vp, _i64, _pi64]),
     "rbmf_filter_batch_host": (_i32, [_vp, _vp, _i32, _f32, _f32, _vp, _i64, _pi64]),
@@ -91,7 +96,7 @@ class Plan:
     works whether or not the caller has made `s` torch's current stream."""
 
     def __init__(self, N, fs, f_low, k, T, w=8, max_candidates=1 << 22, max_triggers=1 << 22, device="cuda:0",
-                 stream=None, max_batch=1):
+                 stream=None, max_batch=1, template_slab=0):
         import torch
         self._torch = torch
         self.N, self.fs, self.f_low, self.k, self.T, self.w = int(N), float(fs), float(f_low), int(k), int(T), int(w)
@@ -107,6 +112,9 @@ class Plan:
         self._check(_lib.rbmf_plan_set_capacity(self._h, self.max_candidates, self.max_triggers),
                     "rbmf_plan_set_capacity")
         self._check(_lib.rbmf_plan_set_batch(self._h, self.max_batch), "rbmf_plan_set_batch")
+        if template_slab:
+            self._check(_lib.rbmf_plan_enable_template_routes(self._h, int(template_slab)),
+                        "rbmf_plan_enable_template_routes")
         nbytes = ctypes.c_size_t()
         self._check(_lib.rbmf_workspace_bytes(self._h, ctypes.byref(nbytes)), "rbmf_workspace_bytes")
         self.workspace_bytes = nbytes.value
@@ -206,6 +214,31 @@ class Plan:
         with torch.cuda.device(self.device):
             self._check(_lib.rbmf_filter(self._h, _ptr(strain_dev), float(thr1), float(thr2), _ptr(self._out),
                                          _ptr(self._n_out)), "rbmf_filter")
+
+    def set_templates(self, templates_dev, sigma=None):
+        """rbmf_set_templates: a (T, N/2+1) complex64 CUDA tensor, RETAINED (kept alive by this object), + sigma."""
+        torch = self._torch
+        if (templates_dev.dtype != torch.complex64 or tuple(templates_dev.shape) != (self.T, self.N // 2 + 1)
+                or not templates_dev.is_cuda or not templates_dev.is_contiguous()):
+            raise ValueError("templates must be a contiguous complex64 CUDA tensor of shape (T, N/2+1)")
+        s = None if sigma is None else self._dev(sigma, torch.float32)
+        self._order_after_current()
+        with torch.cuda.device(self.device):
+            self._check(_lib.rbmf_set_templates(self._h, _ptr(templates_dev), _ptr(s)), "rbmf_set_templates")
+        self.stream.synchronize()
+        self._templates = templates_dev
+
+    def set_stage1_route(self, route):
+        self._check(_lib.rbmf_plan_set_stage1_route(self._h, int(route)), "rbmf_plan_set_stage1_route")
+
+    def filter_flat(self, strain, thr, allow_overflow=False):
+        """rbmf_filter_flat: the flat template method; returns triggers sorted by (template, time)."""
+        torch = self._torch
+        s = self._dev(strain, torch.complex64)
+        with torch.cuda.device(self.device):
+            self._check(_lib.rbmf_filter_flat(self._h, _ptr(s), float(thr), _ptr(self._out), _ptr(self._n_out)),
+                        "rbmf_filter_flat")
+        return self.triggers(allow_overflow)
 
     def prepare_strain(self, x_dev, inv_asd_dev=None):
         """rbmf_prepare_strain: (n_segments, N) float32 CUDA time series [+ (N/2+1,) float32 whitening array] ->
