@@ -271,6 +271,27 @@ def oracle_filter_batch(strains, basis, coeffs, sigma, N, fs, f_low, w, thr1, th
     return out
 
 
+def oracle_filter_banks(strain, banks, N, fs, f_low, thr1, thr2):
+    """Many sub-banks against one strain (Table I): `banks` is a list of dicts with keys basis, coeffs,
+    sigma, w -- each sub-bank has its own basis size and window.  Every sub-bank is the whole hot path on its own;
+    triggers of sub-bank m are reported with template = (templates of the sub-banks before it) + t.
+    Returns {'triggers', 'near', 'n_flat', 'per_bank': [oracle_filter results with local ids]}."""
+    out = {"triggers": [], "near": [], "n_flat": 0, "per_bank": []}
+    base = 0
+    for bk in banks:
+        r = oracle_filter(strain, bk["basis"], bk["coeffs"], bk["sigma"], N, fs, f_low, bk["w"], thr1, thr2)
+        out["per_bank"].append(r)
+        for key in ("triggers", "near"):
+            c = r[key].copy()
+            c["template"] += base
+            out[key].append(c)
+        out["n_flat"] += r["n_flat"]
+        base += np.asarray(bk["coeffs"]).shape[0]
+    out["triggers"] = np.concatenate(out["triggers"])
+    out["near"] = np.concatenate(out["near"])
+    return out
+
+
 # ------------------------------------------------- the paper's template routes (SURVEY.md 8(f) f2)
 def template_method_triggers(strain, templates, sigma, N, fs, f_low, thr, chunk=64):
     """The flat template method (PAPER.md:61-68; cost Eq. 13, :238; the paper's cuFFT baseline, :338): for every

@@ -420,3 +420,28 @@ def test_fast_first_stage_by_templates_gives_the_same_candidates(micro, w):
         a, b = np.sort(res[key], order=("template", "bin")), ref[key]
         assert np.array_equal(a["template"], b["template"]) and np.array_equal(a["bin"], b["bin"])
         assert np.abs(a["re"] - b["re"]).max() < 1e-12 and np.abs(a["im"] - b["im"]).max() < 1e-12
+
+
+def test_sub_banks_with_their_own_basis_size_and_window(micro):
+    """PAPER.md:146, Table I: sub-banks differ in basis size; each is filtered on its own and the triggers carry a
+    global template id.  Two sub-banks cut from `micro` (k = 8 with w = 4, k = 4 with w = 2), against a pure-Python
+    enumeration from the literal Eq. 4 sum."""
+    cfg = micro["config"]
+    N = cfg.N
+    banks = [dict(basis=micro["basis"], coeffs=micro["coeffs"][:5], sigma=micro["sigma"][:5], w=4),
+             dict(basis=micro["basis"][:4], coeffs=micro["coeffs"][5:, :4], sigma=micro["sigma"][5:], w=2)]
+    res = orc.oracle_filter_banks(micro["strain"], banks, N, cfg.fs, cfg.f_low, 1.5, 2.5)
+    exp = []
+    base = 0
+    for bk in banks:
+        hp = orc.reconstructed_templates(bk["coeffs"], bk["basis"])
+        for t in range(len(hp)):
+            rho = orc.snr_series_direct(micro["strain"], hp[t], bk["sigma"][t], N, cfg.j_low)
+            w = bk["w"]
+            for i in range(N // w):
+                if abs(sum(rho[i * w + r] for r in range(w)) / w) >= 1.5:
+                    exp += [(base + t, i * w + r) for r in range(w) if abs(rho[i * w + r]) >= 2.5]
+        base += len(hp)
+    got = [(int(a), int(b)) for a, b in zip(res["triggers"]["template"], res["triggers"]["time"])]
+    assert len(exp) > 10 and got == exp and max(t for t, _ in got) >= 5
+    assert len(res["per_bank"]) == 2 and len(res["near"]) >= len(got)
