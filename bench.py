@@ -359,6 +359,132 @@ def measure(cfg, args, rdist, rbmf, workloads, torch, device, stream, rank, worl
     return line, wl
 
 
+# ------------------------------------------------------------------------- extras: SURVEY.md 8(f) rows f1-f3
+def _time_calls(torch, stream, device, fn, steps, warmup=3):
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize(device)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        fn()
+    e1.record(stream)
+    torch.cuda.synchronize(device)
+    return e0.elapsed_time(e1) / steps
+
+
+def measure_batch(name, B, steps, rbmf, workloads, torch, device, stream):
+    """f1: B segments per call (rbmf_filter_batch) against single-segment calls on the same plan, incl. the front end
+    (rbmf_prepare_strain on B coloured time series)."""
+    cfg = workloads.CONFIGS[name]
+    wl = workloads.make_workload(cfg, device=str(device))
+    with torch.cuda.stream(stream):
+        strains = torch.from_numpy(np.stack([workloads.make_strain(wl, s)[0] for s in range(B)])).to(device)
+        xs, inv_asd = zip(*[workloads.make_time_series(wl, s) for s in range(B)])
+        x_dev, asd_dev = torch.from_numpy(np.stack(xs)).to(device), torch.from_numpy(inv_asd[0]).to(device)
+        plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, device=str(device), stream=stream,
+                         max_candidates=1 << 22, max_triggers=1 << 22, max_batch=B)
+        plan.set_basis(torch.from_numpy(wl["basis"]))
+        plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+        plan.set_timing(True)
+        ms_b = _time_calls(torch, stream, device, lambda: plan.filter_batch_async(strains, cfg.thr1, cfg.thr2), steps)
+        st_b = plan.stage_ms()
+        nc, nt, st = plan.counts(allow_overflow=True)
+        ms_1 = _time_calls(torch, stream, device, lambda: plan.filter_async(strains[0], cfg.thr1, cfg.thr2), steps)
+        st_1 = plan.stage_ms()
+        ms_fe = _time_calls(torch, stream, device, lambda: plan.prepare_strain(x_dev, asd_dev), steps)
+        plan.close()
+    seg = cfg.N / cfg.fs
+    return {"row": "f1 batched segments + front end", "workload": describe(cfg, 1)["workload"], "batch": B,
+            "ms_per_call_batch": ms_b, "ms_per_call_single": ms_1,
+            "value_batch": B * cfg.T * seg / (ms_b * 1e-3), "value_single": cfg.T * seg / (ms_1 * 1e-3),
+            "speedup_per_segment": ms_1 * B / ms_b, "stages_batch_ms": st_b, "stages_single_ms": st_1,
+            "front_end_ms_for_B_series": ms_fe, "n_candidates": nc, "n_triggers": nt,
+            "lists_overflowed": st == rbmf.RBMF_ERR_OVERFLOW, "unit": UNIT}
+
+
+def measure_routes(name, ws, steps, rbmf, workloads, torch, device, stream, slab=256):
+    """f2: the paper's two template routes against the basis/GEMM route on the same inputs."""
+    cfg0 = workloads.CONFIGS[name]
+    wl = workloads.make_workload(cfg0, device=str(device))
+    out = []
+    with torch.cuda.stream(stream):
+        strain = torch.from_numpy(wl["strain"]).to(device)
+        c = torch.from_numpy(wl["coeffs"]).to(device)
+        b = torch.from_numpy(wl["basis"]).to(device)
+        tpl = torch.empty((cfg0.T, cfg0.bins), dtype=torch.complex64, device=device)   # h'_t = sum_k c_tk b_k
+        for a in range(0, cfg0.T, 2048):
+            tpl[a:a + 2048] = c[a:a + 2048] @ b
+        del c, b
+        for w in ws:
+            cfg = cfg0.replace(w=w)
+            plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=w, device=str(device), stream=stream,
+                             max_candidates=1 << 24, max_triggers=1 << 24, template_slab=slab)
+            plan.set_basis(torch.from_numpy(wl["basis"]))
+            plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+            plan.set_templates(tpl, torch.from_numpy(wl["sigma"]))
+            plan.set_timing(True)
+            row = {"row": "f2 template routes vs basis route", "workload": describe(cfg, 1)["workload"], "w": w,
+                   "slab": slab}
+            for label, impl, route in (("basis_gemm_screen", rbmf.RBMF_GEMM_SCREEN, rbmf.RBMF_STAGE1_BASIS),
+                                       ("basis_gemm_bf16x3", rbmf.RBMF_GEMM_TCGEN05, rbmf.RBMF_STAGE1_BASIS),
+                                       ("templates_eq12", rbmf.RBMF_GEMM_TCGEN05, rbmf.RBMF_STAGE1_TEMPLATES)):
+                plan.set_gemm_impl(impl)
+                plan.set_stage1_route(route)
+                ms = _time_calls(torch, stream, device, lambda: plan.filter_async(strain, cfg.thr1, cfg.thr2), steps)
+                st = plan.stage_ms()
+                nc, nt, _ = plan.counts(allow_overflow=True)
+                row[label] = {"ms_per_call": ms, "stage1_ms": st["gemm"], "fft_ms": st["fft"], "stage2_ms": st["stage2"],
+                              "n_candidates": nc, "n_triggers": nt}
+            plan.set_stage1_route(rbmf.RBMF_STAGE1_BASIS)
+            if w == ws[0]:
+                def flat():
+                    plan._check(rbmf.rbmf_filter_flat(plan._h, strain.data_ptr(), float(cfg.thr2), plan._out.data_ptr(),
+                                                      plan._n_out.data_ptr()), "rbmf_filter_flat")
+                ms = _time_calls(torch, stream, device, flat, max(2, steps // 2), warmup=1)
+                _, nt, _ = plan.counts(allow_overflow=True)
+                bank_bytes = cfg.T * (cfg.N // 2 - cfg.j_low) * 8
+                row["flat_template_method"] = {"ms_per_call": ms, "n_triggers": nt,
+                                               "bank_GBps": bank_bytes / (ms * 1e-3) / 1e9,
+                                               "value": cfg.T * (cfg.N / cfg.fs) / (ms * 1e-3)}
+            plan.close()
+            out.append(row)
+    return out
+
+
+def measure_bankset(steps, rbmf, workloads, torch, device, stream):
+    """f3: four sub-banks with their own basis sizes (Table I) against one strain: one bank-set call
+    against the same plans called one after the other."""
+    base = workloads.CONFIGS["small"]
+    parts = [(1.0, 1.5, 64, 500, 8), (1.5, 2.0, 128, 700, 8), (2.0, 2.5, 96, 300, 8), (2.5, 3.0, 128, 500, 16)]
+    subs = workloads.make_subbanks(base, parts, device=str(device))
+    with torch.cuda.stream(stream):
+        strain = torch.from_numpy(subs[0]["strain"]).to(device)
+        plans = []
+        for wl in subs:
+            cfg = wl["config"]
+            p = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, device=str(device), stream=stream,
+                          max_candidates=1 << 20, max_triggers=1 << 20)
+            p.set_basis(torch.from_numpy(wl["basis"]))
+            p.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+            plans.append(p)
+        bs = rbmf.BankSet(plans, max_triggers=1 << 22, stream=stream)
+        ms_set = _time_calls(torch, stream, device, lambda: bs.filter_async(strain, base.thr1, base.thr2), steps)
+        nc, nt, tot, _ = bs.counts()
+
+        def one_by_one():
+            for p in plans:
+                p.filter_async(strain, base.thr1, base.thr2)
+        ms_seq = _time_calls(torch, stream, device, one_by_one, steps)
+        bs.close()
+        for p in plans:
+            p.close()
+    tsec = sum(wl["config"].T for wl in subs) * (base.N / base.fs)
+    return {"row": "f3 many sub-banks", "sub_banks": [{"k": k, "T": T, "w": w, "mc": [lo, hi]} for lo, hi, k, T, w in parts],
+            "N": base.N, "ms_bank_set": ms_set, "ms_one_by_one": ms_seq, "value_bank_set": tsec / (ms_set * 1e-3),
+            "n_triggers": tot, "per_sub_bank_triggers": nt, "unit": UNIT}
+
+
 # ---------------------------------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -374,6 +500,10 @@ def main():
                     help="configs summarised in the `configs` array of the default line ('' = none)")
     ap.add_argument("--summary-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extras", default="batch,routes,bankset",
+                    help="SURVEY 8(f) rows measured into the `extras` array of the default line: batch (f1: small at "
+                         "B=8, paper at B=4), routes (f2: template routes vs GEMM route on small and paper), bankset "
+                         "(f3); '' = none")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -435,6 +565,16 @@ def main():
                                     world, local_rank, False)
                 del wl2
                 line["configs"].append(summ)
+            ex = [e for e in args.extras.split(",") if e]
+            line["extras"] = []
+            if "batch" in ex:
+                line["extras"].append(measure_batch("small", 8, 20, rbmf, workloads, torch, device, stream))
+                line["extras"].append(measure_batch("paper", 4, 10, rbmf, workloads, torch, device, stream))
+            if "routes" in ex:
+                line["extras"] += measure_routes("small", (8, 16), 10, rbmf, workloads, torch, device, stream)
+                line["extras"] += measure_routes("paper", (8, 16), 4, rbmf, workloads, torch, device, stream)
+            if "bankset" in ex:
+                line["extras"].append(measure_bankset(20, rbmf, workloads, torch, device, stream))
         if rank == 0:
             print(json.dumps(line), flush=True)
     rdist.finalize()

@@ -185,6 +185,25 @@ rbmf_status rbmf_plan_set_stage1_route(rbmf_plan* plan, int32_t route);
 rbmf_status rbmf_filter_flat(rbmf_plan* plan, const void* strain_dev, float thr, rbmf_trigger* out_dev,
                              int64_t* n_out_dev);
 
+/* ---- Many sub-banks against one strain (the bank is split into 64 sub-banks of 6250 templates, each
+ * with its own basis P^m and coefficients D^m; Table I :154-165: p = 64 / 254 / 200 ...) -------------------------------
+ * A bank set groups fully set-up plans (workspace, basis, coefficients) that agree on N, fs and f_low; k, T, w, list
+ * capacities and the stage-1 kernel may differ per sub-bank.  rbmf_bankset_filter filters one strain segment against
+ * all of them: the sub-banks are launched most-expensive-first (cost 8 T k N / w) round-robin on up to four internal
+ * streams forked from / joined to `cuda_stream`, so the short kernels and the tails of one sub-bank overlap the next;
+ * all sub-banks append to ONE trigger list out_dev (capacity max_triggers) through one shared position counter
+ * n_out_dev (device int64: total found, may exceed max_triggers), with template_id = (sum of T of the sub-banks before
+ * it in `plans`) + the template's row in its own sub-bank.  The result equals the union of rbmf_filter over the plans.
+ * The plans must not be used by other calls while a bank-set call is in flight; the set does not own them (destroy the
+ * set first).  rbmf_bankset_get_counts synchronises and returns per-sub-bank candidates / triggers (arrays of n_plans,
+ * may be NULL) and the total; RBMF_ERR_OVERFLOW if a sub-bank's candidate list overflowed. */
+typedef struct rbmf_bankset rbmf_bankset;
+rbmf_status rbmf_bankset_create(rbmf_bankset** out, rbmf_plan* const* plans, int32_t n_plans);
+rbmf_status rbmf_bankset_filter(rbmf_bankset* set, const void* strain_dev, float thr_stage1, float thr_stage2,
+                                rbmf_trigger* out_dev, int64_t max_triggers, int64_t* n_out_dev, void* cuda_stream);
+rbmf_status rbmf_bankset_get_counts(rbmf_bankset* set, int64_t* n_candidates, int64_t* n_triggers, int64_t* n_total);
+rbmf_status rbmf_bankset_destroy(rbmf_bankset* set);
+
 /* Counts of the last rbmf_filter (synchronises the stream).  RBMF_ERR_OVERFLOW if a capacity was exceeded
  * (in RBMF_GEMM_SCREEN mode the capacity max_candidates applies to the screened superset, see
  * rbmf_get_screened_count, while *n_candidates reports the candidates confirmed at fp32 accuracy). */

@@ -62,6 +62,10 @@ struct rbmf_plan {
     int tm_slab, stage1_route;
     TmUnit tmF, tmS;     // flat method: length N; fast first stage: length 2 N / w
     const void* tm_templates;   // caller's T x (N/2+1) bank (retained pointer)
+    // bank sets (rbmf_bankset_*): a trigger list and position counter shared with other plans, sub-bank id offset
+    unsigned long long* shared_trig_counter;
+    unsigned long long shared_trig_cap;
+    int template_offset;
     bool have_templates;
     bool have_maps;
     cudaEvent_t ev[5];
@@ -537,9 +541,12 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     memset(&s2, 0, sizeof(s2));
     s2.cand = g.cand; s2.cs = at<float2>(plan, L.cs); s2.beta = at<float2>(plan, L.beta);
     s2.out = out_dev; s2.counters = counters;
+    s2.trig_counter = plan->shared_trig_counter ? plan->shared_trig_counter : counters + 1;
+    s2.template_offset = plan->template_offset;
     const bool confirm = screen && !by_templates;   // the list is the fp16 screen's superset: confirm in fp32
     s2.confirmed = at<rbmf_candidate>(plan, L.cand2); s2.thr1_sq = g.thr1_sq; s2.screen = confirm ? 1 : 0;
-    s2.cand_cap = (unsigned long long)plan->max_cand; s2.trig_cap = (unsigned long long)plan->max_trig;
+    s2.cand_cap = (unsigned long long)plan->max_cand;
+    s2.trig_cap = plan->shared_trig_counter ? plan->shared_trig_cap : (unsigned long long)plan->max_trig;
     s2.thr2_sq = thr_stage2 * thr_stage2; s2.k = plan->k; s2.w = plan->w; s2.N = plan->N;
     s2.bin_count = g.bin_count; s2.bin_start = at<unsigned>(plan, L.bin_start); s2.items = at<int4>(plan, L.items);
     s2.sorted = at<rbmf_candidate>(plan, L.cand3);
@@ -763,5 +770,132 @@ const char* rbmf_status_string(rbmf_status status) {
 }
 
 int32_t rbmf_last_cuda_error(const rbmf_plan* plan) { return plan ? plan->last_cuda : 0; }
+
+// ---- bank sets: many sub-banks against one strain (Table I) ------------------------
+struct rbmf_bankset {
+    int n;
+    rbmf_plan** plans;
+    int* order;          // launch order: most expensive sub-bank first
+    int* offsets;        // template id base of each sub-bank
+    int nstreams;
+    cudaStream_t streams[4];
+    cudaEvent_t fork, join[4];
+    cudaStream_t last_stream;
+    unsigned long long* last_counter;
+    bool filtered;
+};
+
+rbmf_status rbmf_bankset_create(rbmf_bankset** out, rbmf_plan* const* plans, int32_t n_plans) {
+    if (!out) return RBMF_ERR_ARG;
+    *out = nullptr;
+    if (!plans || n_plans < 1 || n_plans > 4096) return RBMF_ERR_ARG;
+    int64_t total_T = 0;
+    for (int i = 0; i < n_plans; ++i) {
+        const rbmf_plan* p = plans[i];
+        if (!p) return RBMF_ERR_ARG;
+        if (!p->have_ws || !p->have_basis || !p->have_coeffs) return RBMF_ERR_STATE;
+        if (p->N != plans[0]->N || p->fs != plans[0]->fs || p->f_low != plans[0]->f_low) return RBMF_ERR_ARG;
+        for (int j = 0; j < i; ++j)
+            if (plans[j] == p) return RBMF_ERR_ARG;
+        total_T += p->T;
+    }
+    if (total_T > (int64_t(1) << 31) - 1) return RBMF_ERR_ARG;
+    rbmf_bankset* b = new (std::nothrow) rbmf_bankset;
+    if (!b) return RBMF_ERR_ARG;
+    memset(b, 0, sizeof(*b));
+    b->n = n_plans;
+    b->plans = new (std::nothrow) rbmf_plan*[n_plans];
+    b->order = new (std::nothrow) int[n_plans];
+    b->offsets = new (std::nothrow) int[n_plans];
+    if (!b->plans || !b->order || !b->offsets) { delete[] b->plans; delete[] b->order; delete[] b->offsets; delete b; return RBMF_ERR_ARG; }
+    int off = 0;
+    for (int i = 0; i < n_plans; ++i) { b->plans[i] = plans[i]; b->order[i] = i; b->offsets[i] = off; off += plans[i]->T; }
+    // longest first: the cost of a sub-bank is dominated by its reconstruction, 8 T k N / w flops
+    auto cost = [&](int i) { const rbmf_plan* p = b->plans[i]; return (double)p->T * p->k * (double)p->M; };
+    for (int i = 1; i < n_plans; ++i) {
+        const int v = b->order[i];
+        int j = i - 1;
+        while (j >= 0 && cost(b->order[j]) < cost(v)) { b->order[j + 1] = b->order[j]; --j; }
+        b->order[j + 1] = v;
+    }
+    b->nstreams = n_plans < 4 ? n_plans : 4;
+    rbmf_plan* plan = plans[0];   // for CK's error slot
+    cudaError_t e = cudaEventCreateWithFlags(&b->fork, cudaEventDisableTiming);
+    for (int i = 0; i < b->nstreams && e == cudaSuccess; ++i) {
+        e = cudaStreamCreateWithFlags(&b->streams[i], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&b->join[i], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) { rbmf_bankset_destroy(b); return cuda_fail(plan, e); }
+    *out = b;
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_bankset_filter(rbmf_bankset* bs, const void* strain_dev, float thr_stage1, float thr_stage2,
+                                rbmf_trigger* out_dev, int64_t max_triggers, int64_t* n_out_dev, void* cuda_stream) {
+    if (!bs || !strain_dev || !out_dev || !n_out_dev || max_triggers < 1) return RBMF_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    rbmf_plan* plan = bs->plans[0];
+    CK(cudaMemsetAsync(n_out_dev, 0, 8, st));
+    CK(cudaEventRecord(bs->fork, st));
+    for (int i = 0; i < bs->nstreams; ++i) CK(cudaStreamWaitEvent(bs->streams[i], bs->fork, 0));
+    rbmf_status result = RBMF_OK;
+    for (int q = 0; q < bs->n && result == RBMF_OK; ++q) {
+        rbmf_plan* p = bs->plans[bs->order[q]];
+        cudaStream_t saved = p->stream;
+        p->stream = bs->streams[q % bs->nstreams];
+        p->shared_trig_counter = (unsigned long long*)n_out_dev;
+        p->shared_trig_cap = (unsigned long long)max_triggers;
+        p->template_offset = bs->offsets[bs->order[q]];
+        // the plan's own trigger count lands in its counter word 9 (word 8 belongs to rbmf_filter_host)
+        result = rbmf_filter(p, strain_dev, thr_stage1, thr_stage2, out_dev,
+                             (int64_t*)(p->ws + p->lay.counters + 72));
+        p->stream = saved;
+        p->shared_trig_counter = nullptr;
+        p->template_offset = 0;
+    }
+    for (int i = 0; i < bs->nstreams; ++i) {
+        CK(cudaEventRecord(bs->join[i], bs->streams[i]));
+        CK(cudaStreamWaitEvent(st, bs->join[i], 0));
+    }
+    bs->last_stream = st;
+    bs->last_counter = (unsigned long long*)n_out_dev;
+    bs->filtered = result == RBMF_OK;
+    return result;
+}
+
+rbmf_status rbmf_bankset_get_counts(rbmf_bankset* bs, int64_t* n_candidates, int64_t* n_triggers, int64_t* n_total) {
+    if (!bs) return RBMF_ERR_ARG;
+    if (!bs->filtered) return RBMF_ERR_STATE;
+    rbmf_plan* plan = bs->plans[0];
+    CK(cudaStreamSynchronize(bs->last_stream));
+    rbmf_status result = RBMF_OK;
+    unsigned long long total = 0;
+    for (int i = 0; i < bs->n; ++i) {
+        rbmf_plan* p = bs->plans[i];
+        unsigned long long h[3] = {0, 0, 0};
+        CK(cudaMemcpy(h, p->ws + p->lay.counters, 24, cudaMemcpyDeviceToHost));
+        if (n_candidates) n_candidates[i] = (int64_t)(p->last_impl == RBMF_GEMM_SCREEN ? h[2] : h[0]);
+        if (n_triggers) n_triggers[i] = (int64_t)h[1];
+        total += h[1];
+        if ((int64_t)h[0] > p->max_cand) result = RBMF_ERR_OVERFLOW;
+    }
+    unsigned long long shared = 0;
+    CK(cudaMemcpy(&shared, bs->last_counter, 8, cudaMemcpyDeviceToHost));
+    if (n_total) *n_total = (int64_t)shared;
+    if (shared != total) { plan->last_cuda = -2; return RBMF_ERR_CUDA; }   // cannot happen: both count the same appends
+    return result;
+}
+
+rbmf_status rbmf_bankset_destroy(rbmf_bankset* bs) {
+    if (!bs) return RBMF_ERR_ARG;
+    for (int i = 0; i < bs->nstreams; ++i) {
+        if (bs->streams[i]) { cudaStreamSynchronize(bs->streams[i]); cudaStreamDestroy(bs->streams[i]); }
+        if (bs->join[i]) cudaEventDestroy(bs->join[i]);
+    }
+    if (bs->fork) cudaEventDestroy(bs->fork);
+    delete[] bs->plans; delete[] bs->order; delete[] bs->offsets;
+    delete bs;
+    return RBMF_OK;
+}
 
 }  // extern "C"

@@ -88,6 +88,9 @@ struct Stage2Args {
     const float2* cs;         // T x k: conj(c_tk) / sigma_t
     const float2* beta;       // [chunk][n][C]
     rbmf_trigger* out;
+    unsigned long long* trig_counter;   // list position counter of `out`: counters + 1, or a counter shared by the
+                                        // plans of a bank set (then counters[1] still counts this plan's own triggers)
+    int template_offset;                // added to the template id of every trigger (sub-bank base in a bank set)
     rbmf_candidate* confirmed;   // screen mode: candidates whose fp32 averaged SNR passes thr1 (counters[2])
     float thr1_sq;
     int screen;                  // 1: `cand` is the screened superset; confirm before scoring

@@ -92,7 +92,10 @@ __global__ void __launch_bounds__(NWARP * 32) stage2_score_kernel(const Stage2Ar
     int tcount = 0, ccount = 0;   // warp-uniform fill levels
     auto flush_triggers = [&]() {
         unsigned long long base = 0;
-        if (lane == 0) base = atomicAdd(a.counters + 1, (unsigned long long)tcount);
+        if (lane == 0) {
+            base = atomicAdd(a.trig_counter, (unsigned long long)tcount);
+            if (a.trig_counter != a.counters + 1) atomicAdd(a.counters + 1, (unsigned long long)tcount);
+        }
         base = __shfl_sync(0xffffffffu, base, 0);
         __syncwarp();
         for (int i = lane; i < tcount; i += 32)
@@ -221,7 +224,7 @@ __global__ void __launch_bounds__(NWARP * 32) stage2_score_kernel(const Stage2Ar
             if (bal) {
                 if (hit) {
                     rbmf_trigger tr;
-                    tr.template_id = t; tr.time_index = bin * W + r; tr.snr_re = re; tr.snr_im = im;
+                    tr.template_id = t + a.template_offset; tr.time_index = bin * W + r; tr.snr_re = re; tr.snr_im = im;
                     tbuf[tcount + __popc(bal & ((1u << lane) - 1u))] = tr;
                 }
                 tcount += __popc(bal);

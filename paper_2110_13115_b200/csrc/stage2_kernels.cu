@@ -22,7 +22,10 @@ __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
     int tcount = 0, ccount = 0;   // warp-uniform fill levels
     auto flush_triggers = [&](int lane_) {
         unsigned long long base = 0;
-        if (lane_ == 0) base = atomicAdd(a.counters + 1, (unsigned long long)tcount);
+        if (lane_ == 0) {
+            base = atomicAdd(a.trig_counter, (unsigned long long)tcount);
+            if (a.trig_counter != a.counters + 1) atomicAdd(a.counters + 1, (unsigned long long)tcount);
+        }
         base = __shfl_sync(0xffffffffu, base, 0);
         __syncwarp();
         for (int i = lane_; i < tcount; i += 32)
@@ -133,7 +136,7 @@ __global__ void __launch_bounds__(256) stage2_kernel(const Stage2Args a) {
             if (ballot) {
                 if (hit) {
                     rbmf_trigger t;
-                    t.template_id = cd.template_id;
+                    t.template_id = cd.template_id + a.template_offset;
                     t.time_index = cd.bin_index * w + r;
                     t.snr_re = vr;
                     t.snr_im = vi;

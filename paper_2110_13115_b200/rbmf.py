@@ -46,6 +46,10 @@ SIGNATURES = {
     "rbmf_set_coeffs": (_i32, [_vp, _vp, _vp]),
     "rbmf_filter": (_i32, [_vp, _vp, _f32, _f32, _vp, _vp]),
     "rbmf_prepare_strain": (_i32, [_vp, _vp, _vp, _i32, _vp]),
+    "rbmf_bankset_create": (_i32, [ctypes.POINTER(_vp), ctypes.POINTER(_vp), _i32]),
+    "rbmf_bankset_filter": (_i32, [_vp, _vp, _f32, _f32, _vp, _i64, _vp, _vp]),
+    "rbmf_bankset_get_counts": (_i32, [_vp, _pi64, _pi64, _pi64]),
+    "rbmf_bankset_destroy": (_i32, [_vp]),
     "rbmf_plan_enable_template_routes": (_i32, [_vp, _i32]),
     "rbmf_set_templates": (_i32, [_vp, _vp, _vp]),
     "rbmf_plan_set_stage1_route": (_i32, [_vp, _i32]),
@@ -407,6 +411,69 @@ class Plan:
             except Exception:
                 pass
             _lib.rbmf_plan_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class BankSet:
+    """rbmf_bankset_*: several fully set-up `Plan`s (sub-banks with their own k, T, w; same N, fs, f_low) filtered
+    against one strain into one trigger list; template ids are offset by the sizes of the sub-banks before."""
+
+    def __init__(self, plans, max_triggers=1 << 22, stream=None):
+        import torch
+        self._torch = torch
+        self.plans = list(plans)
+        self.device = self.plans[0].device
+        self.max_triggers = int(max_triggers)
+        self.stream = stream if stream is not None else self.plans[0].stream
+        self._h = _vp()
+        arr = (_vp * len(self.plans))(*[p._h for p in self.plans])
+        torch.cuda.synchronize(self.device)          # every plan's set-up work is complete
+        with torch.cuda.device(self.device):
+            st = _lib.rbmf_bankset_create(ctypes.byref(self._h), arr, len(self.plans))
+        if st != RBMF_OK:
+            raise RbmfError(st, "rbmf_bankset_create")
+        with torch.cuda.stream(self.stream):
+            self._out = torch.empty(self.max_triggers * 4, dtype=torch.int32, device=self.device)
+            self._n_out = torch.zeros(1, dtype=torch.int64, device=self.device)
+
+    def filter_async(self, strain_dev, thr1, thr2):
+        with self._torch.cuda.device(self.device):
+            st = _lib.rbmf_bankset_filter(self._h, _ptr(strain_dev), float(thr1), float(thr2), _ptr(self._out),
+                                          self.max_triggers, _ptr(self._n_out), _vp(self.stream.cuda_stream))
+        if st != RBMF_OK:
+            raise RbmfError(st, "rbmf_bankset_filter")
+
+    def counts(self):
+        n = len(self.plans)
+        nc, nt, tot = (_i64 * n)(), (_i64 * n)(), _i64()
+        with self._torch.cuda.device(self.device):
+            st = _lib.rbmf_bankset_get_counts(self._h, nc, nt, ctypes.byref(tot))
+        if st not in (RBMF_OK, RBMF_ERR_OVERFLOW):
+            raise RbmfError(st, "rbmf_bankset_get_counts")
+        return list(nc), list(nt), tot.value, st
+
+    def filter(self, strain, thr1, thr2):
+        torch = self._torch
+        with torch.cuda.stream(self.stream):
+            s = torch.as_tensor(strain).to(self.device)
+        self.filter_async(s, thr1, thr2)
+        _, _, tot, _ = self.counts()
+        n = min(tot, self.max_triggers)
+        with torch.cuda.stream(self.stream):
+            raw = self._out[: 4 * n].cpu().numpy()
+        trig = raw.view(TRIGGER_DTYPE).copy() if n else np.empty(0, dtype=TRIGGER_DTYPE)
+        return np.sort(trig, order=("template", "time"))
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._torch.cuda.synchronize(self.device)
+            _lib.rbmf_bankset_destroy(self._h)
             self._h = _vp()
 
     def __del__(self):

@@ -274,3 +274,16 @@ def make_time_series(wl: dict, segment: int = 0) -> tuple:
     asd = np.sqrt(1.0 + (2.0 * cfg.f_low / np.maximum(f, cfg.f_low)) ** 4 + (f / (cfg.fs / 4.0)) ** 2)
     x = np.fft.irfft(d.astype(np.complex128) * asd, n=cfg.N)
     return x.astype(np.float32), (1.0 / asd).astype(np.float32)
+
+
+def make_subbanks(cfg: WorkloadConfig, parts, device: Optional[str] = None) -> list:
+    """Sub-banks in the manner of the paper (Table I: the bank is cut into chirp-time slices, each with
+    its own basis size): `parts` is a list of (mc_lo, mc_hi, k, T, w); sub-bank m is `make_workload` of `cfg` with
+    those fields replaced (seed index 1000 * cfg.index + m).  All are meant to be filtered against the strain of
+    sub-bank 0 (its noise and its injections)."""
+    out = []
+    for m, (mc_lo, mc_hi, k, T, w) in enumerate(parts):
+        sub = cfg.replace(name="%s_sub%d" % (cfg.name, m), index=1000 * cfg.index + m, mc_lo=mc_lo, mc_hi=mc_hi, k=k,
+                          T=T, w=w)
+        out.append(make_workload(sub, device=device))
+    return out

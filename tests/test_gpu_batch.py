@@ -273,3 +273,44 @@ def test_time_series_to_triggers(rbmf):
     rep = compare.compare_triggers(got, ref, nb * cfg.N, *thr)
     plan.close()
     assert rep["ok"] and rep["n_mandatory"] > 100, rep
+
+
+# ------------------------------------------------------------------------------------- many sub-banks (f3)
+def test_bank_set_of_three_sub_banks(rbmf):
+    """Three sub-banks with different basis sizes, template counts and windows (Table I) against one
+    strain: one call, one trigger list with global template ids, equal to the oracle's union."""
+    import torch
+    base = wlm.CONFIGS["mini"]
+    subs = wlm.make_subbanks(base, [(1.0, 1.07, 32, 300, 8), (1.07, 1.14, 48, 130, 4), (1.14, 1.2, 16, 257, 8)],
+                             device="cuda")
+    strain = subs[0]["strain"]
+    thr = (3.0, 4.0)
+    plans = []
+    for i, wl in enumerate(subs):
+        cfg = wl["config"]
+        p = make_plan(rbmf, wl, w=cfg.w, impl=(SCREEN, X3, SCREEN)[i], cap=1 << 18)
+        plans.append(p)
+    bs = rbmf.BankSet(plans, max_triggers=1 << 20)
+    got = bs.filter(torch.from_numpy(strain), *thr)
+    nc, nt, tot, st = bs.counts()
+    ref = orc.oracle_filter_banks(strain, [dict(basis=w_["basis"], coeffs=w_["coeffs"], sigma=w_["sigma"],
+                                                w=w_["config"].w) for w_ in subs], base.N, base.fs, base.f_low, *thr)
+    rep = compare.compare_triggers(got, ref, base.N, *thr)
+    assert rep["ok"] and rep["n_mandatory"] > 500, rep
+    assert st == rbmf.RBMF_OK and tot == len(got) == sum(nt)
+    bounds = np.cumsum([0] + [w_["config"].T for w_ in subs])
+    for m in range(3):
+        in_m = (got["template"] >= bounds[m]) & (got["template"] < bounds[m + 1])
+        assert in_m.sum() == nt[m] > 0
+        crep = compare.compare_candidates(plans[m].candidates(), ref["per_bank"][m], base.N // subs[m]["config"].w, thr[0])
+        assert crep["ok"], crep
+    # the same plans still work on their own afterwards, with local template ids
+    one = plans[1].filter(torch.from_numpy(strain), *thr)
+    sel = got[(got["template"] >= bounds[1]) & (got["template"] < bounds[2])]
+    assert np.array_equal(one["time"], sel["time"]) and np.array_equal(one["template"] + bounds[1], sel["template"])
+    # a second call reuses the set
+    got2 = bs.filter(torch.from_numpy(strain), *thr)
+    assert np.array_equal(got2, got)
+    bs.close()
+    for p in plans:
+        p.close()
