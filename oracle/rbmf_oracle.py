@@ -36,6 +36,7 @@ Pins (tests/test_oracle_pins.py, all `-m "not gpu"`):
   template routes              flat method: pure-Python enumeration of `snr_series_direct` on the BANK templates, and its
                                count == oracle_filter's n_flat on reconstructed templates; fast first stage: candidates ==
                                oracle_filter's (Eq. 12 route == binned mean, already pinned) incl. the values
+  tuning, Eq. 16               hand-built lists with the answer worked out by counting; w = 1 recovers everything
   forward transform, whitening literal O(N^2) sum at small N, a cosine's closed form (N/2 at its bin), Parseval; batches:
                                segment b of `oracle_filter_batch` against the time-domain brute force on strain b alone
 Parity status: every function below is pinned by at least one of these; nothing is "parity unpinned".
@@ -351,6 +352,29 @@ def evaluate_points(strain, basis, coeffs, sigma, N, fs, f_low, w, template, tim
         b = n // w
         rbar.append(sum(snr_point(strain, h, sg, N, j_low, b * w + r) for r in range(w)) / w)
     return np.array(rho), np.array(rbar)
+
+
+# ------------------------------------------------------- tuning of (w, rho_I), Eq. 16
+def rho_target(final_mods, flat_mods, grid, ratio=0.99):
+    """Eq. 16 (PAPER.md:253-258): rho_target(w, rho_I) = min{rho_II : n_final(rho_II) >= ratio * n_flat(rho_II)}, with
+    n_final / n_flat the numbers of hierarchical / flat triggers whose SNR modulus is >= rho_II, searched over the
+    ascending thresholds `grid`.  The hierarchical set is a subset of the flat one and the recovered fraction grows
+    with rho_II in noise, so "min" is read as the first grid value from which the condition holds for ALL larger grid
+    values with flat triggers (a single lucky threshold below a failing one does not count).  Returns (rho_target or
+    None if never reached, n_final[grid], n_flat[grid])."""
+    fm = np.sort(np.asarray(final_mods, dtype=np.float64))
+    fl = np.sort(np.asarray(flat_mods, dtype=np.float64))
+    grid = np.asarray(grid, dtype=np.float64)
+    n_final = len(fm) - np.searchsorted(fm, grid, side="left")
+    n_flat = len(fl) - np.searchsorted(fl, grid, side="left")
+    ok = n_final >= ratio * n_flat
+    target = None
+    for i in range(len(grid) - 1, -1, -1):
+        if not ok[i]:
+            break
+        if n_flat[i] > 0:
+            target = float(grid[i])
+    return target, n_final, n_flat
 
 
 # ------------------------------------------------------- cost model, Eq. 13-15

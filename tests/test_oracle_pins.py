@@ -445,3 +445,36 @@ def test_sub_banks_with_their_own_basis_size_and_window(micro):
     got = [(int(a), int(b)) for a, b in zip(res["triggers"]["template"], res["triggers"]["time"])]
     assert len(exp) > 10 and got == exp and max(t for t, _ in got) >= 5
     assert len(res["per_bank"]) == 2 and len(res["near"]) >= len(got)
+
+
+# ---------------------------------------------------------------- Eq. 16 (tuning part)
+def test_rho_target_on_hand_built_lists():
+    """PAPER.md:253-258.  flat = {4.0 x100, 5.0 x100, 6.0 x100, 7.0 x10}; the hierarchical search lost 30 of the 4.0s,
+    2 of the 5.0s and none above.  Counting by hand at rho_II = 4, 5, 5.5, 6, 7:
+      n_flat = 310, 210, 110, 110, 10;  n_final = 278, 208, 110, 110, 10;  ratios 0.897, 0.990.., 1, 1, 1."""
+    flat = np.r_[np.full(100, 4.0), np.full(100, 5.0), np.full(100, 6.0), np.full(10, 7.0)]
+    final = np.r_[np.full(70, 4.0), np.full(98, 5.0), np.full(100, 6.0), np.full(10, 7.0)]
+    grid = [4.0, 5.0, 5.5, 6.0, 7.0, 8.0]
+    t, nf, nl = orc.rho_target(final, flat, grid, 0.99)
+    assert list(nl) == [310, 210, 110, 110, 10, 0] and list(nf) == [278, 208, 110, 110, 10, 0]
+    assert t == 5.0                                     # 208 / 210 = 0.9905 >= 0.99
+    assert orc.rho_target(final, flat, grid, 0.995)[0] == 5.5
+    assert orc.rho_target(final, flat, grid, 0.85)[0] == 4.0
+    # a lucky low threshold below a failing one does not count
+    final2 = np.r_[np.full(100, 4.0), np.full(50, 5.0), np.full(100, 6.0), np.full(10, 7.0)]
+    assert orc.rho_target(final2, flat, [4.0, 5.0, 6.0], 0.99)[0] == 6.0
+    assert orc.rho_target(final[:0], flat, grid)[0] is None
+
+
+def test_rho_target_of_the_flat_search_is_the_lowest_threshold(micro):
+    cfg = micro["config"]
+    res = orc.oracle_filter(micro["strain"], micro["basis"], micro["coeffs"], micro["sigma"], cfg.N, cfg.fs, cfg.f_low,
+                            1, 2.0, 2.0)
+    mods = np.hypot(res["triggers"]["re"], res["triggers"]["im"])
+    grid = np.arange(2.0, 5.0, 0.25)
+    assert orc.rho_target(mods, mods, grid)[0] == 2.0
+    res4 = orc.oracle_filter(micro["strain"], micro["basis"], micro["coeffs"], micro["sigma"], cfg.N, cfg.fs, cfg.f_low,
+                             4, 1.5, 2.0)
+    m4 = np.hypot(res4["triggers"]["re"], res4["triggers"]["im"])
+    t4, nf, nl = orc.rho_target(m4, mods, grid)
+    assert (nf <= nl).all() and (t4 is None or t4 >= 2.0)
