@@ -171,6 +171,11 @@ __device__ __forceinline__ unsigned long long policy_evict_first() {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
+__device__ __forceinline__ unsigned long long policy_evict_normal() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
 __device__ __forceinline__ unsigned long long policy_evict_last() {
     unsigned long long pol;
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
@@ -235,11 +240,21 @@ struct Cfg {
     static constexpr int TILE_F2 = ROWS * RB;         // float2 per tile buffer
     // strain slice of a pass-1 tile: one row of H values per line, rows offset so that the SUB lines a warp reads at
     // once fall into different banks
-    static constexpr int SPAD = 16 / SUB > 2 ? 16 / SUB : 2;
+    static constexpr int SPAD = fft_spad(LOGL);
     __device__ static __forceinline__ int idx(int p) { return PAD ? p + (p >> 5) : p; }
 };
 
 enum TileType : int { TILE_NOP = 0, TILE_P1 = 1, TILE_P2 = 2, TILE_STOP = 3 };
+
+// Cycle accounting of the producer / consumer hand-off (build with -DRBMF_FFT_PROFILE; read by rbmf_fft_profile_read).
+#ifdef RBMF_FFT_PROFILE
+__device__ unsigned long long g_fft_prof[32];
+#define PROF_T() clock64()
+#define PROF_ADD(i, v) atomicAdd(&g_fft_prof[i], (unsigned long long)(v))
+#else
+#define PROF_T() 0ll
+#define PROF_ADD(i, v) ((void)0)
+#endif
 
 template <int LOG1, int LOG2>
 struct Smem {
@@ -250,8 +265,8 @@ struct Smem {
     static constexpr size_t TW_B = TW_A + ((size_t)8 << LOG1);            // tw1_b: L2 float2
     static constexpr size_t BARS = TW_B + ((size_t)8 << LOG2);            // full[NBUF][NGROUP], empty[NBUF]
     static constexpr size_t E2S = BARS + 3 * NBUF * 8;                    // float2 e2s[NGROUP][kE2Stride]
-    static constexpr size_t META = E2S + NGROUP * kE2Stride * 8;          // int4 meta[NBUF]
-    static constexpr size_t TOTAL = META + NBUF * 16 + 128 /* base alignment slack */;
+    static constexpr size_t META = E2S + NGROUP * kE2Stride * 8;          // int4 meta[2 NBUF]: tile descriptors (ring)
+    static constexpr size_t TOTAL = META + 2 * NBUF * 16 + 128 /* base alignment slack */;
 };
 
 // ------------------------------------------------------------------------------------------- pass 1 (consumer)
@@ -496,99 +511,113 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp >= NGROUP * (GT / 32)) {
         // the producer needs few registers: hand the rest of the register file to the consumer warpgroups
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
         if (warp > NGROUP * (GT / 32)) return;
         // =========================================== producer ===========================================
         if (lane == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmY) : "memory");
-        const unsigned long long pol_first = policy_evict_first(), pol_last = policy_evict_last();
+        const unsigned long long pol_first = policy_evict_first(), pol_last = policy_evict_last(),
+                                 pol_normal = policy_evict_normal();
         int next_ticket = 0;
         if (lane == 0) next_ticket = (int)atomicAdd(a.sched, 1u);
-        int it_chunk[NGROUP] = {0, 0}, it_n1[NGROUP] = {0, 0}, it_rd[NGROUP] = {0, 0};   // open pass-2 items
-        bool it_open[NGROUP] = {false, false};
+        // open pass-2 items of the two groups, as scalars (an array indexed by the group would live in local memory)
+        int oc0 = 0, on0 = 0, or0 = 0, oc1 = 0, on1 = 0, or1 = 0;
+        bool open0 = false, open1 = false;
+        // n1t and n2t are powers of two; the one true division of the ticket decode, by per = n1t + n2t, is done with
+        // a float reciprocal and a correction (tickets stay below 2^24, where float holds them exactly)
+        const int lg_n1t = 31 - __clz(n1t), lg_n2t = 31 - __clz(n2t);
+        const float inv_per = 1.0f / (float)per;
+        const int la = nvc < a.lookahead ? nvc : a.lookahead, nfull = nvc - la;
         int stops = 0;
         for (int i = 0; stops < NGROUP; ++i) {
             const int g = i & 1, buf = i % NBUF;
             const uint32_t use = (uint32_t)(i / NBUF);
             int type = TILE_NOP, chunk = 0, idx = 0, rd = 0;
+            [[maybe_unused]] const long long pt0 = PROF_T();
+            [[maybe_unused]] long long pt_dep = 0, pt1 = 0, pt2 = 0;
             if (lane == 0) {
-                mbar_wait(empty_bar(buf), (use & 1u) ^ 1u);
-                if (it_open[g]) {
-                    type = TILE_P2; chunk = it_chunk[g]; idx = it_n1[g]; rd = it_rd[g];
+                // The tile is chosen (ticket decoded, a pass-2 item's dependency on its chunk's pass-1 counter waited
+                // for) BEFORE the wait for the buffer: that latency then overlaps the consumers' work on the buffer.
+                const bool my_open = g ? open1 : open0, other_open = g ? open0 : open1;
+                if (my_open) {
+                    type = TILE_P2; chunk = g ? oc1 : oc0; idx = g ? on1 : on0; rd = g ? or1 : or0;
                 } else if (next_ticket < total) {
                     const int t = next_ticket;
                     next_ticket = (int)atomicAdd(a.sched, 1u);
                     // queue order, pass 1 running LA chunks ahead of pass 2:
                     //   P1(0) .. P1(LA-1) | P1(LA) P2(0) | P1(LA+1) P2(1) | ... | P2(n-LA) | ... | P2(n-1)
-                    const int LA = a.lookahead;
-                    const int la = nvc < LA ? nvc : LA, nfull = nvc - la;
                     bool first = true;
-                    if (t < la * n1t) {
-                        chunk = t / n1t; idx = t - chunk * n1t;
+                    if (t < (la << lg_n1t)) {
+                        chunk = t >> lg_n1t; idx = t & (n1t - 1);
                     } else {
-                        const int u = t - la * n1t;
+                        const int u = t - (la << lg_n1t);
                         if (u < nfull * per) {
-                            const int blk = u / per, v = u - blk * per;
+                            int blk = (int)((float)u * inv_per);
+                            if (blk * per > u) --blk;
+                            else if ((blk + 1) * per <= u) ++blk;
+                            const int v = u - blk * per;
                             if (v < n1t) { chunk = blk + la; idx = v; }
                             else { first = false; chunk = blk; idx = v - n1t; }
                         } else {
                             const int u2 = u - nfull * per;
-                            first = false; chunk = nfull + u2 / n2t; idx = u2 % n2t;
+                            first = false; chunk = nfull + (u2 >> lg_n2t); idx = u2 & (n2t - 1);
                         }
                     }
                     if (first) {
                         type = TILE_P1;
                     } else {
                         type = TILE_P2; idx *= span; rd = 0;
+                        [[maybe_unused]] const long long d0 = PROF_T();
                         wait_counter(a.sched + kSchedBase + chunk, (unsigned)n1t);   // all of the chunk's Y is in L2
+                        pt_dep = PROF_T() - d0;
                     }
-                } else if (!it_open[g ^ 1]) {
+                } else if (!other_open) {
                     type = TILE_STOP;
                 }
-            }
-            type = __shfl_sync(0xffffffffu, type, 0);
-            chunk = __shfl_sync(0xffffffffu, chunk, 0);
-            idx = __shfl_sync(0xffffffffu, idx, 0);
-            rd = __shfl_sync(0xffffffffu, rd, 0);
-            const uint32_t dst = smem_u32(buf_ptr(buf));
-            if (lane == 0) {
-                meta[buf].x = type; meta[buf].y = chunk; meta[buf].z = idx; meta[buf].w = rd;
-            }
-            if (type == TILE_P1) {
-                constexpr uint32_t basis_bytes = (uint32_t)H * K1::RB * 8, strain_bytes = (uint32_t)K1::SUB * H * 8;
-                if (lane == 0) mbar_expect_tx(full_bar(buf, g), basis_bytes + strain_bytes);
-                __syncwarp();
-                const int bc = chunk / a.nb, bs = chunk - bc * a.nb;
+                // Everything the copies need is worked out, and the tile's descriptor published (the meta ring has
+                // 2 NBUF slots, so the slot of the tile still being processed in this buffer is not touched), BEFORE the
+                // wait for the buffer: once the consumers release it only expect_tx + the copies remain on the path.
+                const int ms = i % (2 * NBUF);
+                meta[ms].x = type; meta[ms].y = chunk; meta[ms].z = idx; meta[ms].w = rd;
+                const uint32_t dst = smem_u32(buf_ptr(buf));
+                const int bc = chunk / a.nb, bs = chunk - bc * a.nb;   // virtual chunk = c * nb + b
+                // both parts of a pass-1 tile sit in global memory in tile-buffer order (rbmf_internal.h): one bulk copy each
+                constexpr uint32_t basis_bytes = (uint32_t)fft_p1_rows(LOG1) * K1::RB * 8;
+                constexpr uint32_t strain_bytes = (uint32_t)K1::SUB * fft_strain_row(LOG1) * 8;
+                static_assert(fft_p1_rows(LOG1) == (K1::PAD ? H + H / 32 : H) && fft_strain_row(LOG1) == H + K1::SPAD, "tile layout");
+                static_assert(basis_bytes % 16 == 0 && strain_bytes % 16 == 0, "bulk copies move multiples of 16 bytes");
+                const float2* src_basis = a.basisP + ((size_t)bc * n1t + idx) * (size_t)(fft_p1_rows(LOG1) * K1::RB);
+                const float2* src_strain = a.dsT + ((size_t)bs * L2 + (size_t)idx * K1::SUB) * fft_strain_row(LOG1);
                 // a basis chunk is streamed from HBM once per call: later segments of a batch find it in L2
-                const unsigned long long pol_basis = bs == a.nb - 1 ? pol_first : pol_last;
-                const float2* src = a.basisP + ((size_t)bc * n1t + idx) * (size_t)(H * K1::RB);
-                if (K1::PAD) {
-                    for (int p = lane; p < H / 32; p += 32)
-                        bulk_g2s(dst + (uint32_t)(33 * p) * K1::RB * 8, src + (size_t)p * 32 * K1::RB, 32 * K1::RB * 8,
-                                 full_bar(buf, g), pol_basis);
-                } else if (lane == 0) {
-                    bulk_g2s(dst, src, basis_bytes, full_bar(buf, g), pol_basis);
+                const unsigned long long pol_basis = bs == a.nb - 1 ? pol_first : pol_normal;
+                constexpr int BR = L2 < 256 ? L2 : 256;          // rows per tensor copy of a pass-2 tile
+                const int x = (idx + rd * K2::SUB) * C * 2;      // floats along the (n1, col) axis
+                const int zc = bs * a.nchunk + bc;               // the chunk's block of the beta array
+                const uint32_t fb = full_bar(buf, g);
+                pt1 = PROF_T();
+                mbar_wait(empty_bar(buf), (use & 1u) ^ 1u);
+                pt2 = PROF_T();
+                if (type == TILE_P1) {
+                    mbar_expect_tx(fb, basis_bytes + strain_bytes);
+                    bulk_g2s(dst, src_basis, basis_bytes, fb, pol_basis);
+                    bulk_g2s(dst + basis_bytes, src_strain, strain_bytes, fb, pol_last);
+                } else if (type == TILE_P2) {
+                    mbar_expect_tx(fb, (uint32_t)L2 * K2::RB * 8);
+#pragma unroll
+                    for (int p = 0; p < L2 / BR; ++p)
+                        tma_load_3d(dst + (uint32_t)K2::idx(p * BR) * K2::RB * 8, &tmY, fb, x, p * BR, zc);
+                    const bool more = rd + 1 < rounds;
+                    if (g) { open1 = more; oc1 = chunk; on1 = idx; or1 = rd + 1; }
+                    else { open0 = more; oc0 = chunk; on0 = idx; or0 = rd + 1; }
+                } else {
+                    mbar_arrive(fb);
                 }
-                if (lane >= 32 - K1::SUB) {   // one copy per line (padded rows, see Cfg::SPAD)
-                    const int l = 31 - lane;
-                    bulk_g2s(dst + (uint32_t)(K1::idx(H) * K1::RB + l * (H + K1::SPAD)) * 8,
-                             a.dsT + (size_t)bs * ((size_t)H * L2) + ((size_t)idx * K1::SUB + l) * H, (uint32_t)H * 8,
-                             full_bar(buf, g), pol_last);
-                }
-            } else if (type == TILE_P2) {
-                constexpr int BR = L2 < 256 ? L2 : 256;   // rows per tensor copy
-                if (lane == 0) mbar_expect_tx(full_bar(buf, g), (uint32_t)L2 * K2::RB * 8);
-                __syncwarp();
-                const int x = (idx + rd * K2::SUB) * C * 2;   // floats along the (n1, col) axis
-                for (int p = lane; p < L2 / BR; p += 32)
-                    tma_load_3d(dst + (uint32_t)K2::idx(p * BR) * K2::RB * 8, &tmY, full_bar(buf, g), x, p * BR,
-                                (chunk % a.nb) * a.nchunk + chunk / a.nb);
-                if (rd + 1 < rounds) { it_open[g] = true; it_chunk[g] = chunk; it_n1[g] = idx; it_rd[g] = rd + 1; }
-                else it_open[g] = false;
-            } else {
-                if (lane == 0) mbar_arrive(full_bar(buf, g));
-                if (type == TILE_STOP) ++stops;
             }
+            if (__shfl_sync(0xffffffffu, type, 0) == TILE_STOP) ++stops;
             __syncwarp();
+            if (lane == 0) {
+                PROF_ADD(0, 1); PROF_ADD(1, pt1 - pt0 - pt_dep); PROF_ADD(2, pt_dep); PROF_ADD(3, pt2 - pt1);
+                PROF_ADD(4, PROF_T() - pt2);
+            }
         }
     } else {
         // =========================================== consumers ==========================================
@@ -599,8 +628,11 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
         for (int it = 0; it < NIT; ++it) acc[it] = make_float2(0.f, 0.f);
         for (int i = g;; i += NGROUP) {
             const int buf = i % NBUF;
+            [[maybe_unused]] const long long ct0 = PROF_T();
             mbar_wait(full_bar(buf, g), (uint32_t)(i / (NBUF * NGROUP)) & 1u);
-            const int type = meta[buf].x, chunk = meta[buf].y, idx = meta[buf].z, rd = meta[buf].w;
+            [[maybe_unused]] const long long ct1 = PROF_T();
+            const int ms = i % (2 * NBUF);
+            const int type = meta[ms].x, chunk = meta[ms].y, idx = meta[ms].z, rd = meta[ms].w;
             if (type == TILE_STOP) break;
             float2* B = buf_ptr(buf);
             if (type == TILE_P1) p1_tile<LOG1, LOG2>(a, g, gt, chunk, idx, B, tw_a, e2s_all + g * kE2Stride);
@@ -608,6 +640,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
             fence_async_smem();   // this thread's generic-proxy writes to the buffer, before the async proxy refills it
             group_sync(g);
             if (gt == 0) {
+                PROF_ADD(8 + 4 * type, 1); PROF_ADD(9 + 4 * type, ct1 - ct0); PROF_ADD(10 + 4 * type, PROF_T() - ct1);
                 mbar_arrive(empty_bar(buf));
                 if (type == TILE_P1) {
                     // release: the group's Y stores happen before this fence through the barrier above (bar.sync
@@ -652,6 +685,18 @@ cudaError_t launch_one(const CUtensorMap& tmY, const FftArgs& a, int grid, cudaS
         case 10 * 16 + 10: return FN<10, 10>(__VA_ARGS__);           \
         default: return cudaErrorInvalidValue;                       \
     }
+
+#ifdef RBMF_FFT_PROFILE
+extern "C" int rbmf_fft_profile_read(unsigned long long* out32, int reset) {
+    cudaDeviceSynchronize();
+    if (cudaMemcpyFromSymbol(out32, g_fft_prof, sizeof(g_fft_prof)) != cudaSuccess) return -1;
+    if (reset) {
+        unsigned long long z[32] = {};
+        if (cudaMemcpyToSymbol(g_fft_prof, z, sizeof(z)) != cudaSuccess) return -1;
+    }
+    return 0;
+}
+#endif
 
 cudaError_t fft_tma_configure(int logL1, int logL2, size_t* smem_bytes) {
     RBMF_FFT_DISPATCH(configure_one, smem_bytes)

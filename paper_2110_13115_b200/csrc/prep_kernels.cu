@@ -69,8 +69,8 @@ __global__ void layout_basis_kernel(const float2* __restrict__ basis, float2* __
         for (int e = tx; e < 32 * kFftC; e += 32) {
             const int j1 = j1_0 + e / kFftC, c = e % kFftC;
             if (j1 < H)
-                basisP[((((size_t)chunk * (L2 / sub) + j2 / sub) * H + j1) * sub + j2 % sub) * kFftC + c] =
-                    tile[c][e / kFftC][r];
+                basisP[((((size_t)chunk * (L2 / sub) + j2 / sub) * fft_p1_rows(logL1) + fft_p1_row(logL1, j1)) * sub +
+                        j2 % sub) * kFftC + c] = tile[c][e / kFftC][r];
         }
     }
 }
@@ -222,7 +222,8 @@ __global__ void prep_strain_kernel(const float2* __restrict__ strain, float2* __
     const int j = blockIdx.x * blockDim.x + threadIdx.x;   // j = j1 L2 + j2 < N/2
     if (j >= H * L2) return;
     const float2 d = strain[(size_t)blockIdx.y * ((size_t)H * L2 + 1) + j];
-    dsT[(size_t)blockIdx.y * ((size_t)H * L2) + (size_t)(j % L2) * H + j / L2] = make_float2(d.x * scale, d.y * scale);
+    const size_t row = (size_t)fft_strain_row(logL1);
+    dsT[((size_t)blockIdx.y * L2 + (size_t)(j % L2)) * row + j / L2] = make_float2(d.x * scale, d.y * scale);
 }
 
 cudaError_t launch_prep_strain(const float2* strain, float2* dsT, int logL1, int logL2, float scale, int nb,

@@ -82,7 +82,8 @@ Layout make_layout(const rbmf_plan* p) {
     const size_t M = (size_t)p->M * B;   // rows of the planes: all segments of a batch, segment-major
     const size_t nkb = (k + 31) / 32;
     L.plane_bytes = nkb * M * 64 * 2;
-    L.basisP = take((size_t)p->n_half * k * 8);
+    // pass-1 tile inputs in tile-buffer order (rbmf_internal.h): k L2 fft_p1_rows(L1) basis values, L2 strain rows
+    L.basisP = take(k * ((size_t)1 << p->logN2) * (size_t)fft_p1_rows(p->logN1) * 8);
     L.beta = take(B * N * k * 8);
     L.bavg_hi = take(L.plane_bytes);
     L.bavg_lo = take(L.plane_bytes);
@@ -95,7 +96,7 @@ Layout make_layout(const rbmf_plan* p) {
     L.tw1_a = take(((size_t)1 << p->logN1) * 8);
     L.tw1_b = take(((size_t)1 << p->logN2) * 8);
     L.twN = take(((size_t)1 << p->logN2) * (size_t)(fft_r0(p->logN1) + fft_r1(p->logN1)) * 8);   // two factor tables
-    L.dsT = take(B * (size_t)p->n_half * 8);
+    L.dsT = take(B * ((size_t)1 << p->logN2) * (size_t)fft_strain_row(p->logN1) * 8);
     L.cand = take((size_t)p->max_cand * sizeof(rbmf_candidate));
     L.cand2 = take((size_t)p->max_cand * sizeof(rbmf_candidate));
     L.cand3 = take((size_t)p->max_cand * sizeof(rbmf_candidate));
@@ -120,12 +121,12 @@ Layout make_layout(const rbmf_plan* p) {
             U.N = u == 0 ? p->N : 2 * p->N / p->w;
             const int n = ilog2(U.N);
             U.logN1 = (n + 1) / 2; U.logN2 = n / 2; U.ncols = p->tm_slab;
-            U.basisP = take((size_t)(U.N / 2) * U.ncols * 8);
+            U.basisP = take((size_t)U.ncols * ((size_t)1 << U.logN2) * (size_t)fft_p1_rows(U.logN1) * 8);
             U.beta = take((size_t)U.N * U.ncols * 8);
             U.tw1_a = take(((size_t)1 << U.logN1) * 8);
             U.tw1_b = take(((size_t)1 << U.logN2) * 8);
             U.twN = take(((size_t)1 << U.logN2) * (size_t)(fft_r0(U.logN1) + fft_r1(U.logN1)) * 8);
-            U.dsT = take((size_t)(U.N / 2) * 8);
+            U.dsT = take(((size_t)1 << U.logN2) * (size_t)fft_strain_row(U.logN1) * 8);
             U.sched = take(((size_t)kSchedBase + kMaxChunks) * 4);
         }
     }
@@ -383,7 +384,7 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
         }
         // S(f) of Eq. 11; the fast first stage feeds its folded spectrum to kernel 1 with a unit "strain"
         CK(launch_tm_tables(at<float2>(plan, L.tm_S), at<float2>(plan, plan->tmS.dsT), plan->N, plan->w,
-                            plan->tmS.N / 2, plan->stream));
+                            ((long long)1 << plan->tmS.logN2) * fft_strain_row(plan->tmS.logN1), plan->stream));
     }
     plan->have_templates = false;
     const uint64_t Mplane = (uint64_t)plan->M * (uint64_t)plan->max_batch;
@@ -482,6 +483,7 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
         const long long cap = (48ll << 20) / ((long long)plan->N * kFftC * 8) - 1;
         if (la > cap) la = cap;
         if (la < 1) la = 1;
+        if (const char* e = getenv("RBMF_FFT_LOOKAHEAD")) { const int v = atoi(e); if (v >= 1) la = v; }   // developer switch
         a.lookahead = (int)la;
     }
     CK(launch_fft_tma(plan->tmY, a, plan->logN1, plan->logN2, plan->fft_grid, st));

@@ -23,6 +23,20 @@ __host__ __device__ constexpr int fft_r1(int logL) { return (1 << logL) / fft_r0
 // lines (independent transforms) a 256-thread consumer group works on in lockstep = lines per tile
 __host__ __device__ constexpr int fft_sub(int logL) { return kFftThreads / (fft_r1(logL) * kFftC); }
 
+// Input of a pass-1 tile (sub lines j2 of one chunk), laid out in global memory exactly as it sits in the tile buffer, so
+// that the producer moves it with TWO bulk copies (a bulk copy costs the producer warp ~150 cycles to issue; sixteen
+// 2 KB pieces into padded rows made the producer, not the consumers, the kernel's bottleneck):
+//   basis part  [row(j1)][line][C], j1 < L1/2, with one pad row after every 32 rows when a row is 64 bytes
+//               (L1 = 1024: keeps stage 1's shared-memory reads conflict-free, see fft_tma.cu);
+//   strain part [line][L1/2 + spad] entries (lines offset so that the lines a warp reads fall into different banks).
+__host__ __device__ constexpr bool fft_p1_pad(int logL) { return fft_sub(logL) * kFftC * 8 == 64; }
+__host__ __device__ constexpr int fft_p1_rows(int logL) {
+    return fft_p1_pad(logL) ? (1 << logL) / 2 + (1 << logL) / 64 : (1 << logL) / 2;
+}
+__host__ __device__ constexpr int fft_p1_row(int logL, int j1) { return fft_p1_pad(logL) ? j1 + (j1 >> 5) : j1; }
+__host__ __device__ constexpr int fft_spad(int logL) { return 16 / fft_sub(logL) > 2 ? 16 / fft_sub(logL) : 2; }
+__host__ __device__ constexpr int fft_strain_row(int logL) { return (1 << logL) / 2 + fft_spad(logL); }
+
 // Scheduler words (uint32) in the workspace: [0] ticket, [16 + v] pass-1 tiles done of virtual chunk v = c * nb + b
 // (c = chunk of 4 basis columns, b = segment of the batch): 16 + kMaxChunks * max_batch words.
 constexpr int kSchedBase = 16;
@@ -34,8 +48,8 @@ constexpr int kStage2Chunk = 128;   // candidates per stage-2 work item (one CTA
 
 // Device views handed to the fused FFT kernel.
 struct FftArgs {
-    const float2* basisP;    // [chunk][tile][j1 < L1/2][line][C], j2 = tile * sub + line: conj NOT applied, zero outside the band
-    const float2* dsT;       // [j2 < L2][j1 < L1/2]: s * d[j1 L2 + j2]
+    const float2* basisP;    // [chunk][tile][fft_p1_row(j1)][line][C], j2 = tile * sub + line: conj NOT applied, zero outside the band
+    const float2* dsT;       // [segment][j2 < L2][fft_strain_row]: s * d[j1 L2 + j2] at entry j1 < L1/2
     const float2* tw1_a;     // pass 1 stage-1 twiddles  [q < R1][b < R0] = e^{2 pi i q b / L1}
     const float2* tw1_b;     // pass 2 stage-1 twiddles, same for L2
     const float2* twN;       // inter-pass twiddles as two factor tables, [j2][b < R0] then [j2][m < R1] (prep_kernels.cu)

@@ -91,8 +91,8 @@ __global__ void tm_fold_kernel(const float2* __restrict__ templates, const float
         for (int e = tx; e < 32 * kFftC; e += 32) {
             const int j1 = j1_0 + e / kFftC, c = e % kFftC;
             if (j1 < H)
-                out[((((size_t)chunk * (L2 / sub) + j2 / sub) * H + j1) * sub + j2 % sub) * kFftC + c] =
-                    tile[c][e / kFftC][r];
+                out[((((size_t)chunk * (L2 / sub) + j2 / sub) * fft_p1_rows(logL1) + fft_p1_row(logL1, j1)) * sub +
+                     j2 % sub) * kFftC + c] = tile[c][e / kFftC][r];
         }
     }
 }
