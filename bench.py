@@ -33,7 +33,7 @@ import numpy as np  # noqa: E402
 METRIC = "template_seconds_filtered_per_second"
 UNIT = "template-seconds/s"
 
-KERNEL_OF = {"fft": "fft_tma_kernel", "gemm": "gemm_", "stage2": "stage2"}
+KERNEL_OF = {"fft": "fft_tma_kernel", "gemm": "gemm_", "stage2": "stage2_score"}
 
 
 def ncu_traffic(config, w, mode):
