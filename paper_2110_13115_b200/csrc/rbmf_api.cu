@@ -446,8 +446,8 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
                               float thr_stage2, rbmf_trigger* out_dev, int64_t* n_out_dev) {
     if (!plan || !strain_dev || !out_dev || !n_out_dev) return RBMF_ERR_ARG;
     if (!(thr_stage1 > 0.f) || !(thr_stage2 > 0.f)) return RBMF_ERR_ARG;
-    if (!plan->have_ws || !plan->have_basis || !plan->have_coeffs) return RBMF_ERR_STATE;
     if (n_segments < 1 || n_segments > plan->max_batch) return RBMF_ERR_ARG;
+    if (!plan->have_ws || !plan->have_basis || !plan->have_coeffs) return RBMF_ERR_STATE;
     const Layout& L = plan->lay;
     cudaStream_t st = plan->stream;
     const bool tm = plan->timing != 0;

@@ -146,3 +146,33 @@ def test_product_path_does_not_import_the_oracle():
         if f.endswith(".py"):
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2110_13115_b200" not in text and "from paper_2110_13115_b200" not in text, f
+
+
+def test_new_entry_points_validate_arguments_without_a_gpu(binding):
+    """rbmf_filter_batch / rbmf_prepare_strain / template routes / bank sets: argument and call-order errors are
+    reported before any CUDA call."""
+    b = binding
+    st, h = _create(b)
+    dummy = ctypes.c_void_p(1024)
+    assert b.rbmf_filter_batch(h, dummy, 0, 5.0, 6.0, dummy, dummy) == b.RBMF_ERR_ARG          # thresholds / state first
+    assert b.rbmf_filter_batch(h, dummy, 1, 5.0, 6.0, dummy, dummy) == b.RBMF_ERR_STATE
+    assert b.rbmf_filter_batch_host(h, dummy, 1, 5.0, 6.0, dummy, 10, ctypes.byref(ctypes.c_int64())) == b.RBMF_ERR_STATE
+    assert b.rbmf_prepare_strain(h, dummy, None, 1, dummy) == b.RBMF_ERR_STATE
+    assert b.rbmf_prepare_strain(h, None, None, 1, dummy) == b.RBMF_ERR_ARG
+    assert b.rbmf_plan_enable_template_routes(h, 1028) == b.RBMF_ERR_ARG
+    assert b.rbmf_plan_set_window(h, 4) == b.RBMF_OK
+    assert b.rbmf_plan_enable_template_routes(h, 0) == b.RBMF_OK
+    before, after = ctypes.c_size_t(), ctypes.c_size_t()
+    assert b.rbmf_workspace_bytes(h, ctypes.byref(before)) == b.RBMF_OK
+    assert b.rbmf_plan_enable_template_routes(h, 64) == b.RBMF_OK
+    assert b.rbmf_workspace_bytes(h, ctypes.byref(after)) == b.RBMF_OK and after.value > before.value
+    # bank sets: NULL / empty / plans that are not set up
+    bs = ctypes.c_void_p()
+    arr = (ctypes.c_void_p * 1)(h)
+    assert b.rbmf_bankset_create(None, arr, 1) == b.RBMF_ERR_ARG
+    assert b.rbmf_bankset_create(ctypes.byref(bs), arr, 0) == b.RBMF_ERR_ARG and not bs.value
+    assert b.rbmf_bankset_create(ctypes.byref(bs), arr, 1) == b.RBMF_ERR_STATE and not bs.value
+    assert b.rbmf_bankset_filter(None, dummy, 5.0, 6.0, dummy, 10, dummy, None) == b.RBMF_ERR_ARG
+    assert b.rbmf_bankset_get_counts(None, None, None, None) == b.RBMF_ERR_ARG
+    assert b.rbmf_bankset_destroy(None) == b.RBMF_ERR_ARG
+    b.rbmf_plan_destroy(h)

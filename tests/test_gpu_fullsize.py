@@ -277,3 +277,87 @@ def test_paper_scale_exhaustive_fp64_crosscheck_not_the_oracle(rbmf):
     assert rep["ok"] and rep["n_mandatory"] > 100000, rep
     assert crep["ok"] and crep["n_mandatory"] > 50000, crep
     _WL.clear()
+
+
+# --------------------------------------------------------------------------------- 8(f) rows at Paper scale
+def test_paper_scale_batch_of_two_equals_two_calls_and_oracle_on_segment_one(rbmf):
+    """rbmf_filter_batch at BASELINE configs[2] sizes: the batch's lists, cut per segment, are exactly the lists of
+    single-segment calls (same kernels, the segments' bins are 128-aligned blocks of the GEMM's M dimension), and
+    segment 1 -- a strain no single-segment test sees -- passes the oracle comparison on a template sample."""
+    import torch
+    wl = workload("paper")
+    cfg = wl["config"]
+    strains = np.stack([wlm.make_strain(wl, s)[0] for s in range(2)])
+    torch.cuda.empty_cache()
+    plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, max_candidates=1 << 22, max_triggers=1 << 22,
+                     max_batch=2)
+    plan.set_basis(torch.from_numpy(wl["basis"]))
+    plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+    sd = torch.from_numpy(strains).cuda()
+    plan.filter_batch_async(sd, cfg.thr1, cfg.thr2)
+    both = plan.triggers()
+    cands = plan.candidates()
+    singles = []
+    for s in range(2):
+        plan.filter_async(sd[s], cfg.thr1, cfg.thr2)
+        singles.append((plan.triggers(), plan.candidates()))
+    plan.close()
+    for s in range(2):
+        seg = both[(both["time"] >= s * cfg.N) & (both["time"] < (s + 1) * cfg.N)].copy()
+        seg["time"] -= s * cfg.N
+        assert len(seg) > 1000 and np.array_equal(seg, singles[s][0])
+        cseg = cands[(cands["bin"] >= s * (cfg.N // cfg.w)) & (cands["bin"] < (s + 1) * (cfg.N // cfg.w))].copy()
+        cseg["bin"] -= s * (cfg.N // cfg.w)
+        assert np.array_equal(cseg, singles[s][1])
+    subset = np.unique(singles[1][0]["template"])[:: max(1, len(np.unique(singles[1][0]["template"])) // 48)]
+    subset = np.union1d(subset, np.random.default_rng(3).choice(cfg.T, 64, replace=False))
+    ref = orc.oracle_filter(strains[1], wl["basis"].astype(np.complex128), wl["coeffs"].astype(np.complex128), wl["sigma"],
+                            cfg.N, cfg.fs, cfg.f_low, cfg.w, cfg.thr1, cfg.thr2, templates=subset)
+    got = singles[1][0]
+    rep = compare.compare_triggers(got[np.isin(got["template"], subset)], ref, cfg.N, cfg.thr1, cfg.thr2)
+    assert rep["ok"] and rep["n_mandatory"] > 100, rep
+
+
+def test_paper_scale_template_routes_sampled(rbmf):
+    """The paper's template routes at BASELINE configs[2] sizes (T = 20000 reconstructed templates = 42 GB, slab 256):
+    the first stage by templates (Eq. 10-12) gives the basis route's candidates and triggers; the flat template method's
+    triggers match the oracle's Eq. 4 series on a template sample."""
+    import torch
+    wl = workload("paper")
+    cfg = wl["config"]
+    torch.cuda.empty_cache()
+    c = torch.from_numpy(wl["coeffs"]).cuda()
+    b = torch.from_numpy(wl["basis"]).cuda()
+    tpl = torch.empty((cfg.T, cfg.bins), dtype=torch.complex64, device="cuda")
+    for a in range(0, cfg.T, 2048):
+        tpl[a:a + 2048] = c[a:a + 2048] @ b                   # input synthesis: h'_t = sum_k c_tk b_k
+    del c, b
+    plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, max_candidates=1 << 22, max_triggers=1 << 22,
+                     template_slab=256)
+    plan.set_basis(torch.from_numpy(wl["basis"]))
+    plan.set_coeffs(torch.from_numpy(wl["coeffs"]), torch.from_numpy(wl["sigma"]))
+    plan.set_templates(tpl, torch.from_numpy(wl["sigma"]))
+    sd = torch.from_numpy(wl["strain"]).cuda()
+    plan.filter_async(sd, cfg.thr1, cfg.thr2)
+    base_t, base_c = plan.triggers(), plan.candidates()
+    plan.set_stage1_route(rbmf.RBMF_STAGE1_TEMPLATES)
+    plan.filter_async(sd, cfg.thr1, cfg.thr2)
+    tm_t, tm_c = plan.triggers(), plan.candidates()
+    key = lambda r, f, n: r["template"].astype(np.int64) * n + r[f]
+    # the two routes may differ only at threshold ties (fp32 rounding of different summation orders)
+    assert len(np.setxor1d(key(base_c, "bin", cfg.N), key(tm_c, "bin", cfg.N))) <= max(8, len(base_c) // 2000)
+    assert len(np.setxor1d(key(base_t, "time", cfg.N), key(tm_t, "time", cfg.N))) <= max(8, len(base_t) // 2000)
+    common = np.intersect1d(key(base_c, "bin", cfg.N), key(tm_c, "bin", cfg.N), return_indices=True)
+    assert np.abs(base_c["re"][common[1]] - tm_c["re"][common[2]]).max() < 2e-4     # averaged SNR values agree
+    flat = plan.filter_flat(sd, cfg.thr2)
+    subset = np.unique(flat["template"])[:: max(1, len(np.unique(flat["template"])) // 24)][:32]
+    ref = orc.template_method_triggers(wl["strain"], tpl[torch.from_numpy(subset).cuda()].cpu().numpy(), wl["sigma"][subset],
+                                       cfg.N, cfg.fs, cfg.f_low, cfg.thr2)
+    for k_ in ("triggers", "near"):
+        ref[k_]["template"] = subset[ref[k_]["template"]]
+    frep = compare.compare_triggers(flat[np.isin(flat["template"], subset)], ref, cfg.N, 1.0, cfg.thr2)
+    plan.close()
+    del tpl
+    torch.cuda.empty_cache()
+    assert frep["ok"] and frep["n_mandatory"] > 100, frep
+    assert len(flat) >= len(base_t)                              # the hierarchical set is a subset of the flat one
