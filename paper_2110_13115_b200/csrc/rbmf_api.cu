@@ -505,7 +505,16 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     g.T = plan->T; g.M = (int)Mtot; g.k2 = 2 * plan->k;
     g.num_tb = plan->Tpad / kGemmTT;
     g.num_ib = (int)(Mtot / kGemmBM);
-    g.group = 32;   // template blocks per raster group: 32 coefficient tiles (8 MB fp16) stay L2-resident
+    {
+        // template blocks per raster group: the group's coefficient tiles (256 rows x 2k values, one fp16 plane or bf16
+        // hi + lo) stay L2-resident -- up to 48 MB of them -- while the beta^avg planes stream past once per group
+        // (measured, Paper config: 32 blocks 2.05 ms, 64 blocks 2.03 ms, all 157 blocks 2.02 ms and a third of the
+        // DRAM traffic)
+        const size_t tile_bytes = (size_t)2 * kGemmTT * g.k2 * 2 * (screen ? 1 : 2);
+        long long grp = (long long)((size_t)(48u << 20) / tile_bytes);
+        g.group = (int)(grp < 8 ? 8 : (grp > g.num_tb ? g.num_tb : grp));
+    }
+    if (const char* e = getenv("RBMF_GEMM_GROUP")) { const int v = atoi(e); if (v >= 1) g.group = v; }   // developer switch
     if (by_templates) {
         // the paper's fast first stage by templates (Eq. 10-12) in the place of the GEMM; exact fp32 candidates
         rbmf_status s1 = stage1_by_templates(plan, (const float2*)strain_dev, thr_stage1);
