@@ -109,3 +109,38 @@ def tune(rbmf, N, fs, f_low, basis, coeffs, sigma, strains, ws=(2, 4, 8, 16), th
                                 "ms_per_segment": ms, "ms_over_flat_search": ms / flat_ms})
         plan.close()
     return out
+
+
+def main(argv=None):
+    """python -m paper_2110_13115_b200.tuning [--config small] [--segments 8] [--ws 2,4,8,16] [--thr1 3.0,3.5,...]
+    Runs the study on noise-only segments of a synthetic config (paper_2110_13115_b200.workloads) and prints one JSON
+    document (the rows of Fig. 5-7: f(w, rho_I), rho_target, Eq. 15 / Eq. 13, measured ms)."""
+    import argparse
+    import json
+
+    import torch
+
+    from . import rbmf, workloads
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", default="small")
+    ap.add_argument("--segments", type=int, default=8)
+    ap.add_argument("--ws", default="2,4,8,16")
+    ap.add_argument("--thr1", default="3.0,3.5,4.0,4.5,5.0,5.5")
+    ap.add_argument("--ratio", type=float, default=0.99)
+    args = ap.parse_args(argv)
+    cfg = workloads.CONFIGS[args.config].replace(n_inj=0)          # Gaussian noise only, as PAPER.md:296
+    wl = workloads.make_workload(cfg, device="cuda" if torch.cuda.is_available() else "cpu")
+    strains = np.stack([workloads.make_strain(wl, s)[0] for s in range(args.segments)])
+    thr1 = [float(x) for x in args.thr1.split(",")]
+    res = tune(rbmf, cfg.N, cfg.fs, cfg.f_low, wl["basis"], wl["coeffs"], wl["sigma"], strains,
+               ws=[int(x) for x in args.ws.split(",")], thr1_grid=thr1,
+               rho2_grid=np.round(np.arange(min(thr1), 7.0001, 0.1), 6), ratio=args.ratio)
+    res["config"] = "%s (noise only): N=%d fs=%g k=%d T=%d, %d segments" % (cfg.name, cfg.N, cfg.fs, cfg.k, cfg.T,
+                                                                          args.segments)
+    print(json.dumps(res))
+    return 0
+
+
+if __name__ == "__main__":
+    import sys
+    sys.exit(main())

@@ -37,3 +37,28 @@ def test_extra_segments_share_the_bank():
     # noise normalisation: |d[j]|^2 averages N for unit-variance white noise
     cfg = wl["config"]
     assert abs((np.abs(s1[10:-10]) ** 2).mean() / cfg.N - 1.0) < 0.15
+
+
+def test_sweep_grid_and_further_segments_and_time_series():
+    """BASELINE.json configs[4] as a grid; segments beyond 0 are fresh draws; the coloured time series whitens back to
+    the frequency-domain strain; sub-banks carry their own (k, T, w)."""
+    import numpy as np
+    from paper_2110_13115_b200 import workloads as wlm
+    assert len(wlm.SWEEP_NAMES) == 15
+    for name in wlm.SWEEP_NAMES:
+        c = wlm.CONFIGS[name]
+        assert c.N == 1 << 20 and c.n_inj == 0 and c.k in wlm.SWEEP_K and c.T in wlm.SWEEP_T
+    assert len({wlm.CONFIGS[n].seed for n in wlm.CONFIGS}) == len(wlm.CONFIGS)      # one seed per config
+    wl = wlm.make_workload(wlm.CONFIGS["tiny"])
+    cfg = wl["config"]
+    s0, inj0 = wlm.make_strain(wl, 0)
+    s1, inj1 = wlm.make_strain(wl, 1)
+    s1b, _ = wlm.make_strain(wl, 1)
+    assert s0 is wl["strain"] and np.array_equal(s1, s1b) and not np.array_equal(s0, s1) and len(inj1) == cfg.n_inj
+    x, inv_asd = wlm.make_time_series(wl, 1)
+    assert x.dtype == np.float32 and x.shape == (cfg.N,) and inv_asd.shape == (cfg.bins,) and (inv_asd > 0).all()
+    back = np.fft.rfft(x.astype(np.float64)) * inv_asd
+    assert np.abs(back - s1)[cfg.j_low:cfg.N // 2].max() < 1e-3          # float32 rounding of x only
+    subs = wlm.make_subbanks(cfg, [(1.0, 1.2, 16, 20, 4), (1.2, 1.5, 32, 12, 2)])
+    assert [w["coeffs"].shape for w in subs] == [(20, 16), (12, 32)] and subs[1]["config"].w == 2
+    assert subs[0]["mc"].max() <= 1.2 < subs[1]["mc"].min()
