@@ -59,6 +59,6 @@ def test_sweep_grid_and_further_segments_and_time_series():
     assert x.dtype == np.float32 and x.shape == (cfg.N,) and inv_asd.shape == (cfg.bins,) and (inv_asd > 0).all()
     back = np.fft.rfft(x.astype(np.float64)) * inv_asd
     assert np.abs(back - s1)[cfg.j_low:cfg.N // 2].max() < 1e-3          # float32 rounding of x only
-    subs = wlm.make_subbanks(cfg, [(1.0, 1.2, 16, 20, 4), (1.2, 1.5, 32, 12, 2)])
-    assert [w["coeffs"].shape for w in subs] == [(20, 16), (12, 32)] and subs[1]["config"].w == 2
+    subs = wlm.make_subbanks(cfg, [(1.0, 1.2, 16, 20, 4), (1.2, 1.5, 8, 12, 2)])
+    assert [w["coeffs"].shape for w in subs] == [(20, 16), (12, 8)] and subs[1]["config"].w == 2
     assert subs[0]["mc"].max() <= 1.2 < subs[1]["mc"].min()
