@@ -36,6 +36,8 @@ Pins (tests/test_oracle_pins.py, all `-m "not gpu"`):
   template routes              flat method: pure-Python enumeration of `snr_series_direct` on the BANK templates, and its
                                count == oracle_filter's n_flat on reconstructed templates; fast first stage: candidates ==
                                oracle_filter's (Eq. 12 route == binned mean, already pinned) incl. the values
+  preparation (PCA)            against numpy's SVD (same subspace projector, same singular values), orthonormality, Eq. 8
+                               with its own singular values, and optimality: no other orthonormal k-set captures more
   tuning, Eq. 16               hand-built lists with the answer worked out by counting; w = 1 recovers everything
   forward transform, whitening literal O(N^2) sum at small N, a cosine's closed form (N/2 at its bin), Parseval; batches:
                                segment b of `oracle_filter_batch` against the time-domain brute force on strain b alone
@@ -352,6 +354,29 @@ def evaluate_points(strain, basis, coeffs, sigma, N, fs, f_low, w, template, tim
         b = n // w
         rbar.append(sum(snr_point(strain, h, sg, N, j_low, b * w + r) for r in range(w)) / w)
     return np.array(rho), np.array(rbar)
+
+
+# ------------------------------------------------------- preparation: PCA of a (sub-)bank
+def pca_basis(templates, k):
+    """The preparation step as the paper describes it (readings R5-R7): templates
+    stored row-wise in T (S x bins, unit norm, no centering), covariance C = T T^H (S x S), EVD, basis vectors
+    p_i = lambda_i^{-1/2} v_i^H T for the k largest eigenvalues, decomposition coefficients D = T P^H.
+    Returns (basis (k, bins) complex128 orthonormal rows, coeffs (S, k), singular values sqrt(lambda) descending (S,))."""
+    Tm = np.asarray(templates, dtype=np.complex128)
+    C = Tm @ Tm.conj().T
+    lam, V = np.linalg.eigh(C)
+    lam, V = lam[::-1], V[:, ::-1]
+    lam = np.clip(lam, 0.0, None)
+    basis = (V[:, :k].conj().T @ Tm) / np.sqrt(lam[:k])[:, None]
+    coeffs = Tm @ basis.conj().T
+    return basis, coeffs, np.sqrt(lam)
+
+
+def captured_power(templates, basis):
+    """mean_t ||c_t||^2 with c = T P^H: the fraction of the bank's power an orthonormal basis captures (the complement
+    of the mean SNR loss of Eq. 8)."""
+    c = np.asarray(templates, dtype=np.complex128) @ np.asarray(basis, dtype=np.complex128).conj().T
+    return float((np.abs(c) ** 2).sum(axis=1).mean())
 
 
 # ------------------------------------------------------- tuning of (w, rho_I), Eq. 16

@@ -478,3 +478,26 @@ def test_rho_target_of_the_flat_search_is_the_lowest_threshold(micro):
     m4 = np.hypot(res4["triggers"]["re"], res4["triggers"]["im"])
     t4, nf, nl = orc.rho_target(m4, mods, grid)
     assert (nf <= nl).all() and (t4 is None or t4 >= 2.0)
+
+
+# ---------------------------------------------------------------- preparation
+def test_pca_basis_against_svd_eq8_and_optimality(tiny):
+    cfg = tiny["config"]
+    U = wlm.bank_templates(tiny, np.arange(cfg.T))                     # unit-norm bank templates, (T, bins)
+    k = 12
+    basis, coeffs, sv = orc.pca_basis(U, k)
+    # orthonormal rows; coefficients are the projections
+    assert np.abs(basis @ basis.conj().T - np.eye(k)).max() < 1e-10
+    assert np.abs(coeffs - U @ basis.conj().T).max() < 1e-12
+    # same singular values and the same subspace as LAPACK's SVD of the template matrix (Eq. 5)
+    _, s_ref, Vh = np.linalg.svd(U, full_matrices=False)
+    assert np.abs(sv[:cfg.T] - s_ref).max() < 1e-8
+    assert np.abs(basis.conj().T @ basis - Vh[:k].conj().T @ Vh[:k]).max() < 1e-8
+    # Eq. 8: mean loss = 1 - sum_{i<k} s_i^2 / sum s_i^2, and sum s_i^2 = T for unit-norm templates
+    cap = orc.captured_power(U, basis)
+    assert abs((1.0 - cap) - orc.truncation_loss(sv, k)) < 1e-10 and abs((sv ** 2).sum() - cfg.T) < 1e-8
+    # optimality (Eckart-Young): a random orthonormal k-set of the bank's span, or the next k vectors, capture less
+    rng = np.random.default_rng(1)
+    Qr, _ = np.linalg.qr(((rng.standard_normal((k, cfg.T)) + 1j * rng.standard_normal((k, cfg.T))) @ U).T)
+    assert orc.captured_power(U, Qr.T) < cap - 1e-3
+    assert orc.captured_power(U, Vh[k:2 * k]) < cap
