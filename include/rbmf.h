@@ -204,6 +204,26 @@ rbmf_status rbmf_bankset_filter(rbmf_bankset* set, const void* strain_dev, float
 rbmf_status rbmf_bankset_get_counts(rbmf_bankset* set, int64_t* n_candidates, int64_t* n_triggers, int64_t* n_total);
 rbmf_status rbmf_bankset_destroy(rbmf_bankset* set);
 
+/* ---- Preparation on the GPU (amortised: once per sub-bank) --------------------------
+ * No plan is needed.  templates_dev: n_templates x (N/2+1) complex64, row-major, the (whitened, unit-norm) templates of
+ * a sub-bank "stored row-wise" (:152); only the band [ceil(f_low N / fs), N/2) is used.
+ * rbmf_prepare_basis: the covariance matrix C = T T^H (n_templates <= 32768), its k leading eigenvectors by
+ * `iterations` steps of block power iteration with re-orthonormalisation from seeded random start vectors (the paper
+ * used Lanczos; any orthonormal basis of the leading subspace serves the path equally), and the basis
+ * P = orth(V^H T): basis_out_dev = k x (N/2+1) complex64 with orthonormal rows over the band and zeros outside -- the
+ * input of rbmf_set_basis.  eig_out_dev (k floats or NULL): estimates of the k leading eigenvalues of C (the squared
+ * singular values of T).  workspace_dev: 16-byte aligned device memory of rbmf_prepare_basis_workspace_bytes.
+ * rbmf_prepare_coeffs: the decomposition coefficients D = T P^H (:167-169), coeffs_out_dev = n_templates x k complex64
+ * (c_tk, unconjugated: the input of rbmf_set_coeffs) and sigma_out_dev (n_templates floats or NULL) = ||c_t||_2.
+ * fp32 arithmetic with fp64 accumulation across blocks of 512 terms; both calls only enqueue on cuda_stream. */
+rbmf_status rbmf_prepare_basis_workspace_bytes(int32_t n_templates, int32_t k, size_t* bytes);
+rbmf_status rbmf_prepare_basis(const void* templates_dev, int32_t n_templates, int64_t N, double fs, double f_low,
+                               int32_t k, int32_t iterations, uint64_t seed, void* workspace_dev, size_t workspace_bytes,
+                               void* basis_out_dev, float* eig_out_dev, void* cuda_stream);
+rbmf_status rbmf_prepare_coeffs(const void* templates_dev, int32_t n_templates, const void* basis_dev, int32_t k,
+                                int64_t N, double fs, double f_low, void* coeffs_out_dev, float* sigma_out_dev,
+                                void* cuda_stream);
+
 /* Counts of the last rbmf_filter (synchronises the stream).  RBMF_ERR_OVERFLOW if a capacity was exceeded
  * (in RBMF_GEMM_SCREEN mode the capacity max_candidates applies to the screened superset, see
  * rbmf_get_screened_count, while *n_candidates reports the candidates confirmed at fp32 accuracy). */

@@ -20,7 +20,7 @@ CSRC = os.path.join(PKG_DIR, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB_PATH = os.path.join(PKG_DIR, "librbmf.so")
 BUILD_DIR = os.path.join(PKG_DIR, "build")
-SOURCES = ["rbmf_api.cu", "prep_kernels.cu", "fft_tma.cu", "gemm_tcgen05.cu", "stage2_kernels.cu", "stage2_bybin.cu", "fft_r2c.cu", "template_route.cu"]
+SOURCES = ["rbmf_api.cu", "prep_kernels.cu", "fft_tma.cu", "gemm_tcgen05.cu", "stage2_kernels.cu", "stage2_bybin.cu", "fft_r2c.cu", "template_route.cu", "prep_basis.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC]
 # developer switches, e.g. RBMF_EXTRA_NVCC_FLAGS=-DRBMF_FFT_PROFILE (cycle accounting of the FFT kernel's hand-offs)

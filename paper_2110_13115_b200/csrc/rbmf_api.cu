@@ -782,6 +782,51 @@ const char* rbmf_status_string(rbmf_status status) {
 
 int32_t rbmf_last_cuda_error(const rbmf_plan* plan) { return plan ? plan->last_cuda : 0; }
 
+// ---- preparation on the GPU ---------------------------------------------------
+namespace {
+bool prep_args_ok(int64_t N, double fs, double f_low, int* j_low, int64_t* n_half) {
+    if (N < 64 || (N & (N - 1)) != 0 || N > (int64_t(1) << 24)) return false;
+    if (!(fs > 0.0) || !(f_low > 0.0) || !(f_low < fs / 2)) return false;
+    *n_half = N / 2;
+    *j_low = (int)ceil(f_low * (double)N / fs - 1e-12);
+    return *j_low < *n_half;
+}
+}  // namespace
+
+rbmf_status rbmf_prepare_basis_workspace_bytes(int32_t n_templates, int32_t k, size_t* bytes) {
+    if (!bytes || n_templates < 1 || k < 1 || k > n_templates || n_templates > 32768) return RBMF_ERR_ARG;
+    *bytes = prep_basis_workspace_bytes(n_templates, k);
+    return RBMF_OK;
+}
+
+rbmf_status rbmf_prepare_basis(const void* templates_dev, int32_t n_templates, int64_t N, double fs, double f_low,
+                               int32_t k, int32_t iterations, uint64_t seed, void* workspace_dev, size_t workspace_bytes,
+                               void* basis_out_dev, float* eig_out_dev, void* cuda_stream) {
+    int j_low = 0;
+    int64_t n_half = 0;
+    if (!templates_dev || !workspace_dev || !basis_out_dev || !prep_args_ok(N, fs, f_low, &j_low, &n_half)) return RBMF_ERR_ARG;
+    if (n_templates < 1 || n_templates > 32768 || k < 1 || k > n_templates || k > 1024 || iterations < 1 || iterations > 1000)
+        return RBMF_ERR_ARG;
+    if (((uintptr_t)workspace_dev % 16) != 0 || workspace_bytes < prep_basis_workspace_bytes(n_templates, k)) return RBMF_ERR_ARG;
+    cudaError_t e = launch_prep_basis((const float2*)templates_dev, n_templates, N / 2 + 1, j_low, n_half, k, iterations,
+                                      (unsigned long long)seed, workspace_dev, (float2*)basis_out_dev, eig_out_dev,
+                                      (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? RBMF_OK : RBMF_ERR_CUDA;
+}
+
+rbmf_status rbmf_prepare_coeffs(const void* templates_dev, int32_t n_templates, const void* basis_dev, int32_t k,
+                                int64_t N, double fs, double f_low, void* coeffs_out_dev, float* sigma_out_dev,
+                                void* cuda_stream) {
+    int j_low = 0;
+    int64_t n_half = 0;
+    if (!templates_dev || !basis_dev || !coeffs_out_dev || !prep_args_ok(N, fs, f_low, &j_low, &n_half)) return RBMF_ERR_ARG;
+    if (n_templates < 1 || n_templates > (1 << 24) || k < 1 || k > 1024) return RBMF_ERR_ARG;
+    cudaError_t e = launch_prep_coeffs_from_templates((const float2*)templates_dev, n_templates, (const float2*)basis_dev, k,
+                                                      N / 2 + 1, j_low, n_half, (float2*)coeffs_out_dev, sigma_out_dev,
+                                                      (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? RBMF_OK : RBMF_ERR_CUDA;
+}
+
 // ---- bank sets: many sub-banks against one strain (Table I) ------------------------
 struct rbmf_bankset {
     int n;

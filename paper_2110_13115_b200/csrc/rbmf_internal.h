@@ -154,6 +154,14 @@ cudaError_t gemm_tcgen05_configure();   // sets the dynamic shared memory attrib
 cudaError_t launch_stage2(const Stage2Args& a, int num_sms, cudaStream_t st);          // one warp per candidate
 cudaError_t launch_stage2_bybin(const Stage2Args& a, int num_sms, cudaStream_t st);    // regrouped by bin (default)
 int stage2_bybin_smem(int w, int k);
+// preparation (prep_basis.cu): PCA of a (sub-)bank and projection of templates onto a basis
+size_t prep_basis_workspace_bytes(int S, int k);
+cudaError_t launch_prep_basis(const float2* templates, int S, long long bins, int j_low, long long n_half, int k,
+                              int iterations, unsigned long long seed, void* workspace, float2* basis_out,
+                              float* eig_out, cudaStream_t st);
+cudaError_t launch_prep_coeffs_from_templates(const float2* templates, int T, const float2* basis, int k, long long bins,
+                                              int j_low, long long n_half, float2* coeffs_out, float* sigma_out,
+                                              cudaStream_t st);
 // front end (fft_r2c.cu): forward real-to-complex FFT of nb series of N = 2^logN samples + whitening
 cudaError_t r2c_configure();
 cudaError_t launch_r2c_table(float2* twF, long long N, cudaStream_t st);

@@ -46,6 +46,10 @@ SIGNATURES = {
     "rbmf_set_coeffs": (_i32, [_vp, _vp, _vp]),
     "rbmf_filter": (_i32, [_vp, _vp, _f32, _f32, _vp, _vp]),
     "rbmf_prepare_strain": (_i32, [_vp, _vp, _vp, _i32, _vp]),
+    "rbmf_prepare_basis_workspace_bytes": (_i32, [_i32, _i32, _psz]),
+    "rbmf_prepare_basis": (_i32, [_vp, _i32, _i64, _f64, _f64, _i32, _i32, ctypes.c_uint64, _vp, ctypes.c_size_t, _vp, _vp,
+                                  _vp]),
+    "rbmf_prepare_coeffs": (_i32, [_vp, _i32, _vp, _i32, _i64, _f64, _f64, _vp, _vp, _vp]),
     "rbmf_bankset_create": (_i32, [ctypes.POINTER(_vp), ctypes.POINTER(_vp), _i32]),
     "rbmf_bankset_filter": (_i32, [_vp, _vp, _f32, _f32, _vp, _i64, _vp, _vp]),
     "rbmf_bankset_get_counts": (_i32, [_vp, _pi64, _pi64, _pi64]),
@@ -481,3 +485,45 @@ class BankSet:
             self.close()
         except Exception:
             pass
+
+
+def prepare_basis(templates_dev, N, fs, f_low, k, iterations=12, seed=1, stream=None):
+    """rbmf_prepare_basis + rbmf_prepare_coeffs on a (S, N/2+1) complex64 CUDA tensor of templates: returns
+    (basis (k, N/2+1) complex64, eigenvalue estimates (k,) float32) as CUDA tensors."""
+    import torch
+    if (templates_dev.dtype != torch.complex64 or templates_dev.dim() != 2 or templates_dev.shape[1] != N // 2 + 1
+            or not templates_dev.is_cuda or not templates_dev.is_contiguous()):
+        raise ValueError("templates must be a contiguous complex64 CUDA tensor of shape (S, N/2+1)")
+    S = int(templates_dev.shape[0])
+    st = stream if stream is not None else torch.cuda.current_stream(templates_dev.device)
+    nbytes = ctypes.c_size_t()
+    rc = _lib.rbmf_prepare_basis_workspace_bytes(S, int(k), ctypes.byref(nbytes))
+    if rc != RBMF_OK:
+        raise RbmfError(rc, "rbmf_prepare_basis_workspace_bytes")
+    with torch.cuda.device(templates_dev.device), torch.cuda.stream(st):
+        ws = torch.empty(nbytes.value + 16, dtype=torch.uint8, device=templates_dev.device)
+        base = (ws.data_ptr() + 15) // 16 * 16
+        basis = torch.empty((int(k), N // 2 + 1), dtype=torch.complex64, device=templates_dev.device)
+        eig = torch.empty(int(k), dtype=torch.float32, device=templates_dev.device)
+        rc = _lib.rbmf_prepare_basis(_ptr(templates_dev), S, int(N), float(fs), float(f_low), int(k), int(iterations),
+                                     int(seed), _vp(base), nbytes.value, _ptr(basis), _ptr(eig), _vp(st.cuda_stream))
+        if rc != RBMF_OK:
+            raise RbmfError(rc, "rbmf_prepare_basis")
+        st.synchronize()
+    return basis, eig
+
+
+def prepare_coeffs(templates_dev, basis_dev, N, fs, f_low, stream=None):
+    """rbmf_prepare_coeffs: (T, N/2+1) templates and (k, N/2+1) basis -> (coeffs (T, k) complex64, sigma (T,) float32)."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(templates_dev.device)
+    T, k = int(templates_dev.shape[0]), int(basis_dev.shape[0])
+    with torch.cuda.device(templates_dev.device), torch.cuda.stream(st):
+        coeffs = torch.empty((T, k), dtype=torch.complex64, device=templates_dev.device)
+        sigma = torch.empty(T, dtype=torch.float32, device=templates_dev.device)
+        rc = _lib.rbmf_prepare_coeffs(_ptr(templates_dev), T, _ptr(basis_dev), k, int(N), float(fs), float(f_low),
+                                      _ptr(coeffs), _ptr(sigma), _vp(st.cuda_stream))
+        if rc != RBMF_OK:
+            raise RbmfError(rc, "rbmf_prepare_coeffs")
+        st.synchronize()
+    return coeffs, sigma

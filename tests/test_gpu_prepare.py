@@ -1,0 +1,71 @@
+"""Preparation on the GPU against the oracle's covariance + EVD route
+(`oracle.pca_basis`), and end to end: a basis and coefficients prepared by the library, handed to the path, pass the
+usual oracle comparison (the oracle takes the very arrays the library produced)."""
+import numpy as np
+import pytest
+
+from oracle import compare
+from oracle import rbmf_oracle as orc
+from paper_2110_13115_b200 import workloads as wlm
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def rbmf(built_library):
+    from paper_2110_13115_b200 import rbmf as mod
+    return mod
+
+
+@pytest.mark.parametrize("name,k,iterations", [("tiny", 16, 40), ("tiny", 48, 30), ("mini", 32, 40)])
+def test_prepared_basis_against_pca_oracle(rbmf, name, k, iterations):
+    import torch
+    wl = wlm.make_workload(wlm.CONFIGS[name], device="cuda")
+    cfg = wl["config"]
+    U = wlm.bank_templates(wl, np.arange(cfg.T), device="cuda")             # (T, bins) complex128, unit norm
+    U32 = U.astype(np.complex64)
+    tpl = torch.from_numpy(U32).cuda()
+    basis_dev, eig = rbmf.prepare_basis(tpl, cfg.N, cfg.fs, cfg.f_low, k, iterations=iterations, seed=7)
+    coeffs_dev, sigma_dev = rbmf.prepare_coeffs(tpl, basis_dev, cfg.N, cfg.fs, cfg.f_low)
+    basis, coeffs, sigma = basis_dev.cpu().numpy(), coeffs_dev.cpu().numpy(), sigma_dev.cpu().numpy()
+    # orthonormal over the band, zero outside it
+    B = basis.astype(np.complex128)
+    assert np.abs(B @ B.conj().T - np.eye(k)).max() < 2e-5
+    assert not B[:, :cfg.j_low].any() and not B[:, cfg.N // 2:].any()
+    # the coefficients are the projections on THIS basis (fp32 products, fp64 block sums)
+    ref_c = U32.astype(np.complex128) @ B.conj().T
+    assert np.abs(coeffs - ref_c).max() < 2e-6
+    assert np.abs(sigma - np.linalg.norm(ref_c, axis=1)).max() < 2e-6
+    # it captures what the exact PCA basis captures (Eq. 8): the subspace iteration has converged in power
+    exact_basis, _, sv = orc.pca_basis(U32.astype(np.complex128), k)
+    cap, cap_exact = orc.captured_power(U32, B), orc.captured_power(U32, exact_basis)
+    assert cap <= cap_exact + 1e-6 and cap >= cap_exact * (1.0 - 2e-3), (cap, cap_exact)
+    # eigenvalue estimates against the squared singular values (leading ones, which converge first)
+    lam = np.sort(eig.cpu().numpy())[::-1]
+    assert np.abs(lam[:4] - sv[:4] ** 2).max() < 2e-2 * sv[0] ** 2
+    # determinism: same seed, same bytes
+    again, _ = rbmf.prepare_basis(tpl, cfg.N, cfg.fs, cfg.f_low, k, iterations=iterations, seed=7)
+    assert torch.equal(again, basis_dev)
+
+
+def test_prepared_inputs_through_the_path(rbmf):
+    """templates -> rbmf_prepare_basis -> rbmf_prepare_coeffs -> rbmf_set_basis / rbmf_set_coeffs -> rbmf_filter."""
+    import torch
+    wl = wlm.make_workload(wlm.CONFIGS["mini"], device="cuda")
+    cfg = wl["config"]
+    tpl = torch.from_numpy(wlm.bank_templates(wl, np.arange(cfg.T), device="cuda").astype(np.complex64)).cuda()
+    basis_dev, _ = rbmf.prepare_basis(tpl, cfg.N, cfg.fs, cfg.f_low, cfg.k, iterations=25, seed=3)
+    coeffs_dev, sigma_dev = rbmf.prepare_coeffs(tpl, basis_dev, cfg.N, cfg.fs, cfg.f_low)
+    plan = rbmf.Plan(cfg.N, cfg.fs, cfg.f_low, cfg.k, cfg.T, w=cfg.w, max_candidates=1 << 20, max_triggers=1 << 20)
+    plan.set_basis(basis_dev)
+    plan.set_coeffs(coeffs_dev, sigma_dev)
+    thr = (3.0, 4.0)
+    got = plan.filter(torch.from_numpy(wl["strain"]), *thr)
+    ref = orc.oracle_filter(wl["strain"], basis_dev.cpu().numpy(), coeffs_dev.cpu().numpy(), sigma_dev.cpu().numpy(),
+                            cfg.N, cfg.fs, cfg.f_low, cfg.w, *thr)
+    rep = compare.compare_triggers(got, ref, cfg.N, *thr)
+    plan.close()
+    assert rep["ok"] and rep["n_mandatory"] > 500, rep
+    # the prepared basis captures what the generator's fp64 SVD basis of the same size captures, to 1 %
+    cap = float((sigma_dev.double() ** 2).mean())
+    assert cap > 0.99 * wl["captured"], (cap, wl["captured"])
