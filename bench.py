@@ -485,6 +485,26 @@ def measure_bankset(steps, rbmf, workloads, torch, device, stream):
             "n_triggers": tot, "per_sub_bank_triggers": nt, "unit": UNIT}
 
 
+def measure_prepare(name, rbmf, workloads, torch, device):
+    """f4: preparation on the GPU (covariance + block power iteration + projection) for one config's bank."""
+    cfg = workloads.CONFIGS[name]
+    wl = workloads.make_workload(cfg, device=str(device))
+    n = min(cfg.T, cfg.basis_subset)
+    ids = np.arange(n)
+    tpl = torch.from_numpy(workloads.bank_templates(wl, ids, device=str(device)).astype(np.complex64)).to(device)
+    torch.cuda.synchronize(device)
+    t0 = time.time()
+    basis, _ = rbmf.prepare_basis(tpl, cfg.N, cfg.fs, cfg.f_low, cfg.k, iterations=12, seed=1)
+    torch.cuda.synchronize(device)
+    t1 = time.time()
+    coeffs, sigma = rbmf.prepare_coeffs(tpl, basis, cfg.N, cfg.fs, cfg.f_low)
+    torch.cuda.synchronize(device)
+    t2 = time.time()
+    return {"row": "f4 preparation on the GPU", "workload": describe(cfg, 1)["workload"], "templates": int(n),
+            "prepare_basis_s": t1 - t0, "prepare_coeffs_s": t2 - t1, "iterations": 12,
+            "captured_power": float((sigma.double() ** 2).mean()), "captured_power_generator_fp64_svd": wl["captured"]}
+
+
 # ---------------------------------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -500,10 +520,10 @@ def main():
                     help="configs summarised in the `configs` array of the default line ('' = none)")
     ap.add_argument("--summary-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--extras", default="batch,routes,bankset",
+    ap.add_argument("--extras", default="batch,routes,bankset,prepare",
                     help="SURVEY 8(f) rows measured into the `extras` array of the default line: batch (f1: small at "
                          "B=8, paper at B=4), routes (f2: template routes vs GEMM route on small and paper), bankset "
-                         "(f3); '' = none")
+                         "(f3), prepare (f4: preparation kernels on small); '' = none")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -575,6 +595,8 @@ def main():
                 line["extras"] += measure_routes("paper", (8, 16), 4, rbmf, workloads, torch, device, stream)
             if "bankset" in ex:
                 line["extras"].append(measure_bankset(20, rbmf, workloads, torch, device, stream))
+            if "prepare" in ex:
+                line["extras"].append(measure_prepare("small", rbmf, workloads, torch, device))
         if rank == 0:
             print(json.dumps(line), flush=True)
     rdist.finalize()
