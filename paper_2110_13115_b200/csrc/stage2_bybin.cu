@@ -78,7 +78,7 @@ __device__ __forceinline__ void lane_reduce(float (&v)[NV], int lane) {
 // CU = basis-column steps (of 32 columns) whose coefficient loads are issued together: the G CU loads per lane come
 // from L2 (~700 cycles) and must be in flight while the previous step's 4 G W FMAs run.
 template <int W, int G, int CU>
-__global__ void __launch_bounds__(NWARP * 32) stage2_score_kernel(const Stage2Args a) {
+__global__ void __launch_bounds__(NWARP * 32, 4) stage2_score_kernel(const Stage2Args a) {
     constexpr int NV = G * W * 2;
     static_assert(NV == 32 || NV == 64, "G W must be 16 or 32");
     extern __shared__ float4 smem4[];
