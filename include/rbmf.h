@@ -14,8 +14,12 @@
  * with s = sqrt(2/N), d = unnormalised forward DFT of the whitened unit-variance strain, b_k orthonormal
  * over the band, c_tk the decomposition coefficients.  Every step runs in hand-written CUDA
  * kernels for sm_100a (a persistent, TMA-fed batched four-step Stockham FFT; a tcgen05/TMEM GEMM -- fp16 screen with a
- * proven error bound by default, split-bf16 on request -- with a fused threshold/compaction epilogue; a
- * warp-per-candidate re-scoring kernel that also confirms the screen's hits in fp32).  There is no CPU fallback.
+ * proven error bound by default, split-bf16 on request -- with a fused threshold/compaction epilogue; a re-scoring
+ * kernel that regroups the candidates by bin, scores them from a shared-memory copy of the bin's block of beta and
+ * also confirms the screen's hits in fp32).  There is no CPU fallback.
+ * Around that path: batches of segments and the step in front of the path (rbmf_filter_batch,
+ * rbmf_prepare_strain), the paper's template routes as comparators (rbmf_filter_flat, RBMF_STAGE1_TEMPLATES), many
+ * sub-banks against one strain (rbmf_bankset_*), and the preparation of a sub-bank (rbmf_prepare_basis / _coeffs).
  *
  * Conventions
  *  - "dev" pointers are CUDA device memory owned by the caller; "host" pointers are ordinary host memory.
