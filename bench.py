@@ -505,6 +505,44 @@ def measure_prepare(name, rbmf, workloads, torch, device):
             "captured_power": float((sigma.double() ** 2).mean()), "captured_power_generator_fp64_svd": wl["captured"]}
 
 
+def measure_cufft_context(names, workloads, torch, device):
+    """Context only, never on the hot path: what the library FFT needs for the same transform sizes -- a batched
+    complex-to-complex inverse FFT of k series of N samples through torch.fft (cuFFT) ALONE, and the paper's three
+    separate steps (pointwise multiply, batched IFFT, w-sample averaging) as torch ops -- next to
+    which the fused kernel 1 (multiply + IFFT + averaging + operand planes in one launch) is reported."""
+    out = []
+    for name in names:
+        cfg = workloads.CONFIGS[name]
+        N, k, w = cfg.N, cfg.k, cfg.w
+        x = torch.randn(k, N, dtype=torch.complex64, device=device)
+        b = torch.randn(k, N // 2, dtype=torch.complex64, device=device)
+        d = torch.randn(N // 2, dtype=torch.complex64, device=device)
+
+        def timed(fn, reps=20):
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize(device)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(reps):
+                fn()
+            e1.record()
+            torch.cuda.synchronize(device)
+            return e0.elapsed_time(e1) / reps
+
+        def three_steps():
+            x[:, :N // 2] = d[None, :] * b.conj()
+            x[:, N // 2:] = 0
+            return torch.fft.ifft(x, dim=1, norm="forward").view(k, N // w, w).mean(dim=2)
+
+        out.append({"row": "context: library FFT (cuFFT through torch.fft), not on the hot path",
+                    "workload": "%s: N=%d k=%d w=%d" % (name, N, k, w),
+                    "cufft_batched_c2c_ifft_alone_ms": timed(lambda: torch.fft.ifft(x, dim=1, norm="forward")),
+                    "multiply_ifft_average_as_torch_ops_ms": timed(three_steps)})
+        del x, b, d
+    return out
+
+
 # ---------------------------------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -520,10 +558,11 @@ def main():
                     help="configs summarised in the `configs` array of the default line ('' = none)")
     ap.add_argument("--summary-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--extras", default="batch,routes,bankset,prepare",
+    ap.add_argument("--extras", default="batch,routes,bankset,prepare,cufft",
                     help="SURVEY 8(f) rows measured into the `extras` array of the default line: batch (f1: small at "
                          "B=8, paper at B=4), routes (f2: template routes vs GEMM route on small and paper), bankset "
-                         "(f3), prepare (f4: preparation kernels on small); '' = none")
+                         "(f3), prepare (f4: preparation kernels on small), cufft (context: the library FFT alone on the same "
+                         "sizes); '' = none")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -597,6 +636,9 @@ def main():
                 line["extras"].append(measure_bankset(20, rbmf, workloads, torch, device, stream))
             if "prepare" in ex:
                 line["extras"].append(measure_prepare("small", rbmf, workloads, torch, device))
+            if "cufft" in ex:
+                line["extras"] += measure_cufft_context(("small", "paper", "large", "sweep_k256_T10000"), workloads, torch,
+                                                        device)
         if rank == 0:
             print(json.dumps(line), flush=True)
     rdist.finalize()
