@@ -535,11 +535,20 @@ def measure_cufft_context(names, workloads, torch, device):
             x[:, N // 2:] = 0
             return torch.fft.ifft(x, dim=1, norm="forward").view(k, N // w, w).mean(dim=2)
 
-        out.append({"row": "context: library FFT (cuFFT through torch.fft), not on the hot path",
-                    "workload": "%s: N=%d k=%d w=%d" % (name, N, k, w),
-                    "cufft_batched_c2c_ifft_alone_ms": timed(lambda: torch.fft.ifft(x, dim=1, norm="forward")),
-                    "multiply_ifft_average_as_torch_ops_ms": timed(three_steps)})
+        row = {"row": "context: library FFT / GEMM (cuFFT, cuBLAS through torch), not on the hot path",
+               "workload": "%s: N=%d k=%d T=%d w=%d" % (name, N, k, cfg.T, w),
+               "cufft_batched_c2c_ifft_alone_ms": timed(lambda: torch.fft.ifft(x, dim=1, norm="forward")),
+               "multiply_ifft_average_as_torch_ops_ms": timed(three_steps)}
         del x, b, d
+        # the paper's stage 1: cuBLAS on beta^avg and the coefficients, then a separate trigger search
+        if cfg.T * (N // w) * 8 <= 48e9:
+            coeff = torch.randn(cfg.T, k, dtype=torch.complex64, device=device)
+            bavg = torch.randn(k, N // w, dtype=torch.complex64, device=device)
+            row["cublas_cgemm_fp32_stage1_ms"] = timed(lambda: torch.matmul(coeff, bavg), reps=3)
+            row["cublas_cgemm_plus_threshold_count_ms"] = timed(
+                lambda: (torch.view_as_real(torch.matmul(coeff, bavg)).square_().sum(dim=-1) >= 25.0).sum(), reps=3)
+            del coeff, bavg
+        out.append(row)
     return out
 
 
@@ -617,7 +626,7 @@ def main():
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
                                     "ms_per_step": ms}
         del wl
-        if args.config != "all" and world == 1 and args.summary_configs:
+        if args.config != "all" and world == 1:
             line["configs"] = []
             for other in [c for c in args.summary_configs.split(",") if c and c != name]:
                 summ, wl2 = measure(workloads.CONFIGS[other], args, rdist, rbmf, workloads, torch, device, stream, rank,
