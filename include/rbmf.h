@@ -146,8 +146,8 @@ rbmf_status rbmf_prepare_strain(rbmf_plan* plan, const float* x_dev, const float
 
 /* Filter n_segments (1 <= n_segments <= max_batch) segments at once ("filtering each segment in
  * parallel", basis and coefficients loaded once).  strain_dev: n_segments x (N/2+1) complex64, row-major, each row as
- * in rbmf_filter.  Steps a1-a3 run once per (segment, basis column) in ONE launch that reads every block of the
- * basis from HBM once and takes it from L2 for the other segments; steps a4-a5 run as ONE contraction over the
+ * in rbmf_filter.  Steps a1-a3 run once per (segment, basis column) in ONE persistent launch (no launch gaps or
+ * pipeline drains between segments); steps a4-a5 run as ONE contraction over the
  * n_segments * N/w bins of the batch (each coefficient tile is loaded once per batch); step a6 over all candidates.
  * Triggers carry the segment in the time index: time_index = segment * N + n, n in [0, N)  (rbmf_candidate:
  * bin_index = segment * N/w + i).  The result equals n_segments calls of rbmf_filter, segment by segment.

@@ -309,7 +309,7 @@ __device__ __forceinline__ void p1_tile(const FftArgs& a, int g, int gt, int chu
 
     // ---- stage 1 + inter-pass twiddle + store of Y (in place in the beta array) -------------------------------
     // virtual chunk = c * nb + b: basis chunk c against segment b's strain; beta arrays are [segment][chunk]
-    const int bc = chunk / a.nb, bs = chunk - bc * a.nb;
+    const int bc = a.seg_major ? chunk % a.nchunk : chunk / a.nb, bs = a.seg_major ? chunk / a.nchunk : chunk % a.nb;
     float2* yrow = a.beta + ((size_t)(bs * a.nchunk + bc) * (size_t)a.N + (size_t)j2 * L1) * C + col;
     const float2* e2 = e2s + line * (R1 + 2);
 #pragma unroll
@@ -365,7 +365,7 @@ __device__ __forceinline__ void p2_round(const FftArgs& a, const CUtensorMap* tm
     const int col = gt % C, line = (gt / C) % SUB, wk = gt / (C * SUB);
     const int slot = line * C + col;
     const int w = a.w;
-    const int bc = chunk / a.nb, bs = chunk - bc * a.nb;   // virtual chunk = c * nb + b (see p1_tile)
+    const int bc = a.seg_major ? chunk % a.nchunk : chunk / a.nb, bs = a.seg_major ? chunk / a.nchunk : chunk % a.nb;
     const int zc = bs * a.nchunk + bc;                     // the chunk's block of the beta array
     const int gcol = bc * C + col;
     const int bin0 = bs * a.Mseg;                          // the segment's first row of the planes
@@ -579,7 +579,8 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                 const int ms = i % (2 * NBUF);
                 meta[ms].x = type; meta[ms].y = chunk; meta[ms].z = idx; meta[ms].w = rd;
                 const uint32_t dst = smem_u32(buf_ptr(buf));
-                const int bc = chunk / a.nb, bs = chunk - bc * a.nb;   // virtual chunk = c * nb + b
+                // virtual chunk = c * nb + b (chunk-major: a basis chunk serves all segments from L2) or b * nchunk + c
+                const int bc = a.seg_major ? chunk % a.nchunk : chunk / a.nb, bs = a.seg_major ? chunk / a.nchunk : chunk % a.nb;
                 // both parts of a pass-1 tile sit in global memory in tile-buffer order (rbmf_internal.h): one bulk copy each
                 constexpr uint32_t basis_bytes = (uint32_t)fft_p1_rows(LOG1) * K1::RB * 8;
                 constexpr uint32_t strain_bytes = (uint32_t)K1::SUB * fft_strain_row(LOG1) * 8;
@@ -588,7 +589,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                 const float2* src_basis = a.basisP + ((size_t)bc * n1t + idx) * (size_t)(fft_p1_rows(LOG1) * K1::RB);
                 const float2* src_strain = a.dsT + ((size_t)bs * L2 + (size_t)idx * K1::SUB) * fft_strain_row(LOG1);
                 // a basis chunk is streamed from HBM once per call: later segments of a batch find it in L2
-                const unsigned long long pol_basis = bs == a.nb - 1 ? pol_first : pol_normal;
+                const unsigned long long pol_basis = (a.seg_major || bs == a.nb - 1) ? pol_first : pol_normal;
                 constexpr int BR = L2 < 256 ? L2 : 256;          // rows per tensor copy of a pass-2 tile
                 const int x = (idx + rd * K2::SUB) * C * 2;      // floats along the (n1, col) axis
                 const int zc = bs * a.nchunk + bc;               // the chunk's block of the beta array

@@ -474,6 +474,11 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     a.nchunk = plan->k / kFftC; a.w = plan->w; a.inv_w = 1.0f / (float)plan->w;
     const bool screen = plan->gemm_impl == RBMF_GEMM_SCREEN && !plan->diag_fp32_check;
     a.plane_fp16 = screen ? 1 : 0;
+    // Batches run segment-major (every segment streams the basis from HBM again): keeping a basis chunk in L2 for the
+    // other segments (chunk-major) displaces the in-place intermediate Y and measured 5-10 % slower per segment at
+    // every size (Small B = 8: 0.74 vs 0.70 ms; Paper B = 4: 3.69 vs 3.37 ms) -- the kernel is not bound by that stream.
+    a.seg_major = 1;
+    if (const char* e = getenv("RBMF_FFT_SEG_MAJOR")) a.seg_major = atoi(e) ? 1 : 0;   // developer switch
     {
         // Pass-1 lookahead: a chunk's pass 2 needs ALL of its pass-1 tiles, so enough pass-1 tiles of later chunks
         // must be queued to keep every consumer group (2 per SM) busy meanwhile -- about two tiles per group --,

@@ -64,6 +64,7 @@ struct FftArgs {
     float inv_w;
     int lookahead;           // (virtual) chunks pass 1 runs ahead of pass 2 in the work queue (their Y must fit in L2)
     int nb;                  // segments of the batch: virtual chunk v = c * nb + b reads basis chunk c, strain b
+    int seg_major;           // 1: v = b * nchunk + c instead (every segment streams the basis from HBM again)
     int Mseg;                // bins per segment (N / w); segment b's bins are [b Mseg, (b + 1) Mseg) of the planes
     int plane_fp16;          // 1: write ONE fp16 plane (screen mode) into plane_hi; 0: bf16 hi + lo planes
     int no_planes;           // 1: skip step a3's plane output altogether (template routes read beta directly)
