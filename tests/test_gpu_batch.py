@@ -314,3 +314,37 @@ def test_bank_set_of_three_sub_banks(rbmf):
     bs.close()
     for p in plans:
         p.close()
+
+
+@pytest.mark.parametrize("name,nb,calls", [("small", 1, 400), ("small", 3, 150), ("mini", 2, 600)])
+def test_soak_hundreds_of_calls_give_identical_digests(rbmf, name, nb, calls):
+    """Hundreds of back-to-back calls: an order-independent digest of the trigger list, of the candidate list and of
+    the raw beta bytes must never change (no sanitizer on this pool: a rare race in the FFT's hand-offs, the GEMM's
+    multicast pipeline or the by-bin regrouping would show here)."""
+    import ctypes
+    import torch
+    wl = workload(name)
+    cfg = wl["config"]
+    strains = torch.from_numpy(strains_of(wl, nb)).cuda()
+    plan = make_plan(rbmf, wl, max_batch=nb, cap=1 << 21)
+    thr = (cfg.thr1, cfg.thr2) if name == "small" else (3.0, 4.0)
+
+    def digest():
+        rows = plan.triggers_device().to(torch.int64)
+        c = plan.candidates_device().to(torch.int64)
+        p, nbytes = ctypes.c_void_p(), ctypes.c_size_t()
+        assert rbmf.rbmf_get_internal(plan._h, 0, ctypes.byref(p), ctypes.byref(nbytes)) == rbmf.RBMF_OK
+        off = p.value - plan._ws.data_ptr()
+        beta = plan._ws[off: off + nbytes.value].view(torch.int32).to(torch.int64).sum()
+        mix = lambda r: ((r[:, 0] * 1000003 + r[:, 1]) * 998244353 + r[:, 2] * 7919 + r[:, 3]).sum()
+        return int(mix(rows)), int(rows.shape[0]), int(mix(c)), int(c.shape[0]), int(beta)
+
+    first = None
+    for _ in range(calls):
+        plan.filter_batch_async(strains, *thr)
+        d = digest()
+        if first is None:
+            first = d
+            assert d[1] > 100
+        assert d == first
+    plan.close()
