@@ -333,10 +333,18 @@ def measure(cfg, args, rdist, rbmf, workloads, torch, device, stream, rank, worl
                     int(products), "one fp16 product: error-bounded screen, fp32 confirm in kernel 3"
                     if args.gemm == "screen" else "bf16x3 split precision"),
                 "useful_tflops": useful_flops / (gemm_ms * 1e-3) / 1e12, "avg_kernel_ms": gemm_ms}
+    # second roofline of kernel 1: its fp32 arithmetic, 5 N log2 N flops per series + 6 per band bin (the paper's count,
+    # PAPER.md:236), against 148 SMs x 128 lanes x 2 (FMA) x the SM clock sampled under load
+    fft_flops = cfg.k * (5.0 * cfg.N * np.log2(cfg.N) + 6.0 * band)
+    sm_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
+    alu_peak = 148 * 128 * 2 * sm_hz / 1e12
+    fft_alu = {"bound": "alu", "achieved": fft_flops / (fft_ms * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
+               "frac": fft_flops / (fft_ms * 1e-3) / 1e12 / alu_peak,
+               "note": "fp32 FMA peak at the sampled clock; a butterfly network is ~2/3 additions, so 0.5 is its ceiling"}
     stages = {"fft_ms": fft_ms, "gemm_ms": gemm_ms, "stage2_ms": s2_ms, "total_ms": statistics.mean(stage["total"]),
               "per_step_ms": {kk: stat(v) for kk, v in stage.items()},
               "fft": {"bound": "hbm", "algorithmic_GBps": fft_gbs, "peak": hbm_peak, "frac": fft_gbs / hbm_peak,
-                      "algorithmic_bytes": fft_alg_bytes, "traffic": traffic.get("fft")},
+                      "algorithmic_bytes": fft_alg_bytes, "traffic": traffic.get("fft"), "alu": fft_alu},
               "stage2": {"candidates_per_s": (nc / (s2_ms * 1e-3)) if s2_ms > 0 else None,
                          "algorithmic_GBps": n_screened * (cfg.w + 1) * cfg.k * 8 / (s2_ms * 1e-3) / 1e9,
                          "traffic": traffic.get("stage2")},
