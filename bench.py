@@ -344,7 +344,12 @@ def measure(cfg, args, rdist, rbmf, workloads, torch, device, stream, rank, worl
     stages = {"fft_ms": fft_ms, "gemm_ms": gemm_ms, "stage2_ms": s2_ms, "total_ms": statistics.mean(stage["total"]),
               "per_step_ms": {kk: stat(v) for kk, v in stage.items()},
               "fft": {"bound": "hbm", "algorithmic_GBps": fft_gbs, "peak": hbm_peak, "frac": fft_gbs / hbm_peak,
-                      "algorithmic_bytes": fft_alg_bytes, "traffic": traffic.get("fft"), "alu": fft_alu},
+                      "algorithmic_bytes": fft_alg_bytes, "traffic": traffic.get("fft"),
+                      # real DRAM bytes of the committed ncu capture over this run's event time (both
+                      # the algorithmic and the achieved DRAM rate are reported)
+                      "dram_GBps": (traffic["fft"] / (fft_ms * 1e-3) / 1e9) if traffic.get("fft") else None,
+                      "dram_frac": (traffic["fft"] / (fft_ms * 1e-3) / 1e9 / hbm_peak) if traffic.get("fft") else None,
+                      "alu": fft_alu},
               "stage2": {"candidates_per_s": (nc / (s2_ms * 1e-3)) if s2_ms > 0 else None,
                          "algorithmic_GBps": n_screened * (cfg.w + 1) * cfg.k * 8 / (s2_ms * 1e-3) / 1e9,
                          "traffic": traffic.get("stage2")},
