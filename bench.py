@@ -640,27 +640,36 @@ def main():
                                     "ms_per_step": ms}
         del wl
         if args.config != "all" and world == 1:
+            # The headline above is complete; what follows adds context to the same line.  A failure in one of these
+            # side measurements (e.g. out of memory on a smaller device) is recorded in the line, not raised.
+            def guarded(target, label, fn):
+                try:
+                    out = fn()
+                    target.extend(out if isinstance(out, list) else [out])
+                except Exception as exc:                  # noqa: BLE001
+                    target.append({"row": label, "error": "%s: %s" % (type(exc).__name__, str(exc)[:300])})
+                    torch.cuda.empty_cache()
+
             line["configs"] = []
             for other in [c for c in args.summary_configs.split(",") if c and c != name]:
-                summ, wl2 = measure(workloads.CONFIGS[other], args, rdist, rbmf, workloads, torch, device, stream, rank,
-                                    world, local_rank, False)
-                del wl2
-                line["configs"].append(summ)
+                guarded(line["configs"], other,
+                        lambda other=other: measure(workloads.CONFIGS[other], args, rdist, rbmf, workloads, torch, device,
+                                                    stream, rank, world, local_rank, False)[0])
             ex = [e for e in args.extras.split(",") if e]
             line["extras"] = []
             if "batch" in ex:
-                line["extras"].append(measure_batch("small", 8, 20, rbmf, workloads, torch, device, stream))
-                line["extras"].append(measure_batch("paper", 4, 10, rbmf, workloads, torch, device, stream))
+                guarded(line["extras"], "f1 batch small", lambda: measure_batch("small", 8, 20, rbmf, workloads, torch, device, stream))
+                guarded(line["extras"], "f1 batch paper", lambda: measure_batch("paper", 4, 10, rbmf, workloads, torch, device, stream))
             if "routes" in ex:
-                line["extras"] += measure_routes("small", (8, 16), 10, rbmf, workloads, torch, device, stream)
-                line["extras"] += measure_routes("paper", (8, 16), 4, rbmf, workloads, torch, device, stream)
+                guarded(line["extras"], "f2 routes small", lambda: measure_routes("small", (8, 16), 10, rbmf, workloads, torch, device, stream))
+                guarded(line["extras"], "f2 routes paper", lambda: measure_routes("paper", (8, 16), 4, rbmf, workloads, torch, device, stream))
             if "bankset" in ex:
-                line["extras"].append(measure_bankset(20, rbmf, workloads, torch, device, stream))
+                guarded(line["extras"], "f3 bank set", lambda: measure_bankset(20, rbmf, workloads, torch, device, stream))
             if "prepare" in ex:
-                line["extras"].append(measure_prepare("small", rbmf, workloads, torch, device))
+                guarded(line["extras"], "f4 preparation", lambda: measure_prepare("small", rbmf, workloads, torch, device))
             if "cufft" in ex:
-                line["extras"] += measure_cufft_context(("small", "paper", "large", "sweep_k256_T10000"), workloads, torch,
-                                                        device)
+                guarded(line["extras"], "library context",
+                        lambda: measure_cufft_context(("small", "paper", "large", "sweep_k256_T10000"), workloads, torch, device))
         if rank == 0:
             print(json.dumps(line), flush=True)
     rdist.finalize()
