@@ -144,6 +144,47 @@ rbmf_status rbmf_filter(rbmf_plan* plan, const void* strain_dev, float thr_stage
 rbmf_status rbmf_prepare_strain(rbmf_plan* plan, const float* x_dev, const float* inv_asd_dev, int32_t n_segments,
                                 void* strain_out_dev);
 
+/* rbmf_prepare_strain for callers that cannot provide device memory: no plan, no workspace, and not one allocation
+ * (no cudaMalloc / cudaFree / allocating library routine) inside the call.
+ *
+ * Who needs it.  Every other entry point works out of a workspace the caller allocates; rbmf_prepare_strain needs a
+ * whole plan (sized for the filter) just to borrow 3 small scratch arrays from it.  Some users of the front end cannot
+ * do that: a strain-conditioning stage that whitens data for several filter processes and owns no plan; a plug-in or
+ * callback that runs inside another program's pipeline and is handed only its input and output buffers; a process in
+ * which a framework's memory pool has already taken the whole GPU, so a raw cudaMalloc fails; a low-latency loop
+ * (online searches use reduced-basis filtering; whitening dominates their latency) where cudaMalloc's device-wide synchronisation would
+ * stall the filter streams running beside it.  For them the scratch (twiddle table, pass-1 intermediate, packed
+ * spectrum) lives in a fixed array inside the library image: RBMF_STATIC_SCRATCH_BYTES (12 MiB) on EVERY GPU on which
+ * the library's CUDA module gets loaded, from that load until the process exits, whether or not this call is used.
+ *
+ * The limit.  One call may transform at most RBMF_STATIC_MAX_SAMPLES = 2^20 samples in total: N a power of two,
+ * 2^10 <= N <= 2^20, and n_segments * N <= 2^20 (e.g. one segment of 2^20, two of the Paper configuration's 2^19,
+ * four of the paper's own 2^18 block).  More returns RBMF_ERR_UNSUPPORTED and launches nothing (N outside
+ * [2^10, 2^24] or not a power of two: RBMF_ERR_ARG, as for rbmf_plan_create); split a larger batch into several
+ * calls.  rbmf_prepare_strain_static_limits reports both numbers at run time (either pointer may be NULL).
+ *
+ * Arguments and result are those of rbmf_prepare_strain -- x_dev: n_segments x N float32 (8-byte aligned);
+ * inv_asd_dev: N/2+1 float32 or NULL; strain_out_dev: n_segments x (N/2+1) complex64, 8-byte aligned, not aliasing
+ * x_dev; all caller-owned device memory on the CURRENT device -- with N and the stream (cudaStream_t, NULL = legacy
+ * default stream) given directly.  The output is bit-identical to rbmf_prepare_strain's (same kernels, same table).
+ * Enqueues four kernels (the table for this N, two FFT passes, split + whitening) and returns; *cuda_error (may be
+ * NULL) receives the cudaError_t when the status is RBMF_ERR_CUDA, else 0.
+ *
+ * First call on a device.  The first call made with a given device current looks up the array's address on that
+ * device and sets the kernels' shared-memory attribute there (host-side work, once per device and process, guarded
+ * by a mutex).  Make that first call during start-up, on the device in question, before any stream capture begins.
+ *
+ * Sharing.  All calls on one device use the SAME array, and it keeps what the last call left in it.  The call does
+ * not rely on its contents (everything it reads it has written first, on its own stream, so nothing has to be
+ * cleared), but two calls whose kernels can overlap on the GPU -- different streams without an event between them,
+ * different host threads -- overwrite each other's table and intermediates and produce garbage without any error.
+ * Run them on one stream, or order them with events.  Calls on different GPUs do not interact. */
+#define RBMF_STATIC_MAX_SAMPLES (1 << 20)
+#define RBMF_STATIC_SCRATCH_BYTES (3 * (RBMF_STATIC_MAX_SAMPLES / 2) * 8)
+rbmf_status rbmf_prepare_strain_static(const float* x_dev, const float* inv_asd_dev, int64_t N, int32_t n_segments,
+                                       void* strain_out_dev, void* cuda_stream, int32_t* cuda_error);
+rbmf_status rbmf_prepare_strain_static_limits(int64_t* max_samples, size_t* scratch_bytes);
+
 /* Filter n_segments (1 <= n_segments <= max_batch) segments at once ("filtering each segment in
  * parallel", basis and coefficients loaded once).  strain_dev: n_segments x (N/2+1) complex64, row-major, each row as
  * in rbmf_filter.  Steps a1-a3 run once per (segment, basis column) in ONE persistent launch (no launch gaps or

@@ -10,6 +10,8 @@
 //     each pass a radix-2 decimation-in-time transform in shared memory (bit-reversed load, log2 L in-place stages);
 //   d[j] = E + e^{-2 pi i j / N} O,  E = (Z[j] + conj Z[Nh - j]) / 2,  O = -i (Z[j] - conj Z[Nh - j]) / 2.
 // All twiddles come from one table twF[m] = e^{-2 pi i m / N}, m < N/2, evaluated in fp64 (sincospi).
+#include <mutex>
+
 #include "rbmf_internal.h"
 
 namespace rbmf {
@@ -152,3 +154,95 @@ cudaError_t launch_r2c(const float* x, const float* inv_asd, float2* S, float2* 
 }
 
 }  // namespace rbmf
+
+// =====================================================================================================================
+// rbmf_prepare_strain_static (include/rbmf.h): the front end above for callers that have no device memory to give.
+//
+// rbmf_prepare_strain borrows three scratch arrays from the plan's workspace: the twiddle table twF (N/2 float2), the
+// pass-1 intermediate S and the packed spectrum Z (n_segments N/2 float2 each).  A caller that only conditions strain
+// -- a data-acquisition or whitening stage that feeds several filter processes, a plug-in that runs inside somebody
+// else's pipeline and is handed nothing but its input and output buffers, a process whose framework has already
+// reserved the whole card for its own pool so that a raw cudaMalloc fails, or a low-latency loop in which a cudaMalloc
+// (which synchronises the device) would stall the filter streams running beside it -- has no plan, no workspace and
+// no way to get either.  For them the same three kernels run on a fixed array that is part of the library image:
+// it is created when the library's module is loaded on a GPU and stays until the process exits (12 MiB per GPU).
+//
+// The name `static_scratch` below is a real address only inside device code.  In host code it is the host-side shadow
+// of the symbol; handing that to a kernel would make the kernel write through a host address.  The device address is
+// looked up once per device with cudaGetSymbolAddress (static_device_state) and that pointer is what the kernels get.
+// =====================================================================================================================
+namespace {
+
+constexpr long long kStaticMax = RBMF_STATIC_MAX_SAMPLES;      // samples per call, all segments together
+constexpr long long kStaticPart = kStaticMax / 2;              // float2 entries of each of the three parts
+// [0, kStaticPart): twF   [kStaticPart, 2 kStaticPart): S   [2 kStaticPart, 3 kStaticPart): Z
+static __device__ __align__(256) float2 static_scratch[3 * kStaticPart];
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticDeviceState {
+    bool ready = false;
+    float2* base = nullptr;   // device address of static_scratch on this device
+};
+std::mutex static_mutex;
+StaticDeviceState static_state[kStaticMaxDevices];
+
+// Once per device, with that device current: resolve the array's device address and raise the two passes' dynamic
+// shared-memory limit (a per-device function attribute).  Neither call allocates.
+cudaError_t static_device_state(float2** base) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(static_mutex);
+    StaticDeviceState& s = static_state[dev];
+    if (!s.ready) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, static_scratch);
+        if (e != cudaSuccess) return e;
+        if (p == nullptr || ((uintptr_t)p % 256) != 0) return cudaErrorInvalidSymbol;
+        e = rbmf::r2c_configure();
+        if (e != cudaSuccess) return e;
+        s.base = static_cast<float2*>(p);
+        s.ready = true;
+    }
+    *base = s.base;
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" rbmf_status rbmf_prepare_strain_static_limits(int64_t* max_samples, size_t* scratch_bytes) {
+    if (max_samples) *max_samples = kStaticMax;
+    if (scratch_bytes) *scratch_bytes = sizeof(float2) * 3 * (size_t)kStaticPart;
+    return RBMF_OK;
+}
+
+extern "C" rbmf_status rbmf_prepare_strain_static(const float* x_dev, const float* inv_asd_dev, int64_t N,
+                                                  int32_t n_segments, void* strain_out_dev, void* cuda_stream,
+                                                  int32_t* cuda_error) {
+    if (cuda_error) *cuda_error = 0;
+    if (!x_dev || !strain_out_dev || n_segments < 1) return RBMF_ERR_ARG;
+    if (N < (1ll << 10) || N > (1ll << 24) || (N & (N - 1)) != 0) return RBMF_ERR_ARG;
+    if (((uintptr_t)x_dev % 8) != 0 || ((uintptr_t)strain_out_dev % 8) != 0) return RBMF_ERR_ARG;
+    // the limit: every segment of the call must fit the fixed array at once
+    if (N > kStaticMax || (long long)n_segments > kStaticMax / N) return RBMF_ERR_UNSUPPORTED;
+    int logN = 0;
+    while ((1ll << logN) < N) ++logN;
+    float2* base = nullptr;
+    cudaError_t e = static_device_state(&base);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    float2* twF = base;
+    float2* S = base + kStaticPart;
+    float2* Z = base + 2 * kStaticPart;
+    // The array still holds whatever the previous call (any N, any stream) left in it.  Nothing here needs zeros: the
+    // table is rewritten for this N on this stream, pass 1 writes every entry of S that pass 2 reads, and pass 2 every
+    // entry of Z that the split reads.
+    if (e == cudaSuccess) e = rbmf::launch_r2c_table(twF, N, st);
+    if (e == cudaSuccess) e = rbmf::launch_r2c(x_dev, inv_asd_dev, S, Z, static_cast<float2*>(strain_out_dev), twF, logN,
+                                               n_segments, st);
+    if (e != cudaSuccess) {
+        if (cuda_error) *cuda_error = (int32_t)e;
+        return RBMF_ERR_CUDA;
+    }
+    return RBMF_OK;
+}

@@ -46,6 +46,8 @@ SIGNATURES = {
     "rbmf_set_coeffs": (_i32, [_vp, _vp, _vp]),
     "rbmf_filter": (_i32, [_vp, _vp, _f32, _f32, _vp, _vp]),
     "rbmf_prepare_strain": (_i32, [_vp, _vp, _vp, _i32, _vp]),
+    "rbmf_prepare_strain_static": (_i32, [_vp, _vp, _i64, _i32, _vp, _vp, _pi32]),
+    "rbmf_prepare_strain_static_limits": (_i32, [_pi64, _psz]),
     "rbmf_prepare_basis_workspace_bytes": (_i32, [_i32, _i32, _psz]),
     "rbmf_prepare_basis": (_i32, [_vp, _i32, _i64, _f64, _f64, _i32, _i32, ctypes.c_uint64, _vp, ctypes.c_size_t, _vp, _vp,
                                   _vp]),
@@ -93,6 +95,43 @@ def _ptr(t):
     if isinstance(t, np.ndarray):
         return t.ctypes.data
     return t.data_ptr()
+
+
+def prepare_strain_static(x_dev, inv_asd_dev=None, out=None, stream=None):
+    """rbmf_prepare_strain_static: time series -> whitened spectrum without a plan and without a workspace.
+
+    For code that may not (or cannot) allocate GPU memory for the library -- a whitening stage with no plan of its
+    own, a callback inside somebody else's pipeline that only gets its input and output buffers, a process whose
+    memory pool already owns the whole card -- the scratch of the transform is a fixed 12 MiB array inside librbmf.so.
+    x_dev: contiguous float32 CUDA tensor (n_segments, N), N a power of two in [2^10, 2^20], n_segments * N <= 2^20
+    (RbmfError with RBMF_ERR_UNSUPPORTED beyond that: split the batch); inv_asd_dev: (N/2+1,) float32 or None;
+    out: a preallocated (n_segments, N/2+1) complex64 CUDA tensor (allocated with torch when None -- pass it if the
+    point is to allocate nothing); stream: a torch stream (default: torch's current one).  Asynchronous.  Same values,
+    bit for bit, as Plan.prepare_strain.  All calls on a device share the one array: keep them on one stream or order
+    them with events, and make the first call on each device before any stream capture."""
+    import torch
+    if x_dev.dtype != torch.float32 or x_dev.dim() != 2 or not x_dev.is_cuda or not x_dev.is_contiguous():
+        raise ValueError("x must be a contiguous float32 CUDA tensor of shape (n_segments, N)")
+    nb, N = int(x_dev.shape[0]), int(x_dev.shape[1])
+    if inv_asd_dev is not None and (inv_asd_dev.dtype != torch.float32 or inv_asd_dev.numel() != N // 2 + 1
+                                    or inv_asd_dev.device != x_dev.device or not inv_asd_dev.is_contiguous()):
+        raise ValueError("inv_asd must be a contiguous float32 CUDA tensor with N/2+1 entries on x's device")
+    if out is None:
+        out = torch.empty((nb, N // 2 + 1), dtype=torch.complex64, device=x_dev.device)
+    elif out.dtype != torch.complex64 or tuple(out.shape) != (nb, N // 2 + 1) or out.device != x_dev.device \
+            or not out.is_contiguous():
+        raise ValueError("out must be a contiguous complex64 CUDA tensor of shape (n_segments, N/2+1) on x's device")
+    with torch.cuda.device(x_dev.device):
+        cur = torch.cuda.current_stream()
+        st = stream if stream is not None else cur
+        if st != cur:
+            st.wait_stream(cur)      # tensors the caller has just produced on the current stream
+        err = _i32(0)
+        status = _lib.rbmf_prepare_strain_static(_ptr(x_dev), _ptr(inv_asd_dev), N, nb, _ptr(out), st.cuda_stream,
+                                                 ctypes.byref(err))
+    if status != RBMF_OK:
+        raise RbmfError(status, "rbmf_prepare_strain_static", err.value)
+    return out
 
 
 class Plan:
