@@ -26,7 +26,10 @@ __global__ void __launch_bounds__(256) cgemm_kernel(const float2* __restrict__ A
                                                     long long ldc, int M, int N, long long p0, long long p1) {
     __shared__ float2 sA[TK][TM + 1];
     __shared__ float2 sB[TK][TN + 1];
-    const int i0 = blockIdx.y * TM, j0 = blockIdx.x * TN;
+    // one-dimensional grid over the (row tile, column tile) pairs, column tiles fastest: M may be 2^24 templates
+    // (rbmf_prepare_coeffs), far more row tiles than gridDim.y allows
+    const int ntn = (N + TN - 1) / TN;
+    const int i0 = (int)(blockIdx.x / ntn) * TM, j0 = (int)(blockIdx.x % ntn) * TN;
     const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
     float2 acc[4][4];
     double2 dacc[4][4];
@@ -181,8 +184,9 @@ __global__ void prep_sigma_kernel(const float2* __restrict__ coeffs, float* __re
 template <bool NN>
 cudaError_t cgemm(const float2* A, long long lda, const float2* B, long long ldb, float2* C, long long ldc, int M, int N,
                   long long p0, long long p1, cudaStream_t st) {
-    dim3 grid((N + TN - 1) / TN, (M + TM - 1) / TM);
-    cgemm_kernel<NN><<<grid, 256, 0, st>>>(A, lda, B, ldb, C, ldc, M, N, p0, p1);
+    const long long tiles = (long long)((N + TN - 1) / TN) * ((M + TM - 1) / TM);
+    if (tiles < 1 || tiles > 0x7fffffffll) return cudaErrorInvalidConfiguration;
+    cgemm_kernel<NN><<<(unsigned)tiles, 256, 0, st>>>(A, lda, B, ldb, C, ldc, M, N, p0, p1);
     return cudaGetLastError();
 }
 
@@ -199,20 +203,28 @@ cudaError_t orthonormalise_rows(float2* Q, long long ld, long long n, int nrows,
             if (e != cudaSuccess) return e;
             gs_dots_kernel<<<dim3(j, splits), 256, 0, st>>>(Q, ld, w, n, r);
             gs_update_kernel<<<gn, 256, 0, st>>>(Q, ld, w, n, r, j);
+            if ((e = cudaGetLastError()) != cudaSuccess) return e;
         }
         cudaError_t e = cudaMemsetAsync(nrm2, 0, sizeof(double), st);
         if (e != cudaSuccess) return e;
         gs_norm_kernel<<<gn < 1024 ? gn : 1024, 256, 0, st>>>(w, n, nrm2);
         gs_scale_kernel<<<gn < 1024 ? gn : 1024, 256, 0, st>>>(w, n, nrm2, norms ? norms + j : nullptr);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
-    return cudaGetLastError();
+    return cudaSuccess;
 }
 
 }  // namespace
 
+// Bytes of the float2 part of the workspace (G, Va, Vb), rounded up to 16: the Gram-Schmidt scratch behind it is read
+// as double2 (128-bit loads), and S (S + 2k) float2 entries are 8 mod 16 bytes when the number of templates S is odd.
+static size_t prep_vectors_bytes(int S, int k) {
+    return (((size_t)S * S + 2ull * k * S) * sizeof(float2) + 15) & ~(size_t)15;
+}
+
 size_t prep_basis_workspace_bytes(int S, int k) {
     // G (S x S) + two sets of k row vectors of length S + Gram-Schmidt scratch
-    return ((size_t)S * S + 2ull * k * S) * sizeof(float2) + (size_t)k * sizeof(double2) + 1024;
+    return prep_vectors_bytes(S, k) + (size_t)k * sizeof(double2) + 1024;
 }
 
 // templates: S x bins (rows), band [j_low, n_half); basis_out: k x bins.  eig_out (optional): k floats, the lengths
@@ -223,7 +235,7 @@ cudaError_t launch_prep_basis(const float2* templates, int S, long long bins, in
     float2* G = reinterpret_cast<float2*>(workspace);
     float2* Va = G + (size_t)S * S;       // k x S: rows = conj of the iteration vectors (V^H)
     float2* Vb = Va + (size_t)k * S;
-    double2* r = reinterpret_cast<double2*>(Vb + (size_t)k * S);
+    double2* r = reinterpret_cast<double2*>(reinterpret_cast<char*>(workspace) + prep_vectors_bytes(S, k));
     double* nrm2 = reinterpret_cast<double*>(r + k);
     cudaError_t e;
     // C = T T^H over the band

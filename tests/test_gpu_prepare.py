@@ -69,3 +69,29 @@ def test_prepared_inputs_through_the_path(rbmf):
     # the prepared basis captures what the generator's fp64 SVD basis of the same size captures, to 1 %
     cap = float((sigma_dev.double() ** 2).mean())
     assert cap > 0.99 * wl["captured"], (cap, wl["captured"])
+
+
+@pytest.mark.parametrize("S,k", [(33, 16), (57, 32)])
+def test_prepare_basis_with_an_odd_number_of_templates(rbmf, S, k):
+    """An odd number of templates puts the end of the float2 part of the workspace (S (S + 2k) entries) at 8 mod 16
+    bytes; the Gram-Schmidt coefficients behind it are read with 128-bit loads and used to fault there.
+    Same checks as above: orthonormal rows, zero outside the band, and the power the exact PCA basis captures."""
+    import torch
+    wl = wlm.make_workload(wlm.CONFIGS["tiny"], device="cuda")
+    cfg = wl["config"]
+    assert S % 2 == 1 and S <= cfg.T
+    U32 = wlm.bank_templates(wl, np.arange(S), device="cuda").astype(np.complex64)
+    tpl = torch.from_numpy(U32).cuda()
+    basis_dev, eig = rbmf.prepare_basis(tpl, cfg.N, cfg.fs, cfg.f_low, k, iterations=40, seed=11)
+    coeffs_dev, sigma_dev = rbmf.prepare_coeffs(tpl, basis_dev, cfg.N, cfg.fs, cfg.f_low)
+    torch.cuda.synchronize()
+    B = basis_dev.cpu().numpy().astype(np.complex128)
+    assert np.abs(B @ B.conj().T - np.eye(k)).max() < 2e-5
+    assert not B[:, :cfg.j_low].any() and not B[:, cfg.N // 2:].any()
+    ref_c = U32.astype(np.complex128) @ B.conj().T
+    assert np.abs(coeffs_dev.cpu().numpy() - ref_c).max() < 2e-6
+    exact_basis, _, sv = orc.pca_basis(U32.astype(np.complex128), k)
+    cap, cap_exact = orc.captured_power(U32, B), orc.captured_power(U32, exact_basis)
+    assert cap <= cap_exact + 1e-6 and cap >= cap_exact * (1.0 - 2e-3), (cap, cap_exact)
+    lam = np.sort(eig.cpu().numpy())[::-1]
+    assert np.abs(lam[:4] - sv[:4] ** 2).max() < 2e-2 * sv[0] ** 2
