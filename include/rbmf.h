@@ -14,7 +14,7 @@
  * with s = sqrt(2/N), d = unnormalised forward DFT of the whitened unit-variance strain, b_k orthonormal
  * over the band, c_tk the decomposition coefficients.  Every step runs in hand-written CUDA
  * kernels for sm_100a (a persistent, TMA-fed batched four-step Stockham FFT; a tcgen05/TMEM GEMM -- fp16 screen with a
- * proven error bound by default, split-bf16 on request -- with a fused threshold/compaction epilogue; a re-scoring
+ * derived error bound by default, split-bf16 on request -- with a fused threshold/compaction epilogue; a re-scoring
  * kernel that regroups the candidates by bin, scores them from a shared-memory copy of the bin's block of beta and
  * also confirms the screen's hits in fp32).  There is no CPU fallback.
  * Around that path: batches of segments and the step in front of the path (rbmf_filter_batch,
@@ -73,8 +73,10 @@ typedef enum {
 typedef enum {
     RBMF_GEMM_TCGEN05 = 0, /* TMA + tcgen05.mma, bf16x3 split precision (fp32-equivalent) + TMEM epilogue          */
     RBMF_GEMM_SCREEN = 2   /* default: the same tensor-core kernel with ONE fp16 product per term and thr_stage1
-                              lowered, per (bin, template block), by a rigorous bound of the fp16 error, so its
-                              output is a superset of the true candidates; kernel 3 then repeats the stage-1 test at
+                              lowered, per (bin, template block), by a derived bound of the fp16 error (operand
+                              rounding is exact analysis; the tensor core's fp32 accumulation term is an assumption
+                              verified on the device, largest observed error / bound 0.56), so its output is a
+                              superset of the true candidates; kernel 3 then repeats the stage-1 test at
                               fp32 accuracy (the mean of the w fp32 samples it computes anyway is the averaged SNR of
                               Eq. 9) before scoring.  Same candidate and trigger sets as RBMF_GEMM_TCGEN05 up to
                               fp32 rounding at the threshold, one third of the tensor-core work.               */
@@ -239,8 +241,10 @@ rbmf_status rbmf_filter_flat(rbmf_plan* plan, const void* strain_dev, float thr,
  * all sub-banks append to ONE trigger list out_dev (capacity max_triggers) through one shared position counter
  * n_out_dev (device int64: total found, may exceed max_triggers), with template_id = (sum of T of the sub-banks before
  * it in `plans`) + the template's row in its own sub-bank.  The result equals the union of rbmf_filter over the plans.
- * The plans must not be used by other calls while a bank-set call is in flight; the set does not own them (destroy the
- * set first).  rbmf_bankset_get_counts synchronises and returns per-sub-bank candidates / triggers (arrays of n_plans,
+ * Ordering: every sub-bank's work starts after what has been enqueued so far on `cuda_stream` (the producer of the
+ * strain) AND on that plan's own stream (rbmf_set_basis / rbmf_set_coeffs, an earlier rbmf_filter); `cuda_stream`
+ * continues after all sub-banks.  The plans' own streams are NOT made to wait for the bank-set call: the plans must not
+ * be used by other calls while a bank-set call is in flight; the set does not own them (destroy the set first).  rbmf_bankset_get_counts synchronises and returns per-sub-bank candidates / triggers (arrays of n_plans,
  * may be NULL) and the total; RBMF_ERR_OVERFLOW if a sub-bank's candidate list overflowed. */
 typedef struct rbmf_bankset rbmf_bankset;
 rbmf_status rbmf_bankset_create(rbmf_bankset** out, rbmf_plan* const* plans, int32_t n_plans);
@@ -325,11 +329,23 @@ int32_t rbmf_last_cuda_error(const rbmf_plan* plan);
  *       clusters of 2); takes effect at the next rbmf_filter;
  *   RBMF_DIAG_STAGE2_PER_CANDIDATE (value 0/1): step a6 with the one-warp-per-candidate kernel (the fallback for
  *       w = 32 with k > 608, where one bin's block of beta does not fit in shared memory) instead of the kernel that
- *       regroups the candidates by bin. */
+ *       regroups the candidates by bin.
+ * Scheduling overrides (results are unchanged, only the order of the work; they replace the RBMF_FFT_SEG_MAJOR,
+ * RBMF_FFT_LOOKAHEAD and RBMF_GEMM_GROUP environment variables of earlier builds -- the library reads no environment
+ * variable any more); they take effect at the next rbmf_filter:
+ *   RBMF_DIAG_FFT_CHUNK_MAJOR (value 0/1): a batch's FFT work runs basis-chunk-major (a chunk of 4 basis columns is
+ *       read once for all segments) instead of segment-major, the measured-faster default;
+ *   RBMF_DIAG_FFT_LOOKAHEAD (value 1..256, 0 = automatic): basis chunks whose first FFT pass may run ahead of the
+ *       second pass in kernel 1's work queue (their intermediates must fit in L2);
+ *   RBMF_DIAG_GEMM_GROUP (value >= 1, 0 = automatic): template blocks per raster group of kernel 2 (the group's
+ *       coefficient tiles stay L2-resident while the beta^avg planes stream past once per group). */
 typedef enum {
     RBMF_DIAG_STAGE1_FP32_CHECK = 1,
     RBMF_DIAG_SINGLE_CTA_SCREEN = 2,
-    RBMF_DIAG_STAGE2_PER_CANDIDATE = 3
+    RBMF_DIAG_STAGE2_PER_CANDIDATE = 3,
+    RBMF_DIAG_FFT_CHUNK_MAJOR = 4,
+    RBMF_DIAG_FFT_LOOKAHEAD = 5,
+    RBMF_DIAG_GEMM_GROUP = 6
 } rbmf_diag_option;
 rbmf_status rbmf_diag_set(rbmf_plan* plan, int32_t option, int32_t value);
 

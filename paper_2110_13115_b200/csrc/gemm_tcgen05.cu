@@ -368,7 +368,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(buf * BN);
             const int bin = ib * BM + row;
-            // MODE 0: the stage-1 threshold itself.  MODE 1: thr1 lowered by a rigorous bound of the fp16 screen's
+            // MODE 0: the stage-1 threshold itself.  MODE 1: thr1 lowered by the derived bound of the fp16 screen's
             // error for this (bin, template block), so that no true candidate can be missed (see file header).
             float thr_sq = g.thr1_sq;
             if (MODE == 1) {

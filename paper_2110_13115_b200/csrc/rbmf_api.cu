@@ -48,6 +48,7 @@ struct rbmf_plan {
     int gemm_impl;
     int last_impl;      // gemm_impl of the last rbmf_filter (decides which candidate list / counter is final)
     int diag_fp32_check, diag_single_cta, diag_stage2_per_cand;   // rbmf_diag_set
+    int diag_fft_chunk_major, diag_fft_lookahead, diag_gemm_group;   // rbmf_diag_set: scheduling overrides, 0 = automatic
     int timing;
     cudaStream_t stream;
     uint8_t* ws;
@@ -448,6 +449,10 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     if (!(thr_stage1 > 0.f) || !(thr_stage2 > 0.f)) return RBMF_ERR_ARG;
     if (n_segments < 1 || n_segments > plan->max_batch) return RBMF_ERR_ARG;
     if (!plan->have_ws || !plan->have_basis || !plan->have_coeffs) return RBMF_ERR_STATE;
+    // every argument and state check comes before the first launch: a refused call leaves the plan's arrays untouched
+    const bool by_templates = plan->stage1_route == RBMF_STAGE1_TEMPLATES;
+    if (by_templates && n_segments != 1) return RBMF_ERR_UNSUPPORTED;
+    if (by_templates && !plan->have_templates) return RBMF_ERR_STATE;
     const Layout& L = plan->lay;
     cudaStream_t st = plan->stream;
     const bool tm = plan->timing != 0;
@@ -477,8 +482,7 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     // Batches run segment-major (every segment streams the basis from HBM again): keeping a basis chunk in L2 for the
     // other segments (chunk-major) displaces the in-place intermediate Y and measured 5-10 % slower per segment at
     // every size (Small B = 8: 0.74 vs 0.70 ms; Paper B = 4: 3.69 vs 3.37 ms) -- the kernel is not bound by that stream.
-    a.seg_major = 1;
-    if (const char* e = getenv("RBMF_FFT_SEG_MAJOR")) a.seg_major = atoi(e) ? 1 : 0;   // developer switch
+    a.seg_major = plan->diag_fft_chunk_major ? 0 : 1;
     {
         // Pass-1 lookahead: a chunk's pass 2 needs ALL of its pass-1 tiles, so enough pass-1 tiles of later chunks
         // must be queued to keep every consumer group (2 per SM) busy meanwhile -- about two tiles per group --,
@@ -488,12 +492,10 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
         const long long cap = (48ll << 20) / ((long long)plan->N * kFftC * 8) - 1;
         if (la > cap) la = cap;
         if (la < 1) la = 1;
-        if (const char* e = getenv("RBMF_FFT_LOOKAHEAD")) { const int v = atoi(e); if (v >= 1) la = v; }   // developer switch
+        if (plan->diag_fft_lookahead >= 1) la = plan->diag_fft_lookahead;
         a.lookahead = (int)la;
     }
     CK(launch_fft_tma(plan->tmY, a, plan->logN1, plan->logN2, plan->fft_grid, st));
-    const bool by_templates = plan->stage1_route == RBMF_STAGE1_TEMPLATES;
-    if (by_templates && (nb != 1 || !plan->have_templates)) return nb != 1 ? RBMF_ERR_UNSUPPORTED : RBMF_ERR_STATE;
     if (screen && !by_templates)
         CK(launch_bin_norm(at<uint16_t>(plan, L.bavg_hi), at<float>(plan, L.bin_norm), (int)Mtot, (int)Mplane,
                            (plan->k + 31) / 32, st));
@@ -519,7 +521,7 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
         long long grp = (long long)((size_t)(48u << 20) / tile_bytes);
         g.group = (int)(grp < 8 ? 8 : (grp > g.num_tb ? g.num_tb : grp));
     }
-    if (const char* e = getenv("RBMF_GEMM_GROUP")) { const int v = atoi(e); if (v >= 1) g.group = v; }   // developer switch
+    if (plan->diag_gemm_group >= 1) g.group = plan->diag_gemm_group;
     if (by_templates) {
         // the paper's fast first stage by templates (Eq. 10-12) in the place of the GEMM; exact fp32 candidates
         rbmf_status s1 = stage1_by_templates(plan, (const float2*)strain_dev, thr_stage1);
@@ -666,6 +668,15 @@ rbmf_status rbmf_diag_set(rbmf_plan* plan, int32_t option, int32_t value) {
         case RBMF_DIAG_STAGE1_FP32_CHECK: plan->diag_fp32_check = value ? 1 : 0; return RBMF_OK;
         case RBMF_DIAG_SINGLE_CTA_SCREEN: plan->diag_single_cta = value ? 1 : 0; return RBMF_OK;
         case RBMF_DIAG_STAGE2_PER_CANDIDATE: plan->diag_stage2_per_cand = value ? 1 : 0; return RBMF_OK;
+        case RBMF_DIAG_FFT_CHUNK_MAJOR: plan->diag_fft_chunk_major = value ? 1 : 0; return RBMF_OK;
+        case RBMF_DIAG_FFT_LOOKAHEAD:
+            if (value < 0 || value > kMaxChunks) return RBMF_ERR_ARG;
+            plan->diag_fft_lookahead = value;
+            return RBMF_OK;
+        case RBMF_DIAG_GEMM_GROUP:
+            if (value < 0) return RBMF_ERR_ARG;
+            plan->diag_gemm_group = value;
+            return RBMF_OK;
         default: return RBMF_ERR_ARG;
     }
 }
@@ -841,6 +852,7 @@ struct rbmf_bankset {
     int nstreams;
     cudaStream_t streams[4];
     cudaEvent_t fork, join[4];
+    cudaEvent_t plan_ready;   // re-recorded per sub-bank on the plan's own stream: its set-up work precedes the filter
     cudaStream_t last_stream;
     unsigned long long* last_counter;
     bool filtered;
@@ -882,6 +894,7 @@ rbmf_status rbmf_bankset_create(rbmf_bankset** out, rbmf_plan* const* plans, int
     b->nstreams = n_plans < 4 ? n_plans : 4;
     rbmf_plan* plan = plans[0];   // for CK's error slot
     cudaError_t e = cudaEventCreateWithFlags(&b->fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&b->plan_ready, cudaEventDisableTiming);
     for (int i = 0; i < b->nstreams && e == cudaSuccess; ++i) {
         e = cudaStreamCreateWithFlags(&b->streams[i], cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&b->join[i], cudaEventDisableTiming);
@@ -903,6 +916,10 @@ rbmf_status rbmf_bankset_filter(rbmf_bankset* bs, const void* strain_dev, float 
     for (int q = 0; q < bs->n && result == RBMF_OK; ++q) {
         rbmf_plan* p = bs->plans[bs->order[q]];
         cudaStream_t saved = p->stream;
+        // what the caller has enqueued on the plan's own stream (rbmf_set_basis / rbmf_set_coeffs, an earlier
+        // rbmf_filter) comes first: the internal streams are non-blocking and ordered against `cuda_stream` only
+        CK(cudaEventRecord(bs->plan_ready, saved));
+        CK(cudaStreamWaitEvent(bs->streams[q % bs->nstreams], bs->plan_ready, 0));
         p->stream = bs->streams[q % bs->nstreams];
         p->shared_trig_counter = (unsigned long long*)n_out_dev;
         p->shared_trig_cap = (unsigned long long)max_triggers;
@@ -954,6 +971,7 @@ rbmf_status rbmf_bankset_destroy(rbmf_bankset* bs) {
         if (bs->join[i]) cudaEventDestroy(bs->join[i]);
     }
     if (bs->fork) cudaEventDestroy(bs->fork);
+    if (bs->plan_ready) cudaEventDestroy(bs->plan_ready);
     delete[] bs->plans; delete[] bs->order; delete[] bs->offsets;
     delete bs;
     return RBMF_OK;

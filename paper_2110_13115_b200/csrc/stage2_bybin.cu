@@ -18,6 +18,8 @@
 // averaged SNR of Eq. 9 (linearity), so the stage-1 test is repeated on it at fp32 accuracy and
 // the confirmed candidates go to their own list before the thr_stage2 test.
 // Batches: a bin index runs over all segments, bin = b Mseg + i, and time_index = bin w + r = b N + n.
+#include <mutex>
+
 #include "rbmf_internal.h"
 
 namespace rbmf {
@@ -238,12 +240,24 @@ __global__ void __launch_bounds__(NWARP * 32, 4) stage2_score_kernel(const Stage
 
 template <int W, int G, int CU>
 cudaError_t launch_score_cu(const Stage2Args& a, int num_sms, cudaStream_t st) {
-    static int configured = 0;   // largest dynamic shared memory size this instantiation has been set up for
-    if (a.smem_bytes > configured) {
-        cudaError_t e = cudaFuncSetAttribute(stage2_score_kernel<W, G, CU>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             a.smem_bytes > 48 * 1024 ? a.smem_bytes : 48 * 1024);
-        if (e != cudaSuccess) return e;
-        configured = a.smem_bytes > 48 * 1024 ? a.smem_bytes : 48 * 1024;
+    // Largest dynamic shared memory size this instantiation has been set up for, PER DEVICE (a function attribute
+    // belongs to the device that was current when it was set: one process-wide flag left a second GPU unconfigured),
+    // under a mutex so that two host threads cannot leave the record above the attribute actually in force.
+    constexpr int kDevices = 64;
+    static std::mutex mu;
+    static int configured[kDevices] = {};
+    const int want = a.smem_bytes > 48 * 1024 ? a.smem_bytes : 48 * 1024;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        const bool known = dev >= 0 && dev < kDevices;
+        if (!known || want > configured[dev]) {
+            e = cudaFuncSetAttribute(stage2_score_kernel<W, G, CU>, cudaFuncAttributeMaxDynamicSharedMemorySize, want);
+            if (e != cudaSuccess) return e;
+            if (known) configured[dev] = want;
+        }
     }
     int per_sm = (200 * 1024) / (a.smem_bytes + 14 * 1024);
     per_sm = per_sm < 1 ? 1 : (per_sm > 6 ? 6 : per_sm);

@@ -26,6 +26,7 @@ RBMF_OK, RBMF_ERR_ARG, RBMF_ERR_STATE, RBMF_ERR_CUDA, RBMF_ERR_OVERFLOW, RBMF_ER
 RBMF_GEMM_TCGEN05, RBMF_GEMM_SCREEN = 0, 2
 RBMF_STAGE1_BASIS, RBMF_STAGE1_TEMPLATES = 0, 1
 RBMF_DIAG_STAGE1_FP32_CHECK, RBMF_DIAG_SINGLE_CTA_SCREEN, RBMF_DIAG_STAGE2_PER_CANDIDATE = 1, 2, 3
+RBMF_DIAG_FFT_CHUNK_MAJOR, RBMF_DIAG_FFT_LOOKAHEAD, RBMF_DIAG_GEMM_GROUP = 4, 5, 6
 
 TRIGGER_DTYPE = np.dtype([("template", np.int32), ("time", np.int32), ("re", np.float32), ("im", np.float32)])
 CANDIDATE_DTYPE = np.dtype([("template", np.int32), ("bin", np.int32), ("re", np.float32), ("im", np.float32)])
@@ -476,7 +477,6 @@ class BankSet:
         self.stream = stream if stream is not None else self.plans[0].stream
         self._h = _vp()
         arr = (_vp * len(self.plans))(*[p._h for p in self.plans])
-        torch.cuda.synchronize(self.device)          # every plan's set-up work is complete
         with torch.cuda.device(self.device):
             st = _lib.rbmf_bankset_create(ctypes.byref(self._h), arr, len(self.plans))
         if st != RBMF_OK:
@@ -486,6 +486,11 @@ class BankSet:
             self._n_out = torch.zeros(1, dtype=torch.int64, device=self.device)
 
     def filter_async(self, strain_dev, thr1, thr2):
+        # the strain may have been produced on torch's current stream: order the set's stream after it, as
+        # Plan._order_after_current does (the library orders the sub-banks after the set's stream and the plans' own)
+        cur = self._torch.cuda.current_stream(self.device)
+        if cur.cuda_stream != self.stream.cuda_stream:
+            self.stream.wait_stream(cur)
         with self._torch.cuda.device(self.device):
             st = _lib.rbmf_bankset_filter(self._h, _ptr(strain_dev), float(thr1), float(thr2), _ptr(self._out),
                                           self.max_triggers, _ptr(self._n_out), _vp(self.stream.cuda_stream))

@@ -101,6 +101,14 @@ def test_window_capacity_and_workspace_size(binding):
     assert b.rbmf_workspace_bytes(h, ctypes.byref(nbytes)) == b.RBMF_OK and nbytes.value > before.value
     assert b.rbmf_plan_set_gemm_impl(h, b.RBMF_GEMM_SCREEN) == b.RBMF_OK
     assert b.rbmf_diag_set(h, 99, 1) == b.RBMF_ERR_ARG
+    # scheduling overrides (formerly environment variables read inside rbmf_filter_batch): validated, 0 = automatic
+    assert b.rbmf_diag_set(h, b.RBMF_DIAG_FFT_CHUNK_MAJOR, 1) == b.RBMF_OK
+    assert b.rbmf_diag_set(h, b.RBMF_DIAG_FFT_CHUNK_MAJOR, 0) == b.RBMF_OK
+    for opt, bad in ((b.RBMF_DIAG_FFT_LOOKAHEAD, (-1, 257)), (b.RBMF_DIAG_GEMM_GROUP, (-1,))):
+        for v in bad:
+            assert b.rbmf_diag_set(h, opt, v) == b.RBMF_ERR_ARG
+        assert b.rbmf_diag_set(h, opt, 3) == b.RBMF_OK
+        assert b.rbmf_diag_set(h, opt, 0) == b.RBMF_OK
     assert b.rbmf_diag_set(h, b.RBMF_DIAG_STAGE1_FP32_CHECK, 1) == b.RBMF_OK
     assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 6
     assert b.rbmf_diag_set(h, b.RBMF_DIAG_STAGE1_FP32_CHECK, 0) == b.RBMF_OK

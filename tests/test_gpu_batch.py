@@ -225,6 +225,28 @@ def test_guarded_calls_repeat_bit_exact(rbmf):
     plan.close()
 
 
+def test_scheduling_overrides_change_the_order_not_the_result(rbmf):
+    """RBMF_DIAG_FFT_CHUNK_MAJOR / _FFT_LOOKAHEAD / _GEMM_GROUP (rbmf_diag_set; environment variables in earlier
+    builds) only reorder the work: beta is bit-identical, candidates and triggers are the same sets."""
+    wl = workload("mini")
+    import torch
+    nb, thr = 3, (3.0, 4.0)
+    strains = torch.from_numpy(strains_of(wl, nb)).cuda()
+    results = []
+    for chunk_major, lookahead, group in ((0, 0, 0), (1, 1, 1), (0, 3, 2)):
+        plan = make_plan(rbmf, wl, max_batch=nb)
+        plan.diag_set(rbmf.RBMF_DIAG_FFT_CHUNK_MAJOR, chunk_major)
+        plan.diag_set(rbmf.RBMF_DIAG_FFT_LOOKAHEAD, lookahead)
+        plan.diag_set(rbmf.RBMF_DIAG_GEMM_GROUP, group)
+        plan.filter_batch_async(strains, *thr)
+        trig = np.sort(plan.triggers(), order=("template", "time"))
+        cand = np.sort(plan.candidates(), order=("template", "bin"))
+        results.append((trig.tobytes(), cand.tobytes(), plan.internal("beta", segment=nb - 1).tobytes()))
+        assert len(trig) > 100
+        plan.close()
+    assert results[1] == results[0] and results[2] == results[0]
+
+
 # ------------------------------------------------------------------------------------- the step before the path
 @pytest.mark.parametrize("N", [1024, 2048, 16384, 131072, 1 << 20])
 def test_prepare_strain_against_oracle(rbmf, N):

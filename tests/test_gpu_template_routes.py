@@ -151,3 +151,26 @@ def test_template_routes_argument_checks(rbmf):
     assert b.rbmf_filter_flat(h, dummy, 5.0, dummy, dummy) == b.RBMF_ERR_STATE
     assert b.rbmf_set_templates(h, dummy, None) == b.RBMF_ERR_STATE
     b.rbmf_plan_destroy(h)
+
+
+def test_refused_template_route_call_launches_nothing(rbmf):
+    """rbmf_filter with RBMF_STAGE1_TEMPLATES selected but no templates set is a call-order error.  It must be refused
+    BEFORE the first launch (it used to be noticed after the FFT kernel had been enqueued): beta of the previous,
+    successful call is still there byte for byte although the refused call was given a different strain, and the
+    previous call's lists are still readable."""
+    import torch
+    wl = workload("tiny")
+    cfg = wl["config"]
+    plan = make_plan(rbmf, wl, 4, 16)
+    first = plan.filter(torch.from_numpy(wl["strain"]), 3.0, 4.0)
+    beta = plan.internal("beta").tobytes()
+    plan.set_stage1_route(rbmf.RBMF_STAGE1_TEMPLATES)
+    other = torch.from_numpy(np.ascontiguousarray(wl["strain"][::-1] * 2.0))
+    with pytest.raises(rbmf.RbmfError) as info:
+        plan.filter(other, 3.0, 4.0)
+    assert info.value.status == rbmf.RBMF_ERR_STATE
+    torch.cuda.synchronize()
+    assert plan.internal("beta").tobytes() == beta
+    assert np.array_equal(np.sort(plan.triggers(), order=("template", "time")),
+                          np.sort(first, order=("template", "time")))
+    plan.close()
