@@ -41,7 +41,11 @@ Pins (tests/test_oracle_pins.py, all `-m "not gpu"`):
   tuning, Eq. 16               hand-built lists with the answer worked out by counting; w = 1 recovers everything
   forward transform, whitening literal O(N^2) sum at small N, a cosine's closed form (N/2 at its bin), Parseval; batches:
                                segment b of `oracle_filter_batch` against the time-domain brute force on strain b alone
-Parity status: every function below is pinned by at least one of these; nothing is "parity unpinned".
+Parity status: every function on the path is pinned by at least one of these.
+PARITY UNPINNED: `z_total` (Eq. 15).  The paper prints no value of Eq. 15 that its own formula
+reproduces (the quoted speed-ups ~6 / ~10 of PAPER.md:316 are matched by Eq. 14 alone, which is what pins `z_first`;
+with the p / T term of Eq. 15 they are not reached), so the only check of `z_total` is that it is the sum of its terms,
+which restates the formula.  It is a three-line calculator off the hot path; no kernel is compared with it.
 """
 from __future__ import annotations
 

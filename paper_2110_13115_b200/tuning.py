@@ -30,16 +30,16 @@ def _counts_at_least(mods, grid):
 
 
 def rho_target(n_final, n_flat, grid, ratio=0.99):
-    """Eq. 16 on cumulative counts: first grid value from which n_final >= ratio n_flat holds for every larger grid
-    value (and flat triggers exist); None if never."""
-    ok = np.asarray(n_final) >= ratio * np.asarray(n_flat)
-    target = None
-    for i in range(len(grid) - 1, -1, -1):
-        if not ok[i]:
-            break
-        if n_flat[i] > 0:
-            target = float(grid[i])
-    return target
+    """Eq. 16 on the cumulative counts n_final[i], n_flat[i] = triggers with |rho| >= grid[i]
+    (ascending grid): the smallest threshold with flat triggers above which the hierarchical search keeps at least
+    `ratio` of the flat triggers at EVERY grid value -- a threshold that passes below one that fails does not count.
+    None if there is no such threshold."""
+    kept = np.asarray(n_final, dtype=np.float64)
+    flat = np.asarray(n_flat, dtype=np.float64)
+    lost_too_many = np.flatnonzero(kept < ratio * flat)
+    first = int(lost_too_many[-1]) + 1 if lost_too_many.size else 0     # the condition holds on grid[first:]
+    populated = np.flatnonzero(flat[first:] > 0)
+    return float(grid[first + int(populated[0])]) if populated.size else None
 
 
 def cost_ratio(N, T, w, p, f_per_template):
