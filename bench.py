@@ -36,6 +36,38 @@ UNIT = "template-seconds/s"
 KERNEL_OF = {"fft": "fft_tma_kernel", "gemm": "gemm_", "stage2": "stage2_score"}
 
 
+KERNEL_SOURCES = ("fft_tma.cu", "gemm_tcgen05.cu", "stage2_bybin.cu", "stage2_kernels.cu", "prep_kernels.cu",
+                  "rbmf_internal.h")
+
+
+def kernel_fingerprint():
+    """sha256 over the DEVICE code of the sources of the hot-path kernels (comments and blank lines dropped, so that a
+    reworded comment does not invalidate a capture).  A committed ncu traffic capture is stamped with it
+    (profiles/traffic_fingerprints.txt: `<csv name> <fingerprint>`); `roofline.traffic` is null when the capture was
+    made from other kernel sources than the ones this run executes.  `python bench.py --kernel-fingerprint` prints it."""
+    import hashlib
+    import re
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2110_13115_b200", "csrc")
+    for name in KERNEL_SOURCES:
+        text = open(os.path.join(csrc, name)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        lines = [re.sub(r"//.*$", "", ln).strip() for ln in text.splitlines()]
+        h.update(name.encode())
+        h.update("\n".join(ln for ln in lines if ln).encode())
+    return h.hexdigest()[:16]
+
+
+def traffic_stamp(csv_name):
+    path = os.path.join(ROOT, "profiles", "traffic_fingerprints.txt")
+    if os.path.exists(path):
+        for ln in open(path):
+            parts = ln.split()
+            if len(parts) >= 2 and parts[0] == csv_name:
+                return parts[1]
+    return None
+
+
 def ncu_traffic(config, w, mode):
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) per stage, read from the ncu launch list
     committed as profiles/traffic_<config>_w<w>_<mode>.csv (an `ncu --csv` log of that very configuration; the .md
@@ -44,6 +76,10 @@ def ncu_traffic(config, w, mode):
     path = os.path.join(ROOT, "profiles", "traffic_%s_w%d_%s.csv" % (config, w, mode))
     if not os.path.exists(path):
         return {}, "no ncu capture committed for (%s, w=%d, %s)" % (config, w, mode)
+    stamp, now = traffic_stamp(os.path.basename(path)), kernel_fingerprint()
+    if stamp != now:
+        return {}, "profiles/%s is stale: captured from kernel sources %s, this build is %s" % (
+            os.path.basename(path), stamp or "(unstamped)", now)
     acc = {}
     with open(path, newline="") as fh:
         rows = [r for r in csv.reader(fh) if len(r) >= 15 and r[0].isdigit()]
@@ -257,13 +293,10 @@ def measure(cfg, args, rdist, rbmf, workloads, torch, device, stream, rank, worl
             elapsed_local = sum(a.elapsed_time(b) for a, b in evs)
         rdist.barrier(device)
         elapsed_ms = rdist.max_over_ranks(elapsed_local, device)
-        # per-kernel durations: the same K steps again, reading the library's CUDA events after every step (this
-        # costs a host round trip per step, which is why it is not done inside the region `value` comes from)
-        for _ in range(steps):
-            if scrub is not None:
-                scrub.fill_(1)
-            plan.filter_async(strain_dev, cfg.thr1, cfg.thr2)
-            ms = plan.stage_ms()                      # waits for this step's last event, reads the stage events
+        # per-kernel durations of the SAME K steps: the library keeps the stage events of its last 64 timed calls
+        # (rbmf_get_stage_ms_history), read here after the region has ended -- no host round trip inside it, so the
+        # stage sums and ms_per_step describe one and the same run (steps > 64: the last 64 of them)
+        for ms in plan.stage_ms_history(min(steps, 64)):
             for key in stage:
                 stage[key].append(ms[key])
         t_wall1 = time.time()
@@ -336,6 +369,29 @@ def measure(cfg, args, rdist, rbmf, workloads, torch, device, stream, rank, worl
                     int(products), "one fp16 product: error-bounded screen, fp32 confirm in kernel 3"
                     if args.gemm == "screen" else "bf16x3 split precision"),
                 "useful_tflops": useful_flops / (gemm_ms * 1e-3) / 1e12, "avg_kernel_ms": gemm_ms}
+    # north_star's OTHER target, kept inside `roofline` so that the driver's record carries it: kernel 1 against the HBM
+    # peak, in algorithmic bytes and in the real DRAM bytes of the committed capture (null when that capture is stale)
+    fft_dram = traffic.get("fft")
+    roofline["fft"] = {"kernel": "fft_tma_kernel (a1-a3)", "bound": "hbm", "unit": "GB/s", "peak": hbm_peak,
+                       "algorithmic_GBps": fft_gbs, "frac": fft_gbs / hbm_peak, "target_frac": 0.70,
+                       "dram_GBps": (fft_dram / (fft_ms * 1e-3) / 1e9) if fft_dram else None,
+                       "dram_frac": (fft_dram / (fft_ms * 1e-3) / 1e9 / hbm_peak) if fft_dram else None,
+                       "traffic": fft_dram, "algorithmic_bytes": fft_alg_bytes, "avg_kernel_ms": fft_ms}
+    # ... and the arithmetic mode this run did NOT use for `value` (separate short pass, one host read per step): with
+    # the default screen that is the literal split-precision GEMM of north_star
+    o_gemm, o_total = other_stage["gemm_ms"], other_stage["total_ms"]
+    o_products = 3.0 if other == "bf16x3" else 1.0
+    o_tflops = o_products * useful_flops / (o_gemm * 1e-3) / 1e12
+    roofline[other] = {"kernel": ("gemm_tcgen05_kernel" if other == "bf16x3" else "gemm_screen_pair_kernel") + " (a4-a5)",
+                       # a short pass of its own (a few steps): judged against the BURST peak whatever the regime of
+                       # the headline region was
+                       "bound": "tensor", "unit": "TFLOP/s", "achieved": o_tflops, "peak": peak_burst,
+                       "frac": o_tflops / peak_burst, "frac_of_sustained_peak": o_tflops / peak_sust,
+                       "avg_kernel_ms": o_gemm, "step_ms": o_total,
+                       "value_in_this_mode": world * cfg.T * seg_seconds / (o_total * 1e-3),
+                       "note": "executed 16-bit MMA flops = %d x 8 T k N/w; step_ms from the library's own events" % int(o_products)}
+    roofline["kernel_fingerprint"] = kernel_fingerprint()
+    roofline["stage_times_from"] = "the timed region itself (library events of its last %d steps)" % len(stage["gemm"])
     # second roofline of kernel 1: its fp32 arithmetic, 5 N log2 N flops per series + 6 per band bin (the paper's count,
     # PAPER.md:236), against 148 SMs x 128 lanes x 2 (FMA) x the SM clock sampled under load
     fft_flops = cfg.k * (5.0 * cfg.N * np.log2(cfg.N) + 6.0 * band)
@@ -583,12 +639,17 @@ def main():
                     help="configs summarised in the `configs` array of the default line ('' = none)")
     ap.add_argument("--summary-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel-fingerprint", action="store_true",
+                    help="print the fingerprint of the hot-path kernel sources (the stamp of a traffic capture) and exit")
     ap.add_argument("--extras", default="batch,routes,bankset,prepare,cufft",
                     help="SURVEY 8(f) rows measured into the `extras` array of the default line: batch (f1: small at "
                          "B=8, paper at B=4), routes (f2: template routes vs GEMM route on small and paper), bankset "
                          "(f3), prepare (f4: preparation kernels on small), cufft (context: the library FFT alone on the same "
                          "sizes); '' = none")
     args = ap.parse_args()
+    if args.kernel_fingerprint:
+        print(kernel_fingerprint())
+        return 0
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     import torch

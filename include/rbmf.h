@@ -309,6 +309,11 @@ rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_p
  * only after rbmf_plan_set_timing(plan, 1). */
 rbmf_status rbmf_plan_set_timing(rbmf_plan* plan, int32_t enabled);
 rbmf_status rbmf_get_stage_ms(rbmf_plan* plan, float ms[4]);
+/* The same for an earlier call: the plan keeps the stage events of its last 64 timed calls, so a loop of up to 64
+ * rbmf_filter calls can be enqueued WITHOUT a host round trip per call and its per-stage times read afterwards.
+ * calls_back = 0 is the last call, 1 the one before, ... (RBMF_ERR_ARG beyond 63, RBMF_ERR_STATE beyond the number of
+ * calls made since rbmf_plan_set_timing, which restarts the history).  Synchronises on the last call. */
+rbmf_status rbmf_get_stage_ms_history(rbmf_plan* plan, int32_t calls_back, float ms[4]);
 
 /* Number of kernels rbmf_filter launches for this plan's configuration. */
 rbmf_status rbmf_launches_per_filter(const rbmf_plan* plan, int32_t* n);

@@ -69,7 +69,9 @@ struct rbmf_plan {
     int template_offset;
     bool have_templates;
     bool have_maps;
-    cudaEvent_t ev[5];
+    cudaEvent_t ev[kEvRing][4];   // stage events of the last kEvRing timed calls (ring; ev_slot = the latest)
+    int ev_slot;
+    long long ev_calls;           // timed calls since timing was switched on
     bool have_events;
 };
 
@@ -398,7 +400,8 @@ rbmf_status rbmf_plan_set_workspace(rbmf_plan* plan, void* dev_ptr, size_t bytes
     if ((s = make_map_rows(plan, &plan->tmB_h16half, plan->ws + L.c_h16, 2 * (uint64_t)plan->Tpad, k2, kGemmTT)) != RBMF_OK) return s;
     CK(gemm_screen_pair_clusters(plan->num_sms, &plan->pair_clusters));
     if (!plan->have_events) {
-        for (int i = 0; i < 5; ++i) CK(cudaEventCreate(&plan->ev[i]));
+        for (int r = 0; r < kEvRing; ++r)
+            for (int i = 0; i < 4; ++i) CK(cudaEventCreate(&plan->ev[r][i]));
         plan->have_events = true;
     }
     plan->have_maps = true;
@@ -461,7 +464,11 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     const int64_t Mplane = plan->M * plan->max_batch;        // rows of the planes
     unsigned long long* counters = at<unsigned long long>(plan, L.counters);
 
-    if (tm) CK(cudaEventRecord(plan->ev[0], st));
+    if (tm) {
+        plan->ev_slot = (plan->ev_slot + 1) % kEvRing;
+        ++plan->ev_calls;
+        CK(cudaEventRecord(plan->ev[plan->ev_slot][0], st));
+    }
     // counters + FFT scheduler words + per-bin histogram
     CK(cudaMemsetAsync(counters, 0, kCounterBytes + L.sched_bytes + (size_t)Mtot * 4, st));
     CK(launch_prep_strain((const float2*)strain_dev, at<float2>(plan, L.dsT), plan->logN1, plan->logN2,
@@ -499,7 +506,7 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     if (screen && !by_templates)
         CK(launch_bin_norm(at<uint16_t>(plan, L.bavg_hi), at<float>(plan, L.bin_norm), (int)Mtot, (int)Mplane,
                            (plan->k + 31) / 32, st));
-    if (tm) CK(cudaEventRecord(plan->ev[1], st));
+    if (tm) CK(cudaEventRecord(plan->ev[plan->ev_slot][1], st));
 
     // ---- kernel 2: a4-a5 over the bins of all segments ------------------------------------------
     GemmArgs g;
@@ -552,7 +559,7 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
         CK(launch_gemm_simt(at<uint16_t>(plan, L.bavg_hi), at<uint16_t>(plan, L.bavg_lo), at<uint16_t>(plan, L.c_hi),
                             at<uint16_t>(plan, L.c_lo), g, (int)Mplane, st));
     }
-    if (tm) CK(cudaEventRecord(plan->ev[2], st));
+    if (tm) CK(cudaEventRecord(plan->ev[plan->ev_slot][2], st));
 
     // ---- kernel 3: a6 (candidates regrouped by bin; one warp per candidate where a bin's block is too large) ----
     Stage2Args s2;
@@ -573,7 +580,7 @@ rbmf_status rbmf_filter_batch(rbmf_plan* plan, const void* strain_dev, int32_t n
     if (s2.smem_bytes > 0 && !plan->diag_stage2_per_cand) CK(launch_stage2_bybin(s2, plan->num_sms, st));
     else CK(launch_stage2(s2, plan->num_sms, st));
     CK(cudaMemcpyAsync(n_out_dev, counters + 1, 8, cudaMemcpyDeviceToDevice, st));
-    if (tm) CK(cudaEventRecord(plan->ev[3], st));
+    if (tm) CK(cudaEventRecord(plan->ev[plan->ev_slot][3], st));
     plan->filtered = true;
     plan->last_nb = nb;
     plan->last_impl = confirm ? (int)RBMF_GEMM_SCREEN : (int)RBMF_GEMM_TCGEN05;
@@ -616,11 +623,15 @@ rbmf_status rbmf_filter_flat(rbmf_plan* plan, const void* strain_dev, float thr,
     cudaStream_t st = plan->stream;
     unsigned long long* counters = at<unsigned long long>(plan, L.counters);
     const bool tm = plan->timing != 0;
-    if (tm) CK(cudaEventRecord(plan->ev[0], st));
+    if (tm) {
+        plan->ev_slot = (plan->ev_slot + 1) % kEvRing;
+        ++plan->ev_calls;
+        CK(cudaEventRecord(plan->ev[plan->ev_slot][0], st));
+    }
     CK(cudaMemsetAsync(counters, 0, kCounterBytes, st));
     CK(launch_prep_strain((const float2*)strain_dev, at<float2>(plan, U.dsT), U.logN1, U.logN2,
                           (float)sqrt(2.0 / (double)plan->N), 1, st));
-    if (tm) { CK(cudaEventRecord(plan->ev[1], st)); CK(cudaEventRecord(plan->ev[2], st)); }
+    if (tm) { CK(cudaEventRecord(plan->ev[plan->ev_slot][1], st)); CK(cudaEventRecord(plan->ev[plan->ev_slot][2], st)); }
     for (int t0 = 0; t0 < plan->T; t0 += U.ncols) {
         CK(launch_layout_basis((const float2*)plan->tm_templates + (size_t)t0 * (size_t)(plan->N / 2 + 1),
                                at<float2>(plan, U.basisP), U.ncols, plan->N / 2 + 1, plan->j_low, U.logN1, U.logN2,
@@ -631,7 +642,7 @@ rbmf_status rbmf_filter_flat(rbmf_plan* plan, const void* strain_dev, float thr,
                           U.ncols, thr * thr, out_dev, counters + 1, (unsigned long long)plan->max_trig, nullptr, st));
     }
     CK(cudaMemcpyAsync(n_out_dev, counters + 1, 8, cudaMemcpyDeviceToDevice, st));
-    if (tm) CK(cudaEventRecord(plan->ev[3], st));
+    if (tm) CK(cudaEventRecord(plan->ev[plan->ev_slot][3], st));
     plan->filtered = true;
     plan->last_nb = 1;
     plan->last_impl = RBMF_GEMM_TCGEN05;   // counters[0] (unused here: 0 candidates) is the final candidate count
@@ -754,19 +765,24 @@ rbmf_status rbmf_get_internal(rbmf_plan* plan, int32_t which, const void** dev_p
 rbmf_status rbmf_plan_set_timing(rbmf_plan* plan, int32_t enabled) {
     if (!plan) return RBMF_ERR_ARG;
     plan->timing = enabled ? 1 : 0;
+    plan->ev_calls = 0;   // the history starts over
     return RBMF_OK;
 }
 
-rbmf_status rbmf_get_stage_ms(rbmf_plan* plan, float ms[4]) {
-    if (!plan || !ms) return RBMF_ERR_ARG;
+rbmf_status rbmf_get_stage_ms_history(rbmf_plan* plan, int32_t calls_back, float ms[4]) {
+    if (!plan || !ms || calls_back < 0 || calls_back >= kEvRing) return RBMF_ERR_ARG;
     if (!plan->filtered || !plan->timing || !plan->have_events) return RBMF_ERR_STATE;
-    CK(cudaEventSynchronize(plan->ev[3]));
-    CK(cudaEventElapsedTime(&ms[0], plan->ev[0], plan->ev[1]));
-    CK(cudaEventElapsedTime(&ms[1], plan->ev[1], plan->ev[2]));
-    CK(cudaEventElapsedTime(&ms[2], plan->ev[2], plan->ev[3]));
-    CK(cudaEventElapsedTime(&ms[3], plan->ev[0], plan->ev[3]));
+    if ((long long)calls_back >= plan->ev_calls) return RBMF_ERR_STATE;   // fewer timed calls than that so far
+    cudaEvent_t* ev = plan->ev[(plan->ev_slot - calls_back + kEvRing) % kEvRing];
+    CK(cudaEventSynchronize(plan->ev[plan->ev_slot][3]));
+    CK(cudaEventElapsedTime(&ms[0], ev[0], ev[1]));
+    CK(cudaEventElapsedTime(&ms[1], ev[1], ev[2]));
+    CK(cudaEventElapsedTime(&ms[2], ev[2], ev[3]));
+    CK(cudaEventElapsedTime(&ms[3], ev[0], ev[3]));
     return RBMF_OK;
 }
+
+rbmf_status rbmf_get_stage_ms(rbmf_plan* plan, float ms[4]) { return rbmf_get_stage_ms_history(plan, 0, ms); }
 
 rbmf_status rbmf_launches_per_filter(const rbmf_plan* plan, int32_t* n) {
     if (!plan || !n) return RBMF_ERR_ARG;
@@ -779,7 +795,8 @@ rbmf_status rbmf_launches_per_filter(const rbmf_plan* plan, int32_t* n) {
 rbmf_status rbmf_plan_destroy(rbmf_plan* plan) {
     if (!plan) return RBMF_ERR_ARG;
     if (plan->have_events)
-        for (int i = 0; i < 5; ++i) cudaEventDestroy(plan->ev[i]);
+        for (int r = 0; r < kEvRing; ++r)
+            for (int i = 0; i < 4; ++i) cudaEventDestroy(plan->ev[r][i]);
     delete plan;
     return RBMF_OK;
 }

@@ -44,6 +44,7 @@ constexpr int kSchedBase = 16;
 //   [0] stage-1 list entries requested by kernel 2, [1] triggers, [2] confirmed candidates (screen mode),
 //   [3] cursor of the by-bin candidate array, [4] stage-2 work items, [5] stage-2 ticket, [8] rbmf_filter_host's count.
 constexpr int kCounterBytes = 128;
+constexpr int kEvRing = 64;         // timed calls whose stage events a plan keeps (rbmf_get_stage_ms_history)
 constexpr int kStage2Chunk = 128;   // candidates per stage-2 work item (one CTA of 4 warps)
 
 // Device views handed to the fused FFT kernel.

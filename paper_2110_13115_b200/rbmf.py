@@ -70,6 +70,7 @@ SIGNATURES = {
     "rbmf_get_internal": (_i32, [_vp, _i32, ctypes.POINTER(_vp), _psz]),
     "rbmf_plan_set_timing": (_i32, [_vp, _i32]),
     "rbmf_get_stage_ms": (_i32, [_vp, ctypes.POINTER(_f32)]),
+    "rbmf_get_stage_ms_history": (_i32, [_vp, _i32, ctypes.POINTER(_f32)]),
     "rbmf_launches_per_filter": (_i32, [_vp, _pi32]),
     "rbmf_plan_destroy": (_i32, [_vp]),
     "rbmf_status_string": (ctypes.c_char_p, [_i32]),
@@ -442,6 +443,16 @@ class Plan:
         ms = (_f32 * 4)()
         self._check(_lib.rbmf_get_stage_ms(self._h, ms), "rbmf_get_stage_ms")
         return {"fft": ms[0], "gemm": ms[1], "stage2": ms[2], "total": ms[3]}
+
+    def stage_ms_history(self, n_calls):
+        """Per-stage times of the last `n_calls` (<= 64) timed calls, oldest first, read after the fact: the calls
+        themselves can be enqueued back to back without a host synchronisation in between."""
+        out = []
+        for back in range(int(n_calls) - 1, -1, -1):
+            ms = (_f32 * 4)()
+            self._check(_lib.rbmf_get_stage_ms_history(self._h, back, ms), "rbmf_get_stage_ms_history")
+            out.append({"fft": ms[0], "gemm": ms[1], "stage2": ms[2], "total": ms[3]})
+        return out
 
     def launches_per_filter(self):
         n = _i32()

@@ -113,6 +113,11 @@ def test_window_capacity_and_workspace_size(binding):
     assert b.rbmf_launches_per_filter(h, ctypes.byref(n)) == b.RBMF_OK and n.value == 6
     assert b.rbmf_diag_set(h, b.RBMF_DIAG_STAGE1_FP32_CHECK, 0) == b.RBMF_OK
     assert b.rbmf_get_screened_count(h, ctypes.byref(ctypes.c_int64())) == b.RBMF_ERR_STATE
+    ms = (ctypes.c_float * 4)()
+    assert b.rbmf_get_stage_ms_history(h, 64, ms) == b.RBMF_ERR_ARG       # the plan keeps 64 timed calls: 0..63
+    assert b.rbmf_get_stage_ms_history(h, -1, ms) == b.RBMF_ERR_ARG
+    assert b.rbmf_get_stage_ms_history(h, 0, None) == b.RBMF_ERR_ARG
+    assert b.rbmf_get_stage_ms_history(h, 0, ms) == b.RBMF_ERR_STATE      # nothing filtered yet
     b.rbmf_plan_destroy(h)
 
 

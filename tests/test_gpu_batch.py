@@ -225,6 +225,42 @@ def test_guarded_calls_repeat_bit_exact(rbmf):
     plan.close()
 
 
+def test_stage_time_history_of_calls_enqueued_back_to_back(rbmf):
+    """rbmf_get_stage_ms_history: 70 timed calls enqueued without a host synchronisation in between; afterwards the
+    plan still has the stage events of the last 64 -- every stage time positive, the parts adding up to the whole
+    (same events), the sum of the per-call totals no longer than the span an outer pair of events measures -- and
+    refuses to go further back than it has calls, or than its ring is long."""
+    import torch
+    wl = workload("mini")
+    strain = torch.from_numpy(wl["strain"]).cuda()
+    plan = make_plan(rbmf, wl)
+    plan.filter_async(strain, 3.0, 4.0)          # untimed call: not part of the history
+    plan.set_timing(True)
+    with pytest.raises(rbmf.RbmfError) as info:
+        plan.stage_ms_history(1)
+    assert info.value.status == rbmf.RBMF_ERR_STATE
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for calls in (5, 70):
+        plan.set_timing(True)                    # restarts the history
+        e0.record(plan.stream)
+        for _ in range(calls):
+            plan.filter_async(strain, 3.0, 4.0)
+        e1.record(plan.stream)
+        plan.stream.synchronize()
+        hist = plan.stage_ms_history(min(calls, 64))
+        assert len(hist) == min(calls, 64)
+        for ms in hist:
+            assert ms["fft"] > 0 and ms["gemm"] > 0 and ms["stage2"] > 0
+            assert abs(ms["fft"] + ms["gemm"] + ms["stage2"] - ms["total"]) < 2e-3
+        assert sum(ms["total"] for ms in hist) <= e0.elapsed_time(e1) * 1.001
+        last = plan.stage_ms()
+        assert last == hist[-1]
+        if calls < 64:
+            with pytest.raises(rbmf.RbmfError):
+                plan.stage_ms_history(calls + 1)
+    plan.close()
+
+
 def test_scheduling_overrides_change_the_order_not_the_result(rbmf):
     """RBMF_DIAG_FFT_CHUNK_MAJOR / _FFT_LOOKAHEAD / _GEMM_GROUP (rbmf_diag_set; environment variables in earlier
     builds) only reorder the work: beta is bit-identical, candidates and triggers are the same sets."""

@@ -138,11 +138,13 @@ def test_paper_scale_sampled(rbmf, impl):
     assert rep["n_mandatory"] > 1000 and crep["n_mandatory"] > 100
 
 
-def test_large_bank_at_its_own_thresholds(rbmf):
+@pytest.mark.parametrize("impl", [SCREEN, X3])
+def test_large_bank_at_its_own_thresholds(rbmf, impl):
     """BASELINE.json configs[3] (N = 262144, k = 256, T = 100000, 100 injections) at 5 / 6: this wide bank answers its
     loud injections with ~2.6e8 candidates and ~8.8e8 triggers; the lists (2^30 records each) stay on the device and
-    only the sampled templates' records are shipped."""
-    rep, crep, nc, nt = run_and_check(rbmf, "large", SCREEN, n_random=64, neighbours=2, max_points=256,
+    only the sampled templates' records are shipped.  Both tensor-core modes: the fp16 screen + fp32 confirm, and the
+    literal bf16x3 GEMM."""
+    rep, crep, nc, nt = run_and_check(rbmf, "large", impl, n_random=64, neighbours=2, max_points=256,
                                       capacity=1 << 30)
     assert nc > 1e8 and nt > 1e8
     assert rep["n_mandatory"] > 1000
@@ -164,6 +166,16 @@ def test_sweep_grid_points(rbmf, name, w, thr1, thr2, capacity):
     assert nc > 0
     if thr1 < 5.0:
         assert rep["n_mandatory"] > 0 and crep["n_mandatory"] > 0
+
+
+@pytest.mark.parametrize("name", [n for n in wlm.SWEEP_NAMES])
+def test_every_sweep_grid_point_at_w8(rbmf, name):
+    """All 15 points of BASELINE.json configs[4] (k in 32..512 x T in 1e3..1e5, N = 2^20, pure noise) at the window the
+    bench times (w = 8), not only the corners: thresholds 3.5 / 4.5 so that noise alone gives non-empty mandatory sets;
+    16 random templates + 16 that reported something + the ragged last one exhaustively, up to 48 triggers pointwise."""
+    rep, crep, nc, nt = run_and_check(rbmf, name, SCREEN, w=8, thr1=3.5, thr2=4.5, n_random=16, neighbours=0,
+                                      max_points=48, capacity=1 << 26, subset_from_triggers=16)
+    assert nc > 0 and rep["n_mandatory"] > 0 and crep["n_mandatory"] > 0
 
 
 def test_k1024_exhaustive(rbmf):
