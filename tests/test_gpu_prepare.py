@@ -17,7 +17,8 @@ def rbmf(built_library):
     return mod
 
 
-@pytest.mark.parametrize("name,k,iterations", [("tiny", 16, 40), ("tiny", 48, 30), ("mini", 32, 40)])
+@pytest.mark.parametrize("name,k,iterations", [("tiny", 16, 40), ("tiny", 48, 30), ("mini", 32, 40),
+                                               ("small", 128, 30)])      # small: the size bench.py's f4 row times
 def test_prepared_basis_against_pca_oracle(rbmf, name, k, iterations):
     import torch
     wl = wlm.make_workload(wlm.CONFIGS[name], device="cuda")
