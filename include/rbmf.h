@@ -24,7 +24,9 @@
  * Conventions
  *  - "dev" pointers are CUDA device memory owned by the caller; "host" pointers are ordinary host memory.
  *  - The library never allocates or frees device memory: the caller provides one workspace
- *    (rbmf_workspace_bytes / rbmf_plan_set_workspace) that must outlive the plan's use.
+ *    (rbmf_workspace_bytes / rbmf_plan_set_workspace) that must outlive the plan's use.  The one entry point that
+ *    needs neither plan nor workspace, rbmf_prepare_strain_static, works out of a fixed 12 MiB array that is part of
+ *    the library image on every GPU (see its description below).
  *  - rbmf_set_basis / rbmf_set_coeffs copy and re-lay-out their inputs into the workspace; the caller's
  *    arrays may be freed after the stream has completed those calls.
  *  - All work is enqueued on the plan's stream (rbmf_set_stream; default: the legacy default stream) and
