@@ -266,7 +266,10 @@ rbmf_status rbmf_bankset_destroy(rbmf_bankset* set);
  * singular values of T).  workspace_dev: 16-byte aligned device memory of rbmf_prepare_basis_workspace_bytes.
  * rbmf_prepare_coeffs: the decomposition coefficients D = T P^H (:167-169), coeffs_out_dev = n_templates x k complex64
  * (c_tk, unconjugated: the input of rbmf_set_coeffs) and sigma_out_dev (n_templates floats or NULL) = ||c_t||_2.
- * fp32 arithmetic with fp64 accumulation across blocks of 512 terms; both calls only enqueue on cuda_stream. */
+ * fp32 arithmetic with fp64 accumulation across blocks of 512 terms; both calls only enqueue on cuda_stream.
+ * Repeatability: the Gram-Schmidt dot products and norms of rbmf_prepare_basis are fp64 sums collected with atomics
+ * from several thread blocks once a row is longer than 4096 entries, so two runs with the same seed agree to fp32
+ * rounding (last-bit differences), not necessarily bit for bit; rbmf_prepare_coeffs is bit-reproducible. */
 rbmf_status rbmf_prepare_basis_workspace_bytes(int32_t n_templates, int32_t k, size_t* bytes);
 rbmf_status rbmf_prepare_basis(const void* templates_dev, int32_t n_templates, int64_t N, double fs, double f_low,
                                int32_t k, int32_t iterations, uint64_t seed, void* workspace_dev, size_t workspace_bytes,
